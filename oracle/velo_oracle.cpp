@@ -1,0 +1,616 @@
+// ORACLE — TEST INFRASTRUCTURE ONLY.
+//
+// Plain, slow, single-threaded-per-event CPU implementation of the VELO pixel hot path of Allen's HLT1
+// (arXiv:1912.09161), written from the paper's statements and the readings listed in DESIGN.md.  It is the
+// parity reference for the CUDA path and the timed CPU baseline of bench.py.  It shares NO code, header,
+// table or helper with paper_1912_09161_b200/csrc: only tests/, __graft_entry__.smoke() and bench.py's
+// cpu_baseline / --impl reference legs may load it.
+//
+// Citations: "P:n" = /root/reference/PAPER.md line n; "D:Rk" = reading k in DESIGN.md §3 (points on which the
+// paper is silent).  Pins for every function below are in tests/test_oracle_*.py (DESIGN.md §4 lists them).
+//   O1 decode            P:153 "Decoding the raw input into coordinates"; raw format v1 D:R1
+//   O2 clustering        P:179 "connected component labeling" -> exact 8-connected components (D:R2), flood fill
+//   O3 centroid/global   P:153 "coordinates in the LHCb global coordinate system"; phi P:183 (D:R3)
+//   O4 phi sort          P:183 "sort hits on every layer by phi" (D:R4)
+//   O5 search by triplet P:181-183 "seeds of three hits from consecutive layers ... extending these to the other
+//                        layers" (D:R5 step-by-step reading T1..T5)
+//   O6 straight-line fit P:149 "tracks in the Velo detector form straight lines" -> unweighted LSQ (D:R6)
+//
+// Build: g++ -O2 -std=c++17 -ffp-contract=off (no fast-math) -shared -fPIC -pthread.
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <thread>
+#include <vector>
+
+namespace {
+
+// ------------------------------------------------------------------------------------------------
+// Inputs
+// ------------------------------------------------------------------------------------------------
+struct Params {  // D:R5 cut values
+  int32_t w_seed_phi16, w_fwd_phi16;
+  float max_slope;
+  float s_seed, s_fwd, s_weak;
+  int32_t max_skipped;
+};
+
+struct Geometry {
+  uint32_t n_sensors, n_modules, n_layers, n_cols, n_rows;
+  float pitch_mm;
+  const uint16_t* sensor_module;
+  const uint16_t* module_layer;
+  const float* sensor_ltg;  // [n_sensors][9]
+  Params params;
+};
+
+enum : uint32_t {
+  STATUS_BAD_HEADER = 1u << 0,
+  STATUS_BAD_SP = 1u << 1,
+  STATUS_TOO_MANY_CLUSTERS = 1u << 2,
+};
+
+// ------------------------------------------------------------------------------------------------
+// O2 helper: membership checksum (D:R2) — sum over the cluster's pixels of mix32(row*n_cols+col), mod 2^32.
+// ------------------------------------------------------------------------------------------------
+uint32_t mix32(uint32_t v) {
+  uint32_t m = (v + 1u) * 2654435761u;
+  m ^= m >> 15;
+  m *= 2246822519u;
+  m ^= m >> 13;
+  return m;
+}
+
+// ------------------------------------------------------------------------------------------------
+// O3: phi as a 16-bit angle.  D:R3 fixes the expression tree: every operation one IEEE-754 binary32
+// round-to-nearest operation, fma = fused.  Polynomial: Abramowitz & Stegun 4.4.49,
+// arctan(t) = t * sum_{k=0..8} a_{2k} t^{2k}, 0 <= t <= 1.
+// ------------------------------------------------------------------------------------------------
+float atan2_poly(float x, float y) {
+  const float a0 = 1.0f, a1 = -0.3333314528f, a2 = 0.1999355085f, a3 = -0.1420889944f, a4 = 0.1065626393f,
+              a5 = -0.0752896400f, a6 = 0.0429096138f, a7 = -0.0161657367f, a8 = 0.0028662257f;
+  float ax = std::fabs(x), ay = std::fabs(y);
+  float mx = ax > ay ? ax : ay, mn = ax > ay ? ay : ax;
+  float t = mx == 0.0f ? 0.0f : mn / mx;
+  float s = t * t;
+  float poly = a8;
+  poly = std::fmaf(poly, s, a7);
+  poly = std::fmaf(poly, s, a6);
+  poly = std::fmaf(poly, s, a5);
+  poly = std::fmaf(poly, s, a4);
+  poly = std::fmaf(poly, s, a3);
+  poly = std::fmaf(poly, s, a2);
+  poly = std::fmaf(poly, s, a1);
+  poly = std::fmaf(poly, s, a0);
+  float p = poly * t;
+  if (ay > ax) p = 1.5707964f - p;
+  if (x < 0.0f) p = 3.1415927f - p;
+  if (y < 0.0f) p = -p;
+  return p;
+}
+
+int16_t phi16_of(float x, float y) {
+  float p = atan2_poly(x, y);
+  float scaled = p * 10430.378f;            // 32768/pi
+  int32_t r = (int32_t)std::nearbyintf(scaled);  // round-half-even (default rounding mode)
+  return (int16_t)(uint16_t)(r & 0xFFFF);   // +32768 wraps to -32768
+}
+
+inline int dphi(int16_t a, int16_t b) { return (int16_t)(uint16_t)((uint16_t)a - (uint16_t)b); }
+
+// ------------------------------------------------------------------------------------------------
+// O5 helper: scatter of candidate c after hits a (older) then b (newer), D:R5.
+// ------------------------------------------------------------------------------------------------
+struct Hit {
+  float x, y, z;
+  int16_t phi;
+};
+
+float scatter(const Hit& a, const Hit& b, const Hit& c) {
+  float dz_ab = b.z - a.z;
+  float tx = (b.x - a.x) / dz_ab;
+  float ty = (b.y - a.y) / dz_ab;
+  float dz = c.z - b.z;
+  float ex = std::fmaf(tx, dz, b.x) - c.x;
+  float ey = std::fmaf(ty, dz, b.y) - c.y;
+  return std::fmaf(ex, ex, ey * ey);
+}
+
+inline uint32_t fbits(float f) {
+  uint32_t u;
+  std::memcpy(&u, &f, 4);
+  return u;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Per-event result
+// ------------------------------------------------------------------------------------------------
+struct Cluster {
+  uint32_t key, n, sum_col, sum_row, checksum;
+  float x, y, z;
+  int16_t phi;
+  uint32_t layer;
+};
+
+struct Track {
+  std::vector<uint32_t> hits;  // event-local cluster indices in the normative order, in order of addition
+  uint32_t seed_key;           // normative index of the seed's middle hit
+  float s_seed;
+  int missed;
+  bool active;
+  float x0, y0, tx, ty;
+};
+
+struct EventResult {
+  uint32_t status = 0;
+  std::vector<Cluster> clusters;             // normative order (layer, phi16, key)
+  std::vector<uint32_t> layer_offsets;       // [n_layers+1]
+  std::vector<uint32_t> pix_key;             // (sensor<<18)|(row*n_cols+col) for every decoded pixel
+  std::vector<uint32_t> pix_cluster;         // its cluster (normative index)
+  std::vector<Track> tracks;                 // accepted tracks, in order of creation
+  uint32_t near_cut = 0;                     // number of decisions within 1e-4 of a cut (D:R7)
+  std::vector<uint32_t> near_cut_hits;       // hits touched by such decisions
+};
+
+struct Scratch {
+  std::vector<int32_t> grid;  // n_cols*n_rows, -1 = empty, -2 = fired/unlabelled, >=0 = cluster id
+};
+
+// ------------------------------------------------------------------------------------------------
+// O1 + O2 + O3 + O4
+// ------------------------------------------------------------------------------------------------
+void cluster_event(const Geometry& g, const uint8_t* raw, size_t bytes, EventResult& out, Scratch& sc) {
+  const uint32_t L = g.n_layers;
+  out.layer_offsets.assign(L + 1, 0);
+  // ---- O1: header and bank table (raw format v1, D:R1)
+  if (bytes < 16 || bytes % 16) { out.status |= STATUS_BAD_HEADER; return; }
+  const uint32_t* w = reinterpret_cast<const uint32_t*>(raw);
+  const size_t n_words = bytes / 4;
+  if (w[0] != 0x56454C4Fu || w[1] != g.n_sensors) { out.status |= STATUS_BAD_HEADER; return; }
+  const uint32_t n_banks = w[1], n_sp_total = w[2];
+  const size_t table_words = ((size_t)n_banks + 1 + 3) / 4 * 4;
+  const size_t sp_words = ((size_t)n_sp_total + 3) / 4 * 4;
+  if (4 + table_words + sp_words != n_words) { out.status |= STATUS_BAD_HEADER; return; }
+  const uint32_t* bank_offset = w + 4;
+  const uint32_t* sp = w + 4 + table_words;
+  if (bank_offset[0] != 0 || bank_offset[n_banks] != n_sp_total) { out.status |= STATUS_BAD_HEADER; return; }
+  for (uint32_t j = 0; j < n_banks; ++j)
+    if (bank_offset[j] > bank_offset[j + 1]) { out.status |= STATUS_BAD_HEADER; return; }
+
+  if (sc.grid.size() != (size_t)g.n_cols * g.n_rows) sc.grid.assign((size_t)g.n_cols * g.n_rows, -1);
+  std::vector<Cluster> clusters;
+  std::vector<uint32_t> pix_key, pix_cluster_unsorted;
+  std::vector<uint32_t> fired;  // pixel indices row*n_cols+col of the current sensor
+  std::vector<uint32_t> stack;
+  for (uint32_t s = 0; s < n_banks; ++s) {
+    // O1: expand every SP word of bank s (= sensor s) into fired pixels.
+    fired.clear();
+    for (uint32_t i = bank_offset[s]; i < bank_offset[s + 1]; ++i) {
+      uint32_t word = sp[i];
+      uint32_t hitmap = word & 0xFF, sp_row = (word >> 8) & 0x3F, sp_col = (word >> 14) & 0x1FF;
+      if (2 * sp_col + 1 >= g.n_cols || 4 * sp_row + 3 >= g.n_rows) { out.status |= STATUS_BAD_SP; continue; }
+      for (uint32_t bit = 0; bit < 8; ++bit) {
+        if (!(hitmap >> bit & 1)) continue;
+        uint32_t col = 2 * sp_col + (bit >> 2), row = 4 * sp_row + (bit & 3);
+        uint32_t idx = row * g.n_cols + col;
+        if (sc.grid[idx] == -1) { sc.grid[idx] = -2; fired.push_back(idx); }  // set semantics: duplicates merge
+      }
+    }
+    // O2: maximal 8-connected components by flood fill.
+    for (uint32_t start : fired) {
+      if (sc.grid[start] != -2) continue;
+      int32_t id = (int32_t)clusters.size();
+      Cluster c{};
+      c.key = 0xFFFFFFFFu;
+      stack.assign(1, start);
+      sc.grid[start] = id;
+      while (!stack.empty()) {
+        uint32_t idx = stack.back();
+        stack.pop_back();
+        uint32_t row = idx / g.n_cols, col = idx % g.n_cols;
+        c.n += 1;
+        c.sum_col += col;
+        c.sum_row += row;
+        c.checksum += mix32(idx);
+        uint32_t k = (s << 18) | idx;
+        if (k < c.key) c.key = k;
+        pix_key.push_back(k);
+        pix_cluster_unsorted.push_back((uint32_t)id);
+        for (int dr = -1; dr <= 1; ++dr)
+          for (int dc = -1; dc <= 1; ++dc) {
+            int r2 = (int)row + dr, c2 = (int)col + dc;
+            if (r2 < 0 || c2 < 0 || r2 >= (int)g.n_rows || c2 >= (int)g.n_cols) continue;
+            uint32_t j = (uint32_t)r2 * g.n_cols + (uint32_t)c2;
+            if (sc.grid[j] == -2) { sc.grid[j] = id; stack.push_back(j); }
+          }
+      }
+      // O3: centroid -> local mm -> global (x,y,z), then phi16 (normative fp32 tree, D:R3).
+      const float* M = g.sensor_ltg + 9 * s;
+      float fc = (float)c.sum_col / (float)c.n + 0.5f;
+      float fr = (float)c.sum_row / (float)c.n + 0.5f;
+      float u = fc * g.pitch_mm, v = fr * g.pitch_mm;
+      c.x = std::fmaf(u, M[0], std::fmaf(v, M[1], M[2]));
+      c.y = std::fmaf(u, M[3], std::fmaf(v, M[4], M[5]));
+      c.z = std::fmaf(u, M[6], std::fmaf(v, M[7], M[8]));
+      c.phi = phi16_of(c.x, c.y);
+      c.layer = g.module_layer[g.sensor_module[s]];
+      clusters.push_back(c);
+    }
+    for (uint32_t idx : fired) sc.grid[idx] = -1;
+  }
+  // O4: normative order = ascending (layer, phi16 signed, key)  (D:R4).
+  std::vector<uint32_t> order(clusters.size());
+  for (uint32_t i = 0; i < order.size(); ++i) order[i] = i;
+  std::sort(order.begin(), order.end(), [&](uint32_t a, uint32_t b) {
+    const Cluster &ca = clusters[a], &cb = clusters[b];
+    if (ca.layer != cb.layer) return ca.layer < cb.layer;
+    if (ca.phi != cb.phi) return ca.phi < cb.phi;
+    return ca.key < cb.key;
+  });
+  std::vector<uint32_t> new_index(clusters.size());
+  out.clusters.resize(clusters.size());
+  for (uint32_t i = 0; i < order.size(); ++i) {
+    out.clusters[i] = clusters[order[i]];
+    new_index[order[i]] = i;
+    out.layer_offsets[out.clusters[i].layer + 1] += 1;
+  }
+  for (uint32_t l = 0; l < L; ++l) out.layer_offsets[l + 1] += out.layer_offsets[l];
+  out.pix_key = pix_key;
+  out.pix_cluster.resize(pix_key.size());
+  for (size_t i = 0; i < pix_key.size(); ++i) out.pix_cluster[i] = new_index[pix_cluster_unsorted[i]];
+  if (out.clusters.size() > 65535) out.status |= STATUS_TOO_MANY_CLUSTERS;
+}
+
+// ------------------------------------------------------------------------------------------------
+// O5: search by triplet (D:R5, steps T1..T5), linear window scans.
+// ------------------------------------------------------------------------------------------------
+struct NearCut {
+  EventResult& out;
+  void touch(uint32_t h) { out.near_cut_hits.push_back(h); }
+  // value against an upper cut: near if |v - cut| <= 1e-4 * cut
+  void cut(float v, float cut, uint32_t h) {
+    if (std::fabs((double)v - (double)cut) <= 1e-4 * std::fabs((double)cut)) { out.near_cut++; touch(h); }
+  }
+  void window(int d, int w, uint32_t h) {
+    int a = std::abs(d);
+    if (a == w || a == w + 1) { out.near_cut++; touch(h); }
+  }
+  // two competing scatter values: near if they differ by <= 1e-4 relative
+  void tie(float s1, float s2, uint32_t h) {
+    double a = s1, b = s2;
+    if (std::fabs(a - b) <= 1e-4 * std::max(a, b)) { out.near_cut++; touch(h); }
+  }
+};
+
+void search_by_triplet(const std::vector<Hit>& hits, const std::vector<uint32_t>& lo, const Params& P,
+                       EventResult& out) {
+  const int L = (int)lo.size() - 1;
+  std::vector<uint8_t> used(hits.size(), 0);
+  std::vector<Track> tracks;  // every track ever created (active or closed), in order of creation
+  NearCut nc{out};
+  struct Choice { bool any; float S; uint32_t c; };
+
+  for (int i = L - 1; i >= 2; --i) {
+    const uint32_t A0 = lo[i], A1 = lo[i + 1], B0 = lo[i - 1], B1 = lo[i], C0 = lo[i - 2], C1 = lo[i - 1];
+
+    // ---- T1 forward: every active track takes best = min (bits(S), c) over the unused hits c of layer C
+    //      inside its phi window and scatter cut.  `used` is not modified until T2 (snapshot).
+    std::vector<Choice> choice(tracks.size(), Choice{false, 0.0f, 0});
+    for (size_t t = 0; t < tracks.size(); ++t) {
+      const Track& T = tracks[t];
+      if (!T.active) continue;
+      const Hit& p = hits[T.hits[T.hits.size() - 2]];  // older
+      const Hit& q = hits[T.hits[T.hits.size() - 1]];  // newest
+      std::vector<float> all_S;
+      for (uint32_t c = C0; c < C1; ++c) {
+        if (used[c]) continue;
+        int d = dphi(hits[c].phi, q.phi);
+        nc.window(d, P.w_fwd_phi16, c);
+        if (std::abs(d) > P.w_fwd_phi16) continue;
+        float S = scatter(p, q, hits[c]);
+        nc.cut(S, P.s_fwd, c);
+        if (!(S <= P.s_fwd)) continue;
+        all_S.push_back(S);
+        Choice& best = choice[t];
+        if (!best.any || fbits(S) < fbits(best.S) || (fbits(S) == fbits(best.S) && c < best.c)) best = {true, S, c};
+      }
+      if (all_S.size() > 1) {  // near-cut bookkeeping only: runner-up within 1e-4 of the winner
+        std::sort(all_S.begin(), all_S.end());
+        nc.tie(all_S[0], all_S[1], choice[t].c);
+      }
+    }
+
+    // ---- T2 resolve: for every hit c chosen by >= 1 track the winner is the track with the minimal
+    //      (bits(S), track_key), track_key = normative index of the seed's middle hit.  The winner appends c;
+    //      every other active track counts a miss and is closed after more than max_skipped misses in a row.
+    std::vector<uint8_t> extended(tracks.size(), 0);
+    for (uint32_t c = C0; c < C1; ++c) {
+      bool any = false;
+      size_t winner = 0;
+      std::vector<float> all_S;
+      for (size_t t = 0; t < tracks.size(); ++t) {
+        if (!tracks[t].active || !choice[t].any || choice[t].c != c) continue;
+        all_S.push_back(choice[t].S);
+        if (!any || fbits(choice[t].S) < fbits(choice[winner].S) ||
+            (fbits(choice[t].S) == fbits(choice[winner].S) && tracks[t].seed_key < tracks[winner].seed_key)) {
+          any = true;
+          winner = t;
+        }
+      }
+      if (!any) continue;
+      if (all_S.size() > 1) { std::sort(all_S.begin(), all_S.end()); nc.tie(all_S[0], all_S[1], c); }
+      tracks[winner].hits.push_back(c);
+      extended[winner] = 1;
+      used[c] = 1;
+    }
+    for (size_t t = 0; t < tracks.size(); ++t) {
+      Track& T = tracks[t];
+      if (!T.active) continue;
+      if (extended[t]) { T.missed = 0; continue; }
+      T.missed += 1;
+      if (T.missed > P.max_skipped) T.active = false;
+    }
+
+    // ---- T3 seed: for every unused middle hit b of layer B, the triplet of b is the argmin over (a, c) of
+    //      (bits(S(a,b,c)), a, c) with a in A, c in C unused, inside the phi windows around b, |slopes(a->b)| <=
+    //      max_slope and S <= s_seed.
+    struct Triplet { uint32_t a, b, c; float S; };
+    std::vector<Triplet> triplets;
+    for (uint32_t b = B0; b < B1; ++b) {
+      if (used[b]) continue;
+      const Hit& hb = hits[b];
+      bool found = false;
+      Triplet best{};
+      std::vector<float> all_S;
+      for (uint32_t a = A0; a < A1; ++a) {
+        if (used[a]) continue;
+        const Hit& ha = hits[a];
+        int da = dphi(ha.phi, hb.phi);
+        nc.window(da, P.w_seed_phi16, a);
+        if (std::abs(da) > P.w_seed_phi16) continue;
+        float dz_ab = hb.z - ha.z;
+        float tx = (hb.x - ha.x) / dz_ab, ty = (hb.y - ha.y) / dz_ab;
+        nc.cut(std::fabs(tx), P.max_slope, a);
+        nc.cut(std::fabs(ty), P.max_slope, a);
+        if (!(std::fabs(tx) <= P.max_slope) || !(std::fabs(ty) <= P.max_slope)) continue;
+        for (uint32_t c = C0; c < C1; ++c) {
+          if (used[c]) continue;
+          int dc = dphi(hits[c].phi, hb.phi);
+          nc.window(dc, P.w_seed_phi16, c);
+          if (std::abs(dc) > P.w_seed_phi16) continue;
+          float S = scatter(ha, hb, hits[c]);
+          nc.cut(S, P.s_seed, b);
+          if (!(S <= P.s_seed)) continue;
+          all_S.push_back(S);
+          bool better = !found || fbits(S) < fbits(best.S) ||
+                        (fbits(S) == fbits(best.S) && (a < best.a || (a == best.a && c < best.c)));
+          if (better) { best = {a, b, c, S}; found = true; }
+        }
+      }
+      if (!found) continue;
+      if (all_S.size() > 1) { std::sort(all_S.begin(), all_S.end()); nc.tie(all_S[0], all_S[1], b); }
+      triplets.push_back(best);
+    }
+
+    // ---- T4 resolve: a triplet is accepted iff it holds the minimal key (bits(S), b) among all triplets (one
+    //      per b) that contain its a, and likewise among all that contain its c.  Accepted -> new active track
+    //      [a, b, c]; rejected triplets vanish and their hits stay free.  (Acceptance depends only on the list
+    //      of triplets, not on `used`, so marking hits here does not make the result order dependent.)
+    for (const Triplet& t : triplets) {
+      const uint64_t key = ((uint64_t)fbits(t.S) << 32) | t.b;
+      bool accepted = true;
+      for (const Triplet& o : triplets) {
+        if (o.b == t.b || (o.a != t.a && o.c != t.c)) continue;
+        nc.tie(t.S, o.S, t.b);
+        const uint64_t okey = ((uint64_t)fbits(o.S) << 32) | o.b;
+        if (okey < key) accepted = false;
+      }
+      if (!accepted) continue;
+      Track T;
+      T.hits = {t.a, t.b, t.c};
+      T.seed_key = t.b;
+      T.s_seed = t.S;
+      T.missed = 0;
+      T.active = true;
+      T.x0 = T.y0 = T.tx = T.ty = 0;
+      tracks.push_back(T);
+      used[t.a] = used[t.b] = used[t.c] = 1;
+    }
+  }
+
+  // ---- T5 finalise: all tracks are closed; >= 4 hits -> output; exactly 3 hits -> output iff S_seed <= s_weak
+  //      (dropped 3-hit tracks keep their hits consumed, which no longer matters after the last iteration).
+  for (Track& T : tracks) {
+    T.active = false;
+    if (T.hits.size() == 3) {
+      nc.cut(T.s_seed, P.s_weak, T.hits[1]);
+      if (!(T.s_seed <= P.s_weak)) continue;
+    }
+    out.tracks.push_back(T);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// O6: unweighted least-squares straight line, x and y separately, reference plane z = 0; fp64 from the fp32 hit
+// coordinates, rounded to fp32 (D:R6).
+// ------------------------------------------------------------------------------------------------
+void fit_line(const std::vector<Hit>& hits, Track& T) {
+  const double n = (double)T.hits.size();
+  double zm = 0, xm = 0, ym = 0;
+  for (uint32_t h : T.hits) { zm += hits[h].z; xm += hits[h].x; ym += hits[h].y; }
+  zm /= n; xm /= n; ym /= n;
+  double szz = 0, szx = 0, szy = 0;
+  for (uint32_t h : T.hits) {
+    double dz = hits[h].z - zm;
+    szz += dz * dz;
+    szx += dz * (hits[h].x - xm);
+    szy += dz * (hits[h].y - ym);
+  }
+  double tx = szx / szz, ty = szy / szz;
+  T.tx = (float)tx;
+  T.ty = (float)ty;
+  T.x0 = (float)(xm - tx * zm);
+  T.y0 = (float)(ym - ty * zm);
+}
+
+void reconstruct_event(const Geometry& g, const uint8_t* raw, size_t bytes, EventResult& out, Scratch& sc) {
+  cluster_event(g, raw, bytes, out, sc);
+  if (out.status & (STATUS_BAD_HEADER | STATUS_TOO_MANY_CLUSTERS)) return;
+  std::vector<Hit> hits(out.clusters.size());
+  for (size_t i = 0; i < hits.size(); ++i) hits[i] = {out.clusters[i].x, out.clusters[i].y, out.clusters[i].z, out.clusters[i].phi};
+  search_by_triplet(hits, out.layer_offsets, g.params, out);
+  for (Track& T : out.tracks) fit_line(hits, T);
+}
+
+struct Run {
+  std::vector<EventResult> events;
+};
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------
+// C interface for ctypes (tests / bench cpu_baseline only)
+// ------------------------------------------------------------------------------------------------
+extern "C" {
+
+uint32_t oracle_mix32(uint32_t v) { return mix32(v); }
+float oracle_atan2_poly(float x, float y) { return atan2_poly(x, y); }
+int32_t oracle_phi16(float x, float y) { return phi16_of(x, y); }
+float oracle_scatter(const float* a, const float* b, const float* c) {
+  Hit ha{a[0], a[1], a[2], 0}, hb{b[0], b[1], b[2], 0}, hc{c[0], c[1], c[2], 0};
+  return scatter(ha, hb, hc);
+}
+
+// Fit one track given its hit coordinates; out = x0, y0, tx, ty.
+void oracle_fit(uint32_t n, const float* x, const float* y, const float* z, float* out4) {
+  std::vector<Hit> hits(n);
+  Track T;
+  for (uint32_t i = 0; i < n; ++i) { hits[i] = {x[i], y[i], z[i], 0}; T.hits.push_back(i); }
+  fit_line(hits, T);
+  out4[0] = T.x0; out4[1] = T.y0; out4[2] = T.tx; out4[3] = T.ty;
+}
+
+void* oracle_run(const Geometry* g, const uint8_t* raw, const uint32_t* event_offsets, uint32_t n_events,
+                 uint32_t n_threads) {
+  Run* run = new Run();
+  run->events.resize(n_events);
+  if (n_threads <= 1) {
+    Scratch sc;
+    for (uint32_t e = 0; e < n_events; ++e)
+      reconstruct_event(*g, raw + event_offsets[e], event_offsets[e + 1] - event_offsets[e], run->events[e], sc);
+  } else {
+    // Contiguous event ranges per thread; every thread runs the unchanged single-threaded code.
+    std::vector<std::thread> pool;
+    for (uint32_t t = 0; t < n_threads; ++t) {
+      uint32_t e0 = (uint64_t)n_events * t / n_threads, e1 = (uint64_t)n_events * (t + 1) / n_threads;
+      pool.emplace_back([=]() {
+        Scratch sc;
+        for (uint32_t e = e0; e < e1; ++e)
+          reconstruct_event(*g, raw + event_offsets[e], event_offsets[e + 1] - event_offsets[e], run->events[e], sc);
+      });
+    }
+    for (auto& th : pool) th.join();
+  }
+  return run;
+}
+
+// Search-by-triplet + fit on caller-given hits of ONE event (already in normative order).
+void* oracle_run_hits(const Params* P, uint32_t n_hits, const float* x, const float* y, const float* z,
+                      const int16_t* phi, uint32_t n_layers, const uint32_t* layer_offsets) {
+  Run* run = new Run();
+  run->events.resize(1);
+  EventResult& out = run->events[0];
+  std::vector<Hit> hits(n_hits);
+  for (uint32_t i = 0; i < n_hits; ++i) hits[i] = {x[i], y[i], z[i], phi[i]};
+  out.layer_offsets.assign(layer_offsets, layer_offsets + n_layers + 1);
+  out.clusters.resize(n_hits);
+  for (uint32_t i = 0; i < n_hits; ++i) {
+    out.clusters[i] = Cluster{};
+    out.clusters[i].x = x[i]; out.clusters[i].y = y[i]; out.clusters[i].z = z[i]; out.clusters[i].phi = phi[i];
+  }
+  search_by_triplet(hits, out.layer_offsets, *P, out);
+  for (Track& T : out.tracks) fit_line(hits, T);
+  return run;
+}
+
+void oracle_free(void* h) { delete (Run*)h; }
+
+// Totals: what = 0 clusters, 1 tracks, 2 track hits, 3 pixels, 4 near-cut hits
+uint64_t oracle_total(void* h, int what) {
+  Run* run = (Run*)h;
+  uint64_t n = 0;
+  for (const EventResult& ev : run->events) {
+    switch (what) {
+      case 0: n += ev.clusters.size(); break;
+      case 1: n += ev.tracks.size(); break;
+      case 2: for (const Track& T : ev.tracks) n += T.hits.size(); break;
+      case 3: n += ev.pix_key.size(); break;
+      case 4: n += ev.near_cut_hits.size(); break;
+    }
+  }
+  return n;
+}
+
+// Flattened, compacted outputs in the layout of the C ABI (include/allen_velo.h), plus oracle-only extras.
+void oracle_export_clusters(void* h, uint32_t n_layers, uint32_t* event_offsets, uint32_t* layer_offsets,
+                            uint32_t* key, uint32_t* n_pixels, uint32_t* sum_col, uint32_t* sum_row, float* x,
+                            float* y, float* z, int16_t* phi16, uint32_t* checksum, uint32_t* status) {
+  Run* run = (Run*)h;
+  uint32_t pos = 0;
+  for (size_t e = 0; e < run->events.size(); ++e) {
+    const EventResult& ev = run->events[e];
+    event_offsets[e] = pos;
+    status[e] = ev.status;
+    for (uint32_t l = 0; l < n_layers; ++l) layer_offsets[e * n_layers + l] = pos + ev.layer_offsets[l];
+    for (const Cluster& c : ev.clusters) {
+      key[pos] = c.key; n_pixels[pos] = c.n; sum_col[pos] = c.sum_col; sum_row[pos] = c.sum_row;
+      x[pos] = c.x; y[pos] = c.y; z[pos] = c.z; phi16[pos] = c.phi; checksum[pos] = c.checksum;
+      ++pos;
+    }
+  }
+  event_offsets[run->events.size()] = pos;
+  layer_offsets[run->events.size() * n_layers] = pos;
+}
+
+void oracle_export_tracks(void* h, uint32_t* event_offsets, uint32_t* hit_offsets, uint16_t* hits, float* x0,
+                          float* y0, float* tx, float* ty) {
+  Run* run = (Run*)h;
+  uint32_t t = 0, hpos = 0;
+  for (size_t e = 0; e < run->events.size(); ++e) {
+    event_offsets[e] = t;
+    for (const Track& T : run->events[e].tracks) {
+      hit_offsets[t] = hpos;
+      for (uint32_t hh : T.hits) hits[hpos++] = (uint16_t)hh;
+      x0[t] = T.x0; y0[t] = T.y0; tx[t] = T.tx; ty[t] = T.ty;
+      ++t;
+    }
+  }
+  event_offsets[run->events.size()] = t;
+  hit_offsets[t] = hpos;
+}
+
+// Pixel membership: for every decoded pixel its key (sensor<<18 | row*n_cols+col), event and cluster (event-local).
+void oracle_export_pixels(void* h, uint32_t* pix_event, uint32_t* pix_key, uint32_t* pix_cluster) {
+  Run* run = (Run*)h;
+  size_t pos = 0;
+  for (size_t e = 0; e < run->events.size(); ++e) {
+    const EventResult& ev = run->events[e];
+    for (size_t i = 0; i < ev.pix_key.size(); ++i) {
+      pix_event[pos] = (uint32_t)e; pix_key[pos] = ev.pix_key[i]; pix_cluster[pos] = ev.pix_cluster[i];
+      ++pos;
+    }
+  }
+}
+
+void oracle_export_near_cut(void* h, uint32_t* per_event_count, uint32_t* hit_event, uint32_t* hit_index) {
+  Run* run = (Run*)h;
+  size_t pos = 0;
+  for (size_t e = 0; e < run->events.size(); ++e) {
+    const EventResult& ev = run->events[e];
+    per_event_count[e] = ev.near_cut;
+    for (uint32_t hh : ev.near_cut_hits) { hit_event[pos] = (uint32_t)e; hit_index[pos] = hh; ++pos; }
+  }
+}
+
+}  // extern "C"
