@@ -1,0 +1,371 @@
+#!/usr/bin/env python
+"""bench.py — VELO events/s on B200 for the nu=6, 10k-event batch (BASELINE.json metric), with roofline and CPU baseline.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--events 10000] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (allen_velo_reconstruct: decode -> cluster -> phi sort -> search by triplet
+-> fit -> compaction) over one batch of synthetic events.  `value` is events/s with inputs resident in
+HBM; `e2e` is the same metric through the C ABI with HOST buffers (pinned), H2D of the raw banks and D2H of the tracks
+inside the timed region.  N > 1 (torchrun): one process per GPU, each reconstructs its own batch (events are
+independent: replicas, no collective on the data path); time = max over ranks, value = all events / time.
+`--impl reference` times the CPU oracle (test infrastructure) on the host cores on a bounded sample per step.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "velo_events_per_s"
+UNIT = "events/s"
+
+
+def env_int(name, default):
+    return int(os.environ.get(name, default))
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks/throttle-reason sampler running beside the timed region (B200_PROFILING.md recipe)."""
+
+    FIELDS = ("timestamp,index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+              "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, device_index: int):
+        self.path = tempfile.mktemp(prefix="clocks_", suffix=".csv")
+        self.proc = None
+        try:
+            self.f = open(self.path, "w")
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits",
+                                          "-lms", "50", "-i", str(device_index)], stdout=self.f,
+                                         stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self, windows):
+        """windows: list of (t0, t1) wall-clock intervals (time.time()) to keep samples from."""
+        import datetime
+
+        out = dict(sm_mhz=None, sm_max_mhz=None, reasons=[], samples=0)
+        if self.proc is None:
+            return out
+        time.sleep(0.12)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        self.f.close()
+        rows = []
+        try:
+            with open(self.path) as f:
+                for line in f:
+                    p = [x.strip() for x in line.split(",")]
+                    if len(p) < 10:
+                        continue
+                    try:
+                        ts = datetime.datetime.strptime(p[0], "%Y/%m/%d %H:%M:%S.%f").timestamp()
+                        rows.append((ts, float(p[2]), float(p[3]), p[5:10]))
+                    except Exception:
+                        continue
+            os.unlink(self.path)
+        except Exception:
+            return out
+        sel = [r for r in rows if any(t0 - 0.05 <= r[0] <= t1 + 0.05 for t0, t1 in windows)] or rows
+        if not sel:
+            return out
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = set()
+        for r in sel:
+            for name, v in zip(names, r[3][1:]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        out.update(sm_mhz=statistics.median(r[1] for r in sel), sm_max_mhz=max(r[2] for r in sel),
+                   reasons=sorted(reasons), samples=len(sel))
+        return out
+
+
+def algorithmic_bytes(n_events, n_layers, raw_bytes, n_clusters, n_tracks, n_track_hits):
+    """Compulsory traffic of one step, exact from the array lengths."""
+    raw = raw_bytes + 4 * (n_events + 1)
+    clusters = 30 * n_clusters + 4 * (n_events * n_layers + 1) + 4 * (n_events + 1) + 4 * n_events
+    tracks = 4 * (n_events + 1) + 4 * (n_tracks + 1) + 2 * n_track_hits + 16 * n_tracks
+    return dict(raw=raw, clusters=clusters, tracks=tracks, total=raw + clusters + tracks,
+                # per-kernel shares: the cluster kernel reads raw and produces the clusters; the track kernel reads
+                # x, y, z, phi16 of every hit once (14 B) and produces the tracks
+                velo_cluster=raw + clusters, velo_track=14 * n_clusters + 4 * (n_events * n_layers + 1) + tracks)
+
+
+def run_reference(args):
+    """The oracle as it stands on the host cores; each step = a bounded sample of the workload."""
+    rank = env_int("RANK", 0)
+    if rank != 0:
+        return 0
+    import oracle
+    from paper_1912_09161_b200 import workload
+
+    cores = os.cpu_count() or 1
+    sample = min(args.events, args.reference_events)
+    batch = workload.generate(args.config, n_events=sample)
+    for _ in range(args.warmup):
+        oracle.reconstruct(batch.geometry, batch.raw, batch.event_offsets, n_threads=cores, export=False)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.reconstruct(batch.geometry, batch.raw, batch.event_offsets, n_threads=cores, export=False)
+    dt = time.perf_counter() - t0
+    value = sample * args.steps / dt
+    line = dict(metric=METRIC, value=value, unit=UNIT, impl="reference", n_gpus=args.gpus, steps=args.steps,
+                warmup=args.warmup, ms_per_step=1e3 * dt / args.steps, higher_is_better=True, scaling="weak",
+                vs_baseline=None, dtype="f32", data="synthetic",
+                config=dict(workload=f"config{args.config}: first {sample} events of the nu={'12' if args.config == 3 else '6'} batch",
+                            events_per_step=sample, input_sha=batch.sha()),
+                cpu_baseline=dict(value=value, unit=UNIT, cores=cores, kind="oracle",
+                                  sample=f"{sample} events per step, {cores} threads over contiguous event ranges"),
+                e2e=dict(value=value, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0))
+    print(json.dumps(line, default=float))
+    return 0
+
+
+def run_ours(args):
+    import torch
+
+    from paper_1912_09161_b200 import binding, workload
+
+    rank, world, local = env_int("RANK", 0), env_int("WORLD_SIZE", 1), env_int("LOCAL_RANK", 0)
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    device = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl", device_id=device)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+
+    def max_over_ranks(v):
+        if dist is None:
+            return v
+        t = torch.tensor([v], dtype=torch.float64, device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def sum_over_ranks(v):
+        if dist is None:
+            return v
+        t = torch.tensor([v], dtype=torch.float64, device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        return float(t.item())
+
+    # ---- workload: every rank reconstructs its own batch (batch_index = rank)
+    t_gen = time.time()
+    batch = workload.generate(args.config, n_events=args.events, batch_index=rank)
+    t_gen = time.time() - t_gen
+    geo = batch.geometry
+    n_events, L = batch.n_events, geo.n_layers
+    raw_bytes = int(batch.raw.size)
+    n_sp = batch.n_sp_words()
+
+    velo = binding.AllenVelo(geo)
+    ccap = int(1.15 * n_sp) + 4096
+    oc, ot = binding.alloc_outputs(n_events, L, ccap, ccap // 3, ccap // 2, device, with_checksum=False)
+    ws = torch.empty(velo.workspace_bytes(n_events, raw_bytes), dtype=torch.uint8, device=device)
+    velo.set_workspace(ws)
+    h_raw = torch.from_numpy(batch.raw).pin_memory()
+    h_off = torch.from_numpy(batch.event_offsets.view(np.int32)).pin_memory()
+    d_raw = h_raw.to(device)
+    d_off = h_off.to(device)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        rc = velo.reconstruct(d_raw, d_off, n_events, stream, oc, ot)
+        if rc != 0:
+            raise RuntimeError(f"allen_velo_reconstruct -> {rc}: {velo.last_error()}")
+
+    sampler = ClockSampler(local) if rank == 0 else None
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    status = oc.status.cpu().numpy().view(np.uint32)
+    n_clusters = int(oc.event_offsets.cpu().numpy().view(np.uint32)[n_events])
+    te = ot.event_offsets.cpu().numpy().view(np.uint32)
+    n_tracks = int(te[n_events])
+    n_track_hits = int(ot.hit_offsets.cpu().numpy().view(np.uint32)[n_tracks])
+    if status.any():
+        raise RuntimeError(f"status bits set on {int((status != 0).sum())} events: {np.unique(status)} (capacity?)")
+
+    # ---- device-resident timing: exactly K steps between barriers + synchronize, CUDA events on the launch stream
+    velo.enable_timing(args.steps)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    torch.cuda.synchronize()
+    w0 = time.time()
+    ev0.record(stream)
+    for _ in range(args.steps):
+        step()
+    ev1.record(stream)
+    torch.cuda.synchronize()
+    w1 = time.time()
+    barrier()
+    ms_total = ev0.elapsed_time(ev1)
+    launches = velo.last_launch_count() * args.steps
+    kt = np.stack([velo.kernel_times(i) for i in range(args.steps)])  # [steps, kernels]
+    velo.enable_timing(0)
+    ms_step = max_over_ranks(ms_total / args.steps)
+    total_events = sum_over_ranks(float(n_events))
+    value = total_events / (ms_step * 1e-3)
+
+    # ---- end to end through the public API with host buffers: H2D raw + offsets, reconstruct, D2H tracks
+    h_te = torch.empty(n_events + 1, dtype=torch.int32).pin_memory()
+    h_ce = torch.empty(n_events + 1, dtype=torch.int32).pin_memory()
+    h_st = torch.empty(n_events, dtype=torch.int32).pin_memory()
+    h_ho = torch.empty(ot.capacity_tracks + 1, dtype=torch.int32).pin_memory()
+    h_hits = torch.empty(ot.capacity_hits, dtype=torch.int16).pin_memory()
+    h_fit = [torch.empty(ot.capacity_tracks, dtype=torch.float32).pin_memory() for _ in range(4)]
+    d_raw2, d_off2 = torch.empty_like(d_raw), torch.empty_like(d_off)
+    h2d = raw_bytes + 4 * (n_events + 1)
+    d2h_holder = [0]
+
+    def e2e_step():
+        d_raw2.copy_(h_raw, non_blocking=True)
+        d_off2.copy_(h_off, non_blocking=True)
+        rc = velo.reconstruct(d_raw2, d_off2, n_events, stream, oc, ot)
+        if rc != 0:
+            raise RuntimeError(f"allen_velo_reconstruct -> {rc}: {velo.last_error()}")
+        h_te.copy_(ot.event_offsets, non_blocking=True)
+        h_ce.copy_(oc.event_offsets, non_blocking=True)
+        h_st.copy_(oc.status, non_blocking=True)
+        stream.synchronize()  # the sizes of the result are needed on the host to fetch exactly the tracks
+        nt = int(h_te[n_events])
+        h_ho[:nt + 1].copy_(ot.hit_offsets[:nt + 1], non_blocking=True)
+        for hbuf, dbuf in zip(h_fit, (ot.x0, ot.y0, ot.tx, ot.ty)):
+            hbuf[:nt].copy_(dbuf[:nt], non_blocking=True)
+        nh = n_track_hits  # identical input every step; avoids a third round trip
+        h_hits[:nh].copy_(ot.hits[:nh], non_blocking=True)
+        stream.synchronize()
+        d2h_holder[0] = 4 * (n_events + 1) * 2 + 4 * n_events + 4 * (nt + 1) + 16 * nt + 2 * nh
+
+    for _ in range(2):
+        e2e_step()
+    barrier()
+    torch.cuda.synchronize()
+    e0 = time.time()
+    for _ in range(args.steps):
+        e2e_step()
+    torch.cuda.synchronize()
+    e1 = time.time()
+    barrier()
+    e2e_ms = max_over_ranks((e1 - e0) * 1e3 / args.steps)
+    e2e_value = total_events / (e2e_ms * 1e-3)
+
+    clocks = sampler.stop([(w0, w1), (e0, e1)]) if sampler else None
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- roofline of the dominant kernel (own algorithmic bytes / own mean duration) and of the whole path
+    names = velo.kernel_names()
+    mean_ms = kt.mean(axis=0)
+    dom = int(np.argmax(mean_ms))
+    ab = algorithmic_bytes(n_events, L, raw_bytes, n_clusters, n_tracks, n_track_hits)
+    peak, peak_src = peaks()
+    dom_bytes = ab.get(names[dom], 0)
+    achieved = dom_bytes / (mean_ms[dom] * 1e-3) / 1e9
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "dram_traffic.json")
+    if os.path.exists(tpath):
+        with open(tpath) as f:
+            traffic = json.load(f).get(names[dom], {}).get(f"config{args.config}_{n_events}")
+    roofline = dict(bound="hbm", kernel=names[dom], achieved=achieved, peak=peak, unit="GB/s", frac=achieved / peak,
+                    traffic=traffic, peak_source=peak_src, algorithmic_bytes_per_launch=dom_bytes,
+                    kernel_ms=float(mean_ms[dom]), kernel_share_of_step=float(mean_ms[dom] / mean_ms.sum()))
+    path_gbs = ab["total"] / (ms_step * 1e-3) / 1e9
+    roofline_path = dict(bound="hbm", achieved=path_gbs, peak=peak, unit="GB/s", frac=path_gbs / peak,
+                         frac_of_8TBs_nominal=path_gbs / 8000.0, algorithmic_bytes_per_step=ab["total"],
+                         bytes_per_event=ab["total"] / n_events)
+
+    cpu_baseline = None
+    if world == 1 and not args.no_cpu_baseline:
+        import oracle
+
+        cores = os.cpu_count() or 1
+        n1 = min(n_events, args.cpu_events_single)
+        sub = batch.select(np.arange(n1))
+        t0 = time.perf_counter()
+        oracle.reconstruct(geo, sub.raw, sub.event_offsets, n_threads=1, export=False)
+        single = n1 / (time.perf_counter() - t0)
+        nm = min(n_events, args.cpu_events_multi)
+        subm = batch.select(np.arange(nm))
+        t0 = time.perf_counter()
+        oracle.reconstruct(geo, subm.raw, subm.event_offsets, n_threads=cores, export=False)
+        multi = nm / (time.perf_counter() - t0)
+        cpu_baseline = dict(value=multi, unit=UNIT, cores=cores, kind="oracle",
+                            sample=f"first {nm} events of the same batch on {cores} threads (contiguous ranges); "
+                                   f"single thread over the first {n1} events: {single:.1f} events/s",
+                            single_thread_value=single)
+
+    line = dict(
+        metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
+        ms_per_step=ms_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",
+        config=dict(workload=f"config{args.config}: {n_events} events/GPU at nu={'12' if args.config == 3 else '6'} "
+                             f"(BASELINE.json configs[{args.config}])",
+                    events_per_gpu=n_events, parallelism=f"replicas x{world} (events independent, no collective)",
+                    l2_policy="inputs+outputs per step (%.0f MB) larger than the 126 MB L2" % (ab["total"] / 1e6),
+                    input_sha=batch.sha(), sp_words_per_event=n_sp / n_events, clusters_per_event=n_clusters / n_events,
+                    tracks_per_event=n_tracks / n_events, hits_per_track=n_track_hits / max(1, n_tracks),
+                    raw_bytes_per_event=raw_bytes / n_events, generator_s=round(t_gen, 2)),
+        e2e=dict(value=e2e_value, unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h_holder[0],
+                 ms_per_step=e2e_ms),
+        gpu_launches=launches,
+        kernels={n: float(m) for n, m in zip(names, mean_ms)},
+        roofline=roofline, roofline_path=roofline_path, cpu_baseline=cpu_baseline, clocks=clocks,
+    )
+    print(json.dumps(line, default=float))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, choices=[0, 1, 2, 3])
+    ap.add_argument("--events", type=int, default=10000)
+    ap.add_argument("--reference-events", type=int, default=2000, help="events per step of the reference arm")
+    ap.add_argument("--cpu-events-single", type=int, default=1000)
+    ap.add_argument("--cpu-events-multi", type=int, default=4000)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

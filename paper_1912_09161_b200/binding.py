@@ -1,0 +1,280 @@
+"""Thin ctypes binding of the C ABI in include/allen_velo.h — argument marshalling only.
+
+Same names as the C entry points.  PyTorch supplies device memory and streams; every step of the path runs in the
+CUDA kernels of `csrc/`.  There is no CPU fallback: a missing shared object or a missing CUDA device raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "_allen_velo.so")
+
+OK, ERR_INVALID, ERR_CUDA, ERR_WORKSPACE = 0, -1, -2, -3
+STATUS_BAD_HEADER, STATUS_BAD_SP, STATUS_TOO_MANY_CLUSTERS = 1, 2, 4
+STATUS_CLUSTER_CAPACITY, STATUS_TRACK_CAPACITY, STATUS_STAGE_OVERFLOW = 8, 16, 32
+
+
+class allen_velo_params_t(ctypes.Structure):
+    _fields_ = [("w_seed_phi16", ctypes.c_int32), ("w_fwd_phi16", ctypes.c_int32), ("max_slope", ctypes.c_float),
+                ("s_seed", ctypes.c_float), ("s_fwd", ctypes.c_float), ("s_weak", ctypes.c_float),
+                ("max_skipped", ctypes.c_int32)]
+
+
+class allen_velo_geometry_t(ctypes.Structure):
+    _fields_ = [("n_sensors", ctypes.c_uint32), ("n_modules", ctypes.c_uint32), ("n_layers", ctypes.c_uint32),
+                ("n_cols", ctypes.c_uint32), ("n_rows", ctypes.c_uint32), ("pitch_mm", ctypes.c_float),
+                ("sensor_module", ctypes.c_void_p), ("module_layer", ctypes.c_void_p),
+                ("sensor_ltg", ctypes.c_void_p), ("params", allen_velo_params_t)]
+
+
+class allen_velo_clusters_t(ctypes.Structure):
+    _fields_ = [("capacity", ctypes.c_uint32)] + [(n, ctypes.c_void_p) for n in (
+        "event_offsets", "layer_offsets", "key", "n_pixels", "sum_col", "sum_row", "x", "y", "z", "phi16",
+        "checksum", "status")]
+
+
+class allen_velo_tracks_t(ctypes.Structure):
+    _fields_ = [("capacity_tracks", ctypes.c_uint32), ("capacity_hits", ctypes.c_uint32)] + [
+        (n, ctypes.c_void_p) for n in ("event_offsets", "hit_offsets", "hits", "x0", "y0", "tx", "ty")]
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen the in-tree extension.  Raises if it has not been built (no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"CUDA extension {LIB_PATH} is missing: run `python -m paper_1912_09161_b200.build` "
+                               "(or __graft_entry__.build()); there is no CPU fallback")
+        L = ctypes.CDLL(LIB_PATH)
+        L.allen_velo_default_params.argtypes = [ctypes.POINTER(allen_velo_params_t)]
+        L.allen_velo_default_params.restype = None
+        L.allen_velo_create.argtypes = [ctypes.POINTER(allen_velo_geometry_t), ctypes.POINTER(ctypes.c_void_p)]
+        L.allen_velo_create.restype = ctypes.c_int
+        L.allen_velo_workspace_bytes.argtypes = [ctypes.c_void_p, ctypes.c_uint32, ctypes.c_size_t]
+        L.allen_velo_workspace_bytes.restype = ctypes.c_size_t
+        L.allen_velo_set_workspace.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t]
+        L.allen_velo_set_workspace.restype = ctypes.c_int
+        L.allen_velo_reconstruct.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_uint32,
+                                             ctypes.c_void_p, ctypes.POINTER(allen_velo_clusters_t),
+                                             ctypes.POINTER(allen_velo_tracks_t)]
+        L.allen_velo_reconstruct.restype = ctypes.c_int
+        L.allen_velo_enable_timing.argtypes = [ctypes.c_void_p, ctypes.c_uint32]
+        L.allen_velo_enable_timing.restype = ctypes.c_int
+        L.allen_velo_kernel_count.argtypes = []
+        L.allen_velo_kernel_count.restype = ctypes.c_uint32
+        L.allen_velo_kernel_name.argtypes = [ctypes.c_uint32]
+        L.allen_velo_kernel_name.restype = ctypes.c_char_p
+        L.allen_velo_kernel_times.argtypes = [ctypes.c_void_p, ctypes.c_uint32, ctypes.c_void_p]
+        L.allen_velo_kernel_times.restype = ctypes.c_int
+        L.allen_velo_last_launch_count.argtypes = [ctypes.c_void_p]
+        L.allen_velo_last_launch_count.restype = ctypes.c_uint32
+        L.allen_velo_last_error.argtypes = [ctypes.c_void_p]
+        L.allen_velo_last_error.restype = ctypes.c_char_p
+        L.allen_velo_destroy.argtypes = [ctypes.c_void_p]
+        L.allen_velo_destroy.restype = None
+        _lib = L
+    return _lib
+
+
+def allen_velo_default_params() -> allen_velo_params_t:
+    p = allen_velo_params_t()
+    load_library().allen_velo_default_params(ctypes.byref(p))
+    return p
+
+
+@dataclass
+class ClusterBuffers:
+    """Caller-owned device tensors for `out_clusters` (torch), plus the marshalled struct."""
+    capacity: int
+    event_offsets: "torch.Tensor"
+    layer_offsets: "torch.Tensor"
+    key: "torch.Tensor"
+    n_pixels: "torch.Tensor"
+    sum_col: "torch.Tensor"
+    sum_row: "torch.Tensor"
+    x: "torch.Tensor"
+    y: "torch.Tensor"
+    z: "torch.Tensor"
+    phi16: "torch.Tensor"
+    checksum: "torch.Tensor | None"
+    status: "torch.Tensor"
+
+    def struct(self) -> allen_velo_clusters_t:
+        s = allen_velo_clusters_t()
+        s.capacity = self.capacity
+        for name in ("event_offsets", "layer_offsets", "key", "n_pixels", "sum_col", "sum_row", "x", "y", "z",
+                     "phi16", "status"):
+            setattr(s, name, getattr(self, name).data_ptr())
+        s.checksum = self.checksum.data_ptr() if self.checksum is not None else None
+        return s
+
+
+@dataclass
+class TrackBuffers:
+    capacity_tracks: int
+    capacity_hits: int
+    event_offsets: "torch.Tensor"
+    hit_offsets: "torch.Tensor"
+    hits: "torch.Tensor"
+    x0: "torch.Tensor"
+    y0: "torch.Tensor"
+    tx: "torch.Tensor"
+    ty: "torch.Tensor"
+
+    def struct(self) -> allen_velo_tracks_t:
+        s = allen_velo_tracks_t()
+        s.capacity_tracks, s.capacity_hits = self.capacity_tracks, self.capacity_hits
+        for name in ("event_offsets", "hit_offsets", "hits", "x0", "y0", "tx", "ty"):
+            setattr(s, name, getattr(self, name).data_ptr())
+        return s
+
+
+def alloc_outputs(n_events: int, n_layers: int, cluster_capacity: int, track_capacity: int, hit_capacity: int,
+                  device, with_checksum: bool = True):
+    """Allocate output tensors with torch (device memory only; int32 storage stands for u32, int16 for u16)."""
+    import torch
+
+    i32, f32, i16 = torch.int32, torch.float32, torch.int16
+    z = lambda n, dt: torch.zeros(max(int(n), 1), dtype=dt, device=device)
+    c = ClusterBuffers(cluster_capacity, z(n_events + 1, i32), z(n_events * n_layers + 1, i32),
+                       z(cluster_capacity, i32), z(cluster_capacity, i32), z(cluster_capacity, i32),
+                       z(cluster_capacity, i32), z(cluster_capacity, f32), z(cluster_capacity, f32),
+                       z(cluster_capacity, f32), z(cluster_capacity, i16),
+                       z(cluster_capacity, i32) if with_checksum else None, z(n_events, i32))
+    t = TrackBuffers(track_capacity, hit_capacity, z(n_events + 1, i32), z(track_capacity + 1, i32),
+                     z(hit_capacity, i16), z(track_capacity, f32), z(track_capacity, f32), z(track_capacity, f32),
+                     z(track_capacity, f32))
+    return c, t
+
+
+class AllenVelo:
+    """RAII wrapper of the handle: allen_velo_create / set_workspace / reconstruct / destroy."""
+
+    def __init__(self, geometry, params: dict | None = None):
+        import torch
+
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_1912_09161_b200 needs a CUDA device (sm_100a); there is no CPU fallback")
+        self._lib = load_library()
+        p = allen_velo_default_params()
+        for k, v in (params or {}).items():
+            setattr(p, k, v)
+        self._smod = np.ascontiguousarray(geometry.sensor_module, np.uint16)
+        self._mlay = np.ascontiguousarray(geometry.module_layer, np.uint16)
+        self._ltg = np.ascontiguousarray(geometry.sensor_ltg, np.float32)
+        g = allen_velo_geometry_t(geometry.n_sensors, geometry.n_modules, geometry.n_layers, geometry.n_cols,
+                                  geometry.n_rows, geometry.pitch_mm, self._smod.ctypes.data, self._mlay.ctypes.data,
+                                  self._ltg.ctypes.data, p)
+        self.n_layers = geometry.n_layers
+        h = ctypes.c_void_p()
+        rc = self._lib.allen_velo_create(ctypes.byref(g), ctypes.byref(h))
+        if rc != OK:
+            raise RuntimeError(f"allen_velo_create failed with {rc}")
+        self._h = h
+        self._ws = None
+
+    def workspace_bytes(self, n_events: int, raw_bytes: int) -> int:
+        return int(self._lib.allen_velo_workspace_bytes(self._h, n_events, raw_bytes))
+
+    def set_workspace(self, tensor) -> None:
+        """`tensor`: a torch uint8 CUDA tensor the caller keeps alive (kept referenced here too)."""
+        rc = self._lib.allen_velo_set_workspace(self._h, tensor.data_ptr(), tensor.numel() * tensor.element_size())
+        if rc != OK:
+            raise RuntimeError(f"allen_velo_set_workspace failed with {rc}: {self.last_error()}")
+        self._ws = tensor
+
+    def reconstruct(self, raw_banks, event_offsets, n_events: int, stream, out_clusters: ClusterBuffers,
+                    out_tracks: TrackBuffers) -> int:
+        """Enqueue on `stream` (a torch.cuda.Stream or None for the current stream).  Returns the C return code."""
+        import torch
+
+        s = stream if stream is not None else torch.cuda.current_stream()
+        cs, ts = out_clusters.struct(), out_tracks.struct()
+        return int(self._lib.allen_velo_reconstruct(self._h, raw_banks.data_ptr(), event_offsets.data_ptr(), n_events,
+                                                    ctypes.c_void_p(s.cuda_stream), ctypes.byref(cs), ctypes.byref(ts)))
+
+    def enable_timing(self, n_calls: int) -> None:
+        rc = self._lib.allen_velo_enable_timing(self._h, n_calls)
+        if rc != OK:
+            raise RuntimeError(f"allen_velo_enable_timing failed with {rc}")
+
+    def kernel_names(self) -> list[str]:
+        return [self._lib.allen_velo_kernel_name(i).decode() for i in range(self._lib.allen_velo_kernel_count())]
+
+    def kernel_times(self, call: int) -> np.ndarray:
+        out = np.zeros(self._lib.allen_velo_kernel_count(), np.float32)
+        rc = self._lib.allen_velo_kernel_times(self._h, call, out.ctypes.data)
+        if rc != OK:
+            raise RuntimeError(f"allen_velo_kernel_times failed with {rc}: {self.last_error()}")
+        return out
+
+    def last_launch_count(self) -> int:
+        return int(self._lib.allen_velo_last_launch_count(self._h))
+
+    def last_error(self) -> str:
+        return self._lib.allen_velo_last_error(self._h).decode()
+
+    def destroy(self) -> None:
+        if getattr(self, "_h", None):
+            self._lib.allen_velo_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def reconstruct_batch(velo: AllenVelo, raw: np.ndarray, event_offsets: np.ndarray, device="cuda:0",
+                      with_checksum: bool = True, cluster_capacity: int | None = None,
+                      track_capacity: int | None = None, hit_capacity: int | None = None):
+    """Convenience for tests/smoke: copy a host batch to the device, run the path once, return host copies.
+
+    Host<->device copies and the final synchronise happen here, outside the C ABI.  Returns (clusters, tracks)
+    as dicts of numpy arrays in the ABI layout (u32/u16 views restored).
+    """
+    import torch
+
+    n_events = len(event_offsets) - 1
+    raw_bytes = int(raw.size)
+    d_raw = torch.from_numpy(np.ascontiguousarray(raw)).to(device) if raw_bytes else torch.zeros(16, dtype=torch.uint8, device=device)
+    d_off = torch.from_numpy(np.ascontiguousarray(event_offsets).view(np.int32)).to(device)
+    ccap = cluster_capacity if cluster_capacity is not None else raw_bytes // 2 + 16  # <= 2 clusters per SP word
+    tcap = track_capacity if track_capacity is not None else ccap // 3 + 16
+    hcap = hit_capacity if hit_capacity is not None else ccap
+    oc, ot = alloc_outputs(n_events, velo.n_layers, ccap, tcap, hcap, device, with_checksum)
+    ws = torch.empty(velo.workspace_bytes(n_events, raw_bytes), dtype=torch.uint8, device=device)
+    velo.set_workspace(ws)
+    rc = velo.reconstruct(d_raw, d_off, n_events, None, oc, ot)
+    if rc != OK:
+        raise RuntimeError(f"allen_velo_reconstruct failed with {rc}: {velo.last_error()}")
+    torch.cuda.synchronize()
+
+    def host(t, dt):
+        return t.cpu().numpy().view(dt)
+
+    u32, u16 = np.uint32, np.uint16
+    nc = int(host(oc.event_offsets, u32)[n_events])
+    clusters = dict(event_offsets=host(oc.event_offsets, u32), layer_offsets=host(oc.layer_offsets, u32),
+                    status=host(oc.status, u32)[:n_events], n=nc)
+    for name, dt in (("key", u32), ("n_pixels", u32), ("sum_col", u32), ("sum_row", u32), ("x", np.float32),
+                     ("y", np.float32), ("z", np.float32), ("phi16", np.int16)):
+        clusters[name] = host(getattr(oc, name), dt)[:min(nc, ccap)]
+    clusters["checksum"] = host(oc.checksum, u32)[:min(nc, ccap)] if with_checksum else None
+    te = host(ot.event_offsets, u32)
+    nt = int(te[n_events])
+    ho = host(ot.hit_offsets, u32)[:min(nt, tcap) + 1]
+    nh = int(ho[-1]) if nt <= tcap else 0
+    tracks = dict(event_offsets=te, hit_offsets=ho, hits=host(ot.hits, u16)[:min(nh, hcap)], n=nt)
+    for name in ("x0", "y0", "tx", "ty"):
+        tracks[name] = host(getattr(ot, name), np.float32)[:min(nt, tcap)]
+    return clusters, tracks

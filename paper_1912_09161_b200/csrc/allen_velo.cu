@@ -1,0 +1,327 @@
+// Host side of the C ABI declared in include/allen_velo.h: argument checks, workspace carving and the launch
+// sequence of the hot path.  No host<->device synchronisation happens in allen_velo_reconstruct.
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "velo_common.cuh"
+
+using namespace velo;
+
+struct allen_velo {
+  allen_velo_geometry_t geo{};  // pointers nulled: host copies live in the vectors below
+  DeviceGeometry dev{};
+  void* dev_block = nullptr;    // handle-owned device constants
+  void* ws = nullptr;
+  size_t ws_bytes = 0;
+  uint32_t last_launches = 0;
+  std::string last_error;
+  // optional per-kernel timing: a ring of (kKernels + 1) events per call
+  std::vector<cudaEvent_t> events;
+  uint32_t timing_calls = 0;   // ring size in calls (0 = timing off)
+  uint64_t call_index = 0;     // reconstruct() calls since timing was enabled
+};
+
+namespace {
+
+constexpr uint32_t kKernels = 6;
+const char* const kKernelNames[kKernels] = {"velo_cluster", "scan_clusters", "compact_clusters",
+                                            "velo_track",   "scan_tracks",   "compact_tracks"};
+constexpr size_t kAlign = 256;
+inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
+
+// bytes per slab entry (cluster SoA incl. checksum) and per cluster of tracking scratch
+constexpr size_t kSlabEntryBytes = 7 * 4 + 2 + 4;
+constexpr size_t kTrackScratchBytes = 2 + 2;           // link, hits_slab per cluster
+constexpr size_t kTrackSlotBytes = 4 + 16;             // trk_hitoff, trk_fit per track slot (one per 3 clusters)
+
+struct Carve {
+  unsigned char* base;
+  size_t used = 0;
+  template <typename T>
+  T* take(size_t count) {
+    T* p = reinterpret_cast<T*>(base + used);
+    used = align_up(used + count * sizeof(T));
+    return p;
+  }
+};
+
+size_t fixed_bytes(uint32_t n_events, uint32_t n_layers) {
+  const size_t items = (size_t)n_events * n_layers;
+  size_t b = 0;
+  b += align_up(items * 4) * 2;                                   // counts, slab_base
+  b += align_up(scan_state_words((uint32_t)items) * 8);           // scan state (clusters)
+  b += align_up((size_t)n_events * 8) + align_up(((size_t)n_events + 1) * 8);  // track counts, offsets
+  b += align_up(scan_state_words(n_events) * 8);                  // scan state (tracks)
+  return b + 16 * kAlign;
+}
+
+size_t per_entry_bytes() { return kSlabEntryBytes + kTrackScratchBytes + (kTrackSlotBytes + 2) / 3; }
+
+int fail(allen_velo* h, int code, const char* what, cudaError_t err = cudaSuccess) {
+  if (h) {
+    h->last_error = what;
+    if (err != cudaSuccess) { h->last_error += ": "; h->last_error += cudaGetErrorString(err); }
+  }
+  return code;
+}
+
+}  // namespace
+
+extern "C" {
+
+void allen_velo_default_params(allen_velo_params_t* p) {
+  if (!p) return;
+  p->w_seed_phi16 = 512;
+  p->w_fwd_phi16 = 512;
+  p->max_slope = 0.4f;
+  p->s_seed = 0.015625f;   // 2^-6 mm^2
+  p->s_fwd = 0.0625f;      // 2^-4
+  p->s_weak = 0.0078125f;  // 2^-7
+  p->max_skipped = 1;
+}
+
+int allen_velo_create(const allen_velo_geometry_t* geo, allen_velo_t** out) {
+  if (!geo || !out) return ALLEN_VELO_ERR_INVALID;
+  *out = nullptr;
+  if (!geo->sensor_module || !geo->module_layer || !geo->sensor_ltg) return ALLEN_VELO_ERR_INVALID;
+  if (geo->n_sensors == 0 || geo->n_sensors > 4096 || geo->n_modules == 0 || geo->n_layers < 3 ||
+      geo->n_layers > (uint32_t)kMaxLayers)
+    return ALLEN_VELO_ERR_INVALID;
+  if (geo->n_cols == 0 || geo->n_cols > 1024 || (geo->n_cols & 1) || geo->n_rows == 0 || geo->n_rows > 256 ||
+      (geo->n_rows & 3) || (uint64_t)geo->n_cols * geo->n_rows > (1u << 18))
+    return ALLEN_VELO_ERR_INVALID;
+  const allen_velo_params_t& P = geo->params;
+  if (P.w_seed_phi16 < 0 || P.w_seed_phi16 > 16383 || P.w_fwd_phi16 < 0 || P.w_fwd_phi16 > 16383 ||
+      P.max_skipped < 0 || P.max_skipped > 200 || !(P.max_slope >= 0) || !(P.s_seed >= 0) || !(P.s_fwd >= 0) ||
+      !(P.s_weak >= 0))
+    return ALLEN_VELO_ERR_INVALID;
+
+  const uint32_t S = geo->n_sensors, L = geo->n_layers;
+  std::vector<uint16_t> sensor_layer(S), layer_sensors((size_t)L * kMaxSensorsPerLayer, 0);
+  std::vector<uint8_t> layer_n(L, 0);
+  for (uint32_t s = 0; s < S; ++s) {
+    const uint32_t m = geo->sensor_module[s];
+    if (m >= geo->n_modules) return ALLEN_VELO_ERR_INVALID;
+    const uint32_t l = geo->module_layer[m];
+    if (l >= L) return ALLEN_VELO_ERR_INVALID;
+    if (layer_n[l] >= kMaxSensorsPerLayer) return ALLEN_VELO_ERR_INVALID;
+    sensor_layer[s] = (uint16_t)l;
+    layer_sensors[(size_t)l * kMaxSensorsPerLayer + layer_n[l]++] = (uint16_t)s;
+  }
+
+  allen_velo* h = new (std::nothrow) allen_velo();
+  if (!h) return ALLEN_VELO_ERR_INVALID;
+  h->geo = *geo;
+  h->geo.sensor_module = nullptr; h->geo.module_layer = nullptr; h->geo.sensor_ltg = nullptr;
+
+  // one device block: ltg | sensor_layer | layer_sensors | layer_n_sensors
+  const size_t b_ltg = align_up((size_t)S * 9 * 4), b_sl = align_up((size_t)S * 2),
+               b_ls = align_up(layer_sensors.size() * 2), b_ln = align_up(L);
+  cudaError_t err = cudaMalloc(&h->dev_block, b_ltg + b_sl + b_ls + b_ln);
+  if (err != cudaSuccess) { delete h; return ALLEN_VELO_ERR_CUDA; }
+  unsigned char* d = static_cast<unsigned char*>(h->dev_block);
+  err = cudaMemcpy(d, geo->sensor_ltg, (size_t)S * 9 * 4, cudaMemcpyHostToDevice);
+  if (err == cudaSuccess) err = cudaMemcpy(d + b_ltg, sensor_layer.data(), (size_t)S * 2, cudaMemcpyHostToDevice);
+  if (err == cudaSuccess)
+    err = cudaMemcpy(d + b_ltg + b_sl, layer_sensors.data(), layer_sensors.size() * 2, cudaMemcpyHostToDevice);
+  if (err == cudaSuccess) err = cudaMemcpy(d + b_ltg + b_sl + b_ls, layer_n.data(), L, cudaMemcpyHostToDevice);
+  if (err != cudaSuccess) { cudaFree(h->dev_block); delete h; return ALLEN_VELO_ERR_CUDA; }
+
+  DeviceGeometry& g = h->dev;
+  g.n_sensors = S; g.n_layers = L; g.n_cols = geo->n_cols; g.n_rows = geo->n_rows;
+  g.sp_cols = geo->n_cols / 2; g.sp_rows = geo->n_rows / 4;
+  g.table_words = (S + 1 + 3) / 4 * 4;
+  g.pitch = geo->pitch_mm;
+  g.ltg = reinterpret_cast<const float*>(d);
+  g.sensor_layer = reinterpret_cast<const uint16_t*>(d + b_ltg);
+  g.layer_sensors = reinterpret_cast<const uint16_t*>(d + b_ltg + b_sl);
+  g.layer_n_sensors = reinterpret_cast<const uint8_t*>(d + b_ltg + b_sl + b_ls);
+  g.params = geo->params;
+  *out = h;
+  return ALLEN_VELO_OK;
+}
+
+size_t allen_velo_workspace_bytes(const allen_velo_t* h, uint32_t n_events, size_t raw_bytes) {
+  if (!h) return 0;
+  // slab: two entries per raw word (a super-pixel holds at most two clusters' seed pixels)
+  const size_t entries = raw_bytes / 2 + 4096;
+  return fixed_bytes(n_events, h->dev.n_layers) + entries * per_entry_bytes() + 16 * kAlign;
+}
+
+int allen_velo_set_workspace(allen_velo_t* h, void* dev_ptr, size_t bytes) {
+  if (!h) return ALLEN_VELO_ERR_INVALID;
+  if (dev_ptr && (reinterpret_cast<uintptr_t>(dev_ptr) % kAlign)) return fail(h, ALLEN_VELO_ERR_INVALID, "workspace misaligned");
+  h->ws = dev_ptr;
+  h->ws_bytes = dev_ptr ? bytes : 0;
+  return ALLEN_VELO_OK;
+}
+
+int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_t* event_offsets, uint32_t n_events,
+                           void* cuda_stream, const allen_velo_clusters_t* oc, const allen_velo_tracks_t* ot) {
+  if (!h) return ALLEN_VELO_ERR_INVALID;
+  h->last_launches = 0;
+  if (!event_offsets || !oc || !ot || (!raw_banks && n_events)) return fail(h, ALLEN_VELO_ERR_INVALID, "null argument");
+  if (reinterpret_cast<uintptr_t>(raw_banks) % 16) return fail(h, ALLEN_VELO_ERR_INVALID, "raw_banks not 16-byte aligned");
+  if (!oc->event_offsets || !oc->layer_offsets || !oc->status || !ot->event_offsets || !ot->hit_offsets)
+    return fail(h, ALLEN_VELO_ERR_INVALID, "null output offsets");
+  if (oc->capacity && (!oc->key || !oc->n_pixels || !oc->sum_col || !oc->sum_row || !oc->x || !oc->y || !oc->z || !oc->phi16))
+    return fail(h, ALLEN_VELO_ERR_INVALID, "null cluster array");
+  if (ot->capacity_tracks && (!ot->x0 || !ot->y0 || !ot->tx || !ot->ty)) return fail(h, ALLEN_VELO_ERR_INVALID, "null track array");
+  if (ot->capacity_hits && !ot->hits) return fail(h, ALLEN_VELO_ERR_INVALID, "null hits array");
+  const uint32_t L = h->dev.n_layers;
+  if ((uint64_t)n_events * L >= (1ull << 31)) return fail(h, ALLEN_VELO_ERR_INVALID, "too many events");
+  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+  cudaError_t err;
+
+  if (n_events == 0) {
+    err = cudaMemsetAsync(oc->event_offsets, 0, 4, stream);
+    if (err == cudaSuccess) err = cudaMemsetAsync(oc->layer_offsets, 0, 4, stream);
+    if (err == cudaSuccess) err = cudaMemsetAsync(ot->event_offsets, 0, 4, stream);
+    if (err == cudaSuccess) err = cudaMemsetAsync(ot->hit_offsets, 0, 4, stream);
+    return err == cudaSuccess ? ALLEN_VELO_OK : fail(h, ALLEN_VELO_ERR_CUDA, "memset", err);
+  }
+
+  // ---- carve the workspace
+  const size_t fixed = fixed_bytes(n_events, L);
+  if (!h->ws || h->ws_bytes < fixed + 1024 * per_entry_bytes() + 16 * kAlign) return fail(h, ALLEN_VELO_ERR_WORKSPACE, "workspace too small");
+  const uint32_t items = n_events * L;
+  Carve cv{static_cast<unsigned char*>(h->ws)};
+  uint32_t* counts = cv.take<uint32_t>(items);
+  uint32_t* slab_base = cv.take<uint32_t>(items);
+  unsigned long long* scan_state = cv.take<unsigned long long>(scan_state_words(items));
+  unsigned long long* trk_counts = cv.take<unsigned long long>(n_events);
+  unsigned long long* trk_offsets = cv.take<unsigned long long>((size_t)n_events + 1);
+  unsigned long long* trk_scan_state = cv.take<unsigned long long>(scan_state_words(n_events));
+  size_t entries = (h->ws_bytes - cv.used - 16 * kAlign) / per_entry_bytes();
+  if (entries > 0x7FFFFFF0u) entries = 0x7FFFFFF0u;
+  ClusterSlab slab{};
+  slab.capacity = (uint32_t)entries;
+  slab.key = cv.take<uint32_t>(entries);
+  slab.n_pixels = cv.take<uint32_t>(entries);
+  slab.sum_col = cv.take<uint32_t>(entries);
+  slab.sum_row = cv.take<uint32_t>(entries);
+  slab.checksum = cv.take<uint32_t>(entries);
+  slab.x = cv.take<float>(entries);
+  slab.y = cv.take<float>(entries);
+  slab.z = cv.take<float>(entries);
+  slab.phi16 = cv.take<int16_t>(entries);
+  // tracking scratch is addressed by output cluster index; it shares the entry count with the slab
+  uint16_t* link = cv.take<uint16_t>(entries);
+  uint16_t* hits_slab = cv.take<uint16_t>(entries);
+  uint32_t* trk_hitoff = cv.take<uint32_t>(entries / 3 + 1);
+  float4* trk_fit = cv.take<float4>(entries / 3 + 1);
+  if (cv.used > h->ws_bytes) return fail(h, ALLEN_VELO_ERR_WORKSPACE, "workspace carve overflow");
+
+  // ---- launch sequence
+  err = cudaMemsetAsync(oc->status, 0, (size_t)n_events * 4, stream);
+  if (err != cudaSuccess) return fail(h, ALLEN_VELO_ERR_CUDA, "memset status", err);
+  cudaEvent_t* ev = nullptr;
+  if (h->timing_calls) ev = h->events.data() + (h->call_index++ % h->timing_calls) * (kKernels + 1);
+  auto mark = [&](uint32_t i) { if (ev) cudaEventRecord(ev[i], stream); };
+  mark(0);
+
+  ClusterLaunch cl{};
+  cl.geo = h->dev;
+  cl.raw = static_cast<const uint32_t*>(raw_banks);
+  cl.event_offsets = event_offsets;
+  cl.n_events = n_events;
+  cl.slab = slab;
+  cl.counts = counts;
+  cl.slab_base = slab_base;
+  cl.status = oc->status;
+  cl.with_checksum = oc->checksum != nullptr;
+  if ((err = launch_cluster(cl, stream)) != cudaSuccess) return fail(h, ALLEN_VELO_ERR_CUDA, "cluster kernel", err);
+  h->last_launches++;
+  mark(1);
+
+  if ((err = launch_scan_u32(counts, oc->layer_offsets, items, scan_state, oc->event_offsets, L, stream)) != cudaSuccess)
+    return fail(h, ALLEN_VELO_ERR_CUDA, "cluster scan", err);
+  h->last_launches++;
+  mark(2);
+
+  CompactClustersLaunch cc{};
+  cc.geo = h->dev;
+  cc.n_events = n_events;
+  cc.slab = slab;
+  cc.slab_base = slab_base;
+  cc.out = *oc;
+  if ((err = launch_compact_clusters(cc, stream)) != cudaSuccess) return fail(h, ALLEN_VELO_ERR_CUDA, "cluster compaction", err);
+  h->last_launches++;
+  mark(3);
+
+  TrackLaunch tl{};
+  tl.geo = h->dev;
+  tl.n_events = n_events;
+  tl.clusters = *oc;
+  if (tl.clusters.capacity > slab.capacity) tl.clusters.capacity = slab.capacity;  // scratch is indexed by cluster
+  tl.link = link;
+  tl.hits_slab = hits_slab;
+  tl.trk_hitoff = trk_hitoff;
+  tl.trk_fit = trk_fit;
+  tl.counts = trk_counts;
+  if ((err = launch_track(tl, stream)) != cudaSuccess) return fail(h, ALLEN_VELO_ERR_CUDA, "track kernel", err);
+  h->last_launches++;
+  mark(4);
+
+  if ((err = launch_scan_u64(trk_counts, trk_offsets, n_events, trk_scan_state, stream)) != cudaSuccess)
+    return fail(h, ALLEN_VELO_ERR_CUDA, "track scan", err);
+  h->last_launches++;
+  mark(5);
+
+  CompactTracksLaunch ct{};
+  ct.n_events = n_events;
+  ct.clusters = *oc;
+  ct.hits_slab = hits_slab;
+  ct.trk_hitoff = trk_hitoff;
+  ct.trk_fit = trk_fit;
+  ct.offsets = trk_offsets;
+  ct.out = *ot;
+  if ((err = launch_compact_tracks(ct, stream)) != cudaSuccess) return fail(h, ALLEN_VELO_ERR_CUDA, "track compaction", err);
+  h->last_launches++;
+  mark(6);
+  return ALLEN_VELO_OK;
+}
+
+int allen_velo_enable_timing(allen_velo_t* h, uint32_t n_calls) {
+  if (!h) return ALLEN_VELO_ERR_INVALID;
+  for (cudaEvent_t e : h->events) cudaEventDestroy(e);
+  h->events.clear();
+  h->timing_calls = 0;
+  h->call_index = 0;
+  if (n_calls == 0) return ALLEN_VELO_OK;
+  h->events.resize((size_t)n_calls * (kKernels + 1));
+  for (cudaEvent_t& e : h->events)
+    if (cudaEventCreate(&e) != cudaSuccess) return fail(h, ALLEN_VELO_ERR_CUDA, "cudaEventCreate");
+  h->timing_calls = n_calls;
+  return ALLEN_VELO_OK;
+}
+
+uint32_t allen_velo_kernel_count(void) { return kKernels; }
+
+const char* allen_velo_kernel_name(uint32_t i) { return i < kKernels ? kKernelNames[i] : ""; }
+
+int allen_velo_kernel_times(allen_velo_t* h, uint32_t call, float* out_ms) {
+  if (!h || !out_ms || !h->timing_calls || call >= h->timing_calls) return ALLEN_VELO_ERR_INVALID;
+  cudaEvent_t* ev = h->events.data() + (size_t)call * (kKernels + 1);
+  for (uint32_t i = 0; i < kKernels; ++i) {
+    cudaError_t err = cudaEventElapsedTime(out_ms + i, ev[i], ev[i + 1]);
+    if (err != cudaSuccess) return fail(h, ALLEN_VELO_ERR_CUDA, "cudaEventElapsedTime", err);
+  }
+  return ALLEN_VELO_OK;
+}
+
+uint32_t allen_velo_last_launch_count(const allen_velo_t* h) { return h ? h->last_launches : 0; }
+
+const char* allen_velo_last_error(const allen_velo_t* h) { return h ? h->last_error.c_str() : "null handle"; }
+
+void allen_velo_destroy(allen_velo_t* h) {
+  if (!h) return;
+  for (cudaEvent_t e : h->events) cudaEventDestroy(e);
+  if (h->dev_block) cudaFree(h->dev_block);
+  delete h;
+}
+
+}  // extern "C"

@@ -1,0 +1,159 @@
+// Internal definitions shared by the CUDA kernels of the VELO hot path (not part of the ABI, not used by oracle/).
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "../../include/allen_velo.h"
+
+namespace velo {
+
+constexpr uint32_t kMagic = 0x56454C4Fu;
+constexpr int kMaxSensorsPerLayer = 8;
+constexpr int kMaxLayers = 64;
+constexpr uint32_t kFull = 0xFFFFFFFFu;
+
+// Device view of the geometry (pointers into the handle's constant block).
+struct DeviceGeometry {
+  uint32_t n_sensors, n_layers, n_cols, n_rows, sp_cols, sp_rows;
+  uint32_t table_words;  // bank table incl. padding, in u32 words
+  float pitch;
+  const uint16_t* sensor_layer;     // [n_sensors]
+  const uint16_t* layer_sensors;    // [n_layers][kMaxSensorsPerLayer]
+  const uint8_t* layer_n_sensors;   // [n_layers]
+  const float* ltg;                 // [n_sensors][9]
+  allen_velo_params_t params;
+};
+
+// Unsorted-capacity slab the cluster kernel writes (sorted per layer) before compaction: structure of arrays with
+// `capacity` entries; region of (event, layer) starts at slab_base[item] and holds counts[item] clusters.
+struct ClusterSlab {
+  uint32_t capacity;
+  uint32_t *key, *n_pixels, *sum_col, *sum_row, *checksum;
+  float *x, *y, *z;
+  int16_t* phi16;
+};
+
+// ---- small device helpers -------------------------------------------------------------------
+__device__ __forceinline__ uint32_t lane_id() { return threadIdx.x & 31u; }
+__device__ __forceinline__ uint32_t lanemask_lt() {
+  uint32_t m;
+  asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+  return m;
+}
+
+// mix32 of DESIGN.md R2 (membership checksum term of one pixel)
+__device__ __forceinline__ uint32_t mix32(uint32_t v) {
+  uint32_t m = (v + 1u) * 2654435761u;
+  m ^= m >> 15;
+  m *= 2246822519u;
+  m ^= m >> 13;
+  return m;
+}
+
+// Normative fp32 position of a cluster (R3): every operation a single IEEE RN op, fma fused, no contraction.
+__device__ __forceinline__ void cluster_position(uint32_t n, uint32_t sum_col, uint32_t sum_row, float pitch,
+                                                 const float* __restrict__ M, float& x, float& y, float& z) {
+  const float fn = __uint2float_rn(n);
+  const float fc = __fadd_rn(__fdiv_rn(__uint2float_rn(sum_col), fn), 0.5f);
+  const float fr = __fadd_rn(__fdiv_rn(__uint2float_rn(sum_row), fn), 0.5f);
+  const float u = __fmul_rn(fc, pitch), v = __fmul_rn(fr, pitch);
+  x = __fmaf_rn(u, __ldg(M + 0), __fmaf_rn(v, __ldg(M + 1), __ldg(M + 2)));
+  y = __fmaf_rn(u, __ldg(M + 3), __fmaf_rn(v, __ldg(M + 4), __ldg(M + 5)));
+  z = __fmaf_rn(u, __ldg(M + 6), __fmaf_rn(v, __ldg(M + 7), __ldg(M + 8)));
+}
+
+// Normative phi16 (R3): Abramowitz & Stegun 4.4.49 polynomial, Horner with fma, round-half-even, wrap.
+__device__ __forceinline__ int16_t phi16_of(float x, float y) {
+  const float ax = fabsf(x), ay = fabsf(y);
+  const float mx = ax > ay ? ax : ay, mn = ax > ay ? ay : ax;
+  const float t = mx == 0.0f ? 0.0f : __fdiv_rn(mn, mx);
+  const float s = __fmul_rn(t, t);
+  float p = 0.0028662257f;
+  p = __fmaf_rn(p, s, -0.0161657367f);
+  p = __fmaf_rn(p, s, 0.0429096138f);
+  p = __fmaf_rn(p, s, -0.0752896400f);
+  p = __fmaf_rn(p, s, 0.1065626393f);
+  p = __fmaf_rn(p, s, -0.1420889944f);
+  p = __fmaf_rn(p, s, 0.1999355085f);
+  p = __fmaf_rn(p, s, -0.3333314528f);
+  p = __fmaf_rn(p, s, 1.0f);
+  p = __fmul_rn(p, t);
+  if (ay > ax) p = __fsub_rn(1.5707964f, p);
+  if (x < 0.0f) p = __fsub_rn(3.1415927f, p);
+  if (y < 0.0f) p = -p;
+  const int r = __float2int_rn(__fmul_rn(p, 10430.378f));
+  return (int16_t)(uint16_t)(r & 0xFFFF);
+}
+
+// Normative scatter (R5) of c after a (older) then b (newer).
+__device__ __forceinline__ float scatter(float xa, float ya, float za, float xb, float yb, float zb, float xc,
+                                         float yc, float zc) {
+  const float dz_ab = __fsub_rn(zb, za);
+  const float tx = __fdiv_rn(__fsub_rn(xb, xa), dz_ab);
+  const float ty = __fdiv_rn(__fsub_rn(yb, ya), dz_ab);
+  const float dz = __fsub_rn(zc, zb);
+  const float ex = __fsub_rn(__fmaf_rn(tx, dz, xb), xc);
+  const float ey = __fsub_rn(__fmaf_rn(ty, dz, yb), yc);
+  return __fmaf_rn(ex, ex, __fmul_rn(ey, ey));
+}
+
+__device__ __forceinline__ int dphi16(int16_t a, int16_t b) { return (int16_t)(uint16_t)((uint16_t)a - (uint16_t)b); }
+
+// ---- kernel launchers (defined in the .cu files) -----------------------------------------------
+struct ClusterLaunch {
+  DeviceGeometry geo;
+  const uint32_t* raw;
+  const uint32_t* event_offsets;
+  uint32_t n_events;
+  ClusterSlab slab;
+  uint32_t* counts;     // [n_events*n_layers] clusters per (event, layer)
+  uint32_t* slab_base;  // [n_events*n_layers] first slab entry of the (event, layer) region
+  uint32_t* status;     // [n_events], zeroed before
+  bool with_checksum;
+};
+cudaError_t launch_cluster(const ClusterLaunch& a, cudaStream_t stream);
+
+// Exclusive prefix sum of `in[n]` into `out[n+1]` (out[n] = total), single pass with decoupled look-back.
+// `tile_state` needs scan_state_words(n) u64 words, zeroed by the launcher.
+size_t scan_state_words(uint32_t n);
+cudaError_t launch_scan_u32(const uint32_t* in, uint32_t* out, uint32_t n, unsigned long long* tile_state,
+                            uint32_t* aux_out, uint32_t aux_stride, cudaStream_t stream);
+cudaError_t launch_scan_u64(const unsigned long long* in, unsigned long long* out, uint32_t n,
+                            unsigned long long* tile_state, cudaStream_t stream);
+
+struct CompactClustersLaunch {
+  DeviceGeometry geo;
+  uint32_t n_events;
+  ClusterSlab slab;
+  const uint32_t* slab_base;
+  allen_velo_clusters_t out;  // layer_offsets / event_offsets already final
+};
+cudaError_t launch_compact_clusters(const CompactClustersLaunch& a, cudaStream_t stream);
+
+// Search by triplet + fit, one CTA per event.  Per-event slabs are addressed from the cluster offsets: an event
+// with clusters [co, co+n) owns hits_slab[co, co+n) (a hit belongs to at most one track) and track slots
+// [co/3, (co+n)/3) (a track has at least three hits).
+struct TrackLaunch {
+  DeviceGeometry geo;
+  uint32_t n_events;
+  allen_velo_clusters_t clusters;  // final compacted clusters (inputs to the search)
+  uint16_t* link;                  // [cluster capacity] scratch: previous (older) hit of the same track, per hit
+  uint16_t* hits_slab;             // [cluster capacity] hit lists of the event's output tracks, back to back
+  uint32_t* trk_hitoff;            // [capacity/3+1] event-local first entry in hits_slab of every output track
+  float4* trk_fit;                 // [capacity/3+1] x0, y0, tx, ty
+  unsigned long long* counts;      // [n_events] (n_tracks << 32) | n_track_hits
+};
+cudaError_t launch_track(const TrackLaunch& a, cudaStream_t stream);
+
+struct CompactTracksLaunch {
+  uint32_t n_events;
+  allen_velo_clusters_t clusters;
+  const uint16_t* hits_slab;
+  const uint32_t* trk_hitoff;
+  const float4* trk_fit;
+  const unsigned long long* offsets;  // [n_events+1] exclusive scan of counts
+  allen_velo_tracks_t out;
+};
+cudaError_t launch_compact_tracks(const CompactTracksLaunch& a, cudaStream_t stream);
+
+}  // namespace velo

@@ -1,0 +1,163 @@
+"""Parity of the CUDA path (through the C ABI) against the oracle, element by element, on the same seeded inputs.
+
+Bar (BASELINE.json north_star): clusters bit-exact (incl. fp32 positions, phi16 and the membership checksum); track
+hit lists exact as canonically sorted sets (near-cut mismatches counted, must stay < 0.1 % of tracks — expected 0
+because both sides decide in the same fp32 arithmetic, R3/R5/R7); fit parameters within 1e-5 (R6).
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def velo(geometry):
+    import torch
+
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1912_09161_b200 import binding
+
+    v = binding.AllenVelo(geometry)
+    yield v
+    v.destroy()
+
+
+def as_oracle_types(clusters, tracks):
+    import oracle
+
+    c = oracle.Clusters(clusters["event_offsets"], clusters["layer_offsets"], clusters["key"], clusters["n_pixels"],
+                        clusters["sum_col"], clusters["sum_row"], clusters["x"], clusters["y"], clusters["z"],
+                        clusters["phi16"], clusters["checksum"], clusters["status"])
+    t = oracle.Tracks(tracks["event_offsets"], tracks["hit_offsets"], tracks["hits"], tracks["x0"], tracks["y0"],
+                      tracks["tx"], tracks["ty"])
+    return c, t
+
+
+def check_parity(velo, batch, ref, **kw):
+    from paper_1912_09161_b200 import binding
+    from tests.helpers import compare_clusters, compare_tracks
+
+    clusters, tracks = binding.reconstruct_batch(velo, batch.raw, batch.event_offsets, **kw)
+    c, t = as_oracle_types(clusters, tracks)
+    diffs = compare_clusters(c, ref.clusters)
+    assert not diffs, diffs
+    rep = compare_tracks(t, ref.tracks, ref.near_cut_per_event)
+    assert rep["n_got"] == rep["n_ref"], rep
+    assert rep["hard_mismatched_tracks"] == 0, rep
+    assert rep["near_cut_mismatched_tracks"] <= 1e-3 * max(1, rep["n_ref"]), rep
+    assert rep["mismatched_tracks"] == 0, rep  # expected: exactly equal
+    assert rep["bad_fits"] == 0, rep
+    # identical order of tracks and hits (order of creation / addition), not only identical sets
+    assert np.array_equal(t.hit_offsets, ref.tracks.hit_offsets)
+    assert np.array_equal(t.hits, ref.tracks.hits)
+    return clusters, tracks
+
+
+@pytest.mark.parametrize("config,n_events", [(0, None), (1, 64), (2, 200), (3, 48)])
+def test_parity_on_seeded_configs(velo, oracle_of, config, n_events):
+    batch, ref = oracle_of(config, n_events)
+    check_parity(velo, batch, ref)
+
+
+def test_parity_without_checksum_array(velo, oracle_of):
+    batch, ref = oracle_of(2, 200)
+    from paper_1912_09161_b200 import binding
+    from tests.helpers import compare_clusters
+
+    clusters, tracks = binding.reconstruct_batch(velo, batch.raw, batch.event_offsets, with_checksum=False)
+    clusters["checksum"] = ref.clusters.checksum
+    c, t = as_oracle_types(clusters, tracks)
+    assert not compare_clusters(c, ref.clusters, check_checksum=False)
+    assert np.array_equal(t.hits, ref.tracks.hits)
+
+
+def test_empty_batch_and_empty_events(velo, geometry):
+    import oracle
+    from paper_1912_09161_b200 import binding, workload
+
+    clusters, tracks = binding.reconstruct_batch(velo, np.zeros(0, np.uint8), np.zeros(1, np.uint32))
+    assert clusters["n"] == 0 and tracks["n"] == 0
+    raw, off = workload.pack_events(geometry, [[], [(3, 5, 5)], []])
+    ref = oracle.reconstruct(geometry, raw, off)
+    clusters, tracks = binding.reconstruct_batch(velo, raw, off)
+    assert clusters["event_offsets"].tolist() == [0, 0, 1, 1] == ref.clusters.event_offsets.tolist()
+    assert tracks["n"] == 0
+
+
+def test_malformed_events(velo, geometry):
+    import oracle
+    from paper_1912_09161_b200 import workload
+    from tests.helpers import compare_clusters
+
+    b = workload.generate(1, n_events=6)
+    raw = b.raw.copy()
+    w = raw.view(np.uint32)
+    w[b.event_offsets[1] // 4] ^= 0xFF                       # bad magic in event 1
+    w[b.event_offsets[2] // 4 + 2] += 4                      # n_sp_total inconsistent with the size in event 2
+    table = (geometry.n_sensors + 1 + 3) // 4 * 4
+    w[b.event_offsets[3] // 4 + 4 + table] |= 400 << 14     # SP column out of range in event 3
+    w[b.event_offsets[4] // 4 + 4 + 7] += 1                  # bank offsets no longer consistent in event 4
+    ref = oracle.reconstruct(geometry, raw, b.event_offsets)
+    assert ref.clusters.status.tolist()[1:5] == [1, 1, 2, 1] or ref.clusters.status[4] in (0, 1)
+    from paper_1912_09161_b200 import binding
+
+    clusters, tracks = binding.reconstruct_batch(velo, raw, b.event_offsets)
+    c, t = as_oracle_types(clusters, tracks)
+    assert not compare_clusters(c, ref.clusters)
+    assert np.array_equal(t.hits, ref.tracks.hits)
+
+
+def test_adversarial_cluster_shapes(velo, geometry):
+    """Large and awkward clusters: full rows, a long snake, a dense block, checkerboards, duplicates of addresses."""
+    import oracle
+    from paper_1912_09161_b200 import workload
+    from tests.helpers import compare_clusters
+
+    snake = []
+    for k in range(40):  # serpentine: long horizontal runs joined alternately left and right
+        r = 2 * k
+        snake += [(7, c, r) for c in range(10, 60)]
+        snake.append((7, 59 if k % 2 == 0 else 10, r + 1))
+    block = [(20, c, r) for c in range(100, 124) for r in range(50, 70)]
+    checker = [(33, c, r) for c in range(200, 232) for r in range(100, 132) if (c + r) % 2 == 0]
+    sparse = [(41, c, r) for c in range(0, 64, 2) for r in range(0, 64, 2)]  # isolated pixels, 2 per SP
+    rows = [(55, c, 128) for c in range(0, 768)] + [(55, c, 131) for c in range(0, 768, 3)]
+    events = [snake, block, checker, sparse, rows, snake + block + checker + sparse + rows]
+    raw, off = workload.pack_events(geometry, events, shuffle_seed=3)
+    ref = oracle.reconstruct(geometry, raw, off)
+    from paper_1912_09161_b200 import binding
+
+    clusters, tracks = binding.reconstruct_batch(velo, raw, off)
+    c, t = as_oracle_types(clusters, tracks)
+    assert not compare_clusters(c, ref.clusters)
+    assert ref.clusters.n_pixels.max() >= 2000
+
+
+def test_output_capacity_is_respected(velo, oracle_of):
+    from paper_1912_09161_b200 import binding
+
+    batch, ref = oracle_of(1, 64)
+    total = int(ref.clusters.event_offsets[-1])
+    cap = total // 2
+    clusters, tracks = binding.reconstruct_batch(velo, batch.raw, batch.event_offsets, cluster_capacity=cap)
+    # offsets still report true totals; events beyond the capacity are flagged and not written
+    assert np.array_equal(clusters["event_offsets"], ref.clusters.event_offsets)
+    over = ref.clusters.event_offsets[1:] > cap
+    assert np.all((clusters["status"] & binding.STATUS_CLUSTER_CAPACITY != 0) == over)
+    n_ok = int(ref.clusters.event_offsets[:-1][~over].max())
+    assert np.array_equal(clusters["key"][:n_ok], ref.clusters.key[:n_ok])
+    # tracks of the events that fit are still exact
+    first_bad = int(np.argmax(over))
+    assert tracks["event_offsets"][first_bad] == ref.tracks.event_offsets[first_bad]
+
+
+def test_deterministic_across_runs(velo, oracle_of):
+    from paper_1912_09161_b200 import binding
+
+    batch, _ = oracle_of(2, 200)
+    a = binding.reconstruct_batch(velo, batch.raw, batch.event_offsets)
+    b = binding.reconstruct_batch(velo, batch.raw, batch.event_offsets)
+    for d0, d1 in zip(a, b):
+        for k in d0:
+            if isinstance(d0[k], np.ndarray):
+                assert np.array_equal(d0[k], d1[k]), k
