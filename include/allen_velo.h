@@ -34,7 +34,7 @@ extern "C" {
 #define ALLEN_VELO_STATUS_BAD_HEADER 1u         /* magic / bank count / sizes / offsets inconsistent: event skipped */
 #define ALLEN_VELO_STATUS_BAD_SP 2u             /* an SP word addressed a pixel outside the sensor: word ignored */
 #define ALLEN_VELO_STATUS_TOO_MANY_CLUSTERS 4u  /* > 65535 clusters: clusters written, tracking skipped */
-#define ALLEN_VELO_STATUS_CLUSTER_CAPACITY 8u   /* out_clusters.capacity exceeded: this event's clusters not written */
+#define ALLEN_VELO_STATUS_CLUSTER_CAPACITY 8u   /* out_clusters.capacity exceeded: layers of this event that do not fit are not written */
 #define ALLEN_VELO_STATUS_TRACK_CAPACITY 16u    /* out_tracks capacities exceeded: this event's tracks not written */
 #define ALLEN_VELO_STATUS_STAGE_OVERFLOW 32u    /* an on-chip staging capacity was exceeded: event incomplete */
 

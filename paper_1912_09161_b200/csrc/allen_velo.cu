@@ -17,6 +17,7 @@ struct allen_velo {
   void* ws = nullptr;
   size_t ws_bytes = 0;
   uint32_t last_launches = 0;
+  uint32_t n_mid_sms = 0;      // SM ids the mid-slot pool of the cluster kernel covers
   std::string last_error;
   // optional per-kernel timing: a ring of (kKernels + 1) events per call
   std::vector<cudaEvent_t> events;
@@ -26,16 +27,14 @@ struct allen_velo {
 
 namespace {
 
-constexpr uint32_t kKernels = 6;
-const char* const kKernelNames[kKernels] = {"velo_cluster", "scan_clusters", "compact_clusters",
-                                            "velo_track",   "scan_tracks",   "compact_tracks"};
+constexpr uint32_t kKernels = 4;  // timed segments; velo_track is three launches (one per staging capacity)
+const char* const kKernelNames[kKernels] = {"velo_cluster", "velo_track", "scan_tracks", "compact_tracks"};
 constexpr size_t kAlign = 256;
 inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
-// bytes per slab entry (cluster SoA incl. checksum) and per cluster of tracking scratch
-constexpr size_t kSlabEntryBytes = 7 * 4 + 2 + 4;
-constexpr size_t kTrackScratchBytes = 2 + 2;           // link, hits_slab per cluster
-constexpr size_t kTrackSlotBytes = 4 + 16;             // trk_hitoff, trk_fit per track slot (one per 3 clusters)
+// tracking scratch per cluster (link, hits_slab) and per track slot (trk_hitoff, trk_fit; one slot per 3 clusters)
+constexpr size_t kTrackScratchBytes = 2 + 2;
+constexpr size_t kTrackSlotBytes = 4 + 16;
 
 struct Carve {
   unsigned char* base;
@@ -48,17 +47,22 @@ struct Carve {
   }
 };
 
-size_t fixed_bytes(uint32_t n_events, uint32_t n_layers) {
-  const size_t items = (size_t)n_events * n_layers;
+// Pool slots for layers that exceed the cluster kernel's shared memory (velo_cluster.cu): sized with the batch.
+uint32_t big_slots(uint32_t items) { return 16 + items / 4096; }
+
+size_t fixed_bytes(uint32_t n_events, uint32_t n_layers, uint32_t n_mid_sms) {
+  const uint32_t items = n_events * n_layers;
   size_t b = 0;
-  b += align_up(items * 4) * 2;                                   // counts, slab_base
-  b += align_up(scan_state_words((uint32_t)items) * 8);           // scan state (clusters)
+  b += align_up(((size_t)items + 1) * 8 + (size_t)n_mid_sms * 4);  // look-back state, big-pool counter, mid masks
+  b += align_up((size_t)n_mid_sms * 32 * cluster_mid_slot_bytes());
+  b += align_up((size_t)big_slots(items) * cluster_big_slot_bytes());
   b += align_up((size_t)n_events * 8) + align_up(((size_t)n_events + 1) * 8);  // track counts, offsets
   b += align_up(scan_state_words(n_events) * 8);                  // scan state (tracks)
+  b += align_up(n_events);                                        // track kernel instance per event
   return b + 16 * kAlign;
 }
 
-size_t per_entry_bytes() { return kSlabEntryBytes + kTrackScratchBytes + (kTrackSlotBytes + 2) / 3; }
+size_t per_entry_bytes() { return kTrackScratchBytes + (kTrackSlotBytes + 2) / 3; }
 
 int fail(allen_velo* h, int code, const char* what, cudaError_t err = cudaSuccess) {
   if (h) {
@@ -130,6 +134,11 @@ int allen_velo_create(const allen_velo_geometry_t* geo, allen_velo_t** out) {
   if (err == cudaSuccess) err = cudaMemcpy(d + b_ltg + b_sl + b_ls, layer_n.data(), L, cudaMemcpyHostToDevice);
   if (err != cudaSuccess) { cudaFree(h->dev_block); delete h; return ALLEN_VELO_ERR_CUDA; }
 
+  int dev = 0, n_sm = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n_sm <= 0) {
+    cudaFree(h->dev_block); delete h; return ALLEN_VELO_ERR_CUDA;
+  }
+  h->n_mid_sms = (uint32_t)n_sm + 16;  // %smid is below the SM count on the parts seen; margin for gaps in the numbering
   DeviceGeometry& g = h->dev;
   g.n_sensors = S; g.n_layers = L; g.n_cols = geo->n_cols; g.n_rows = geo->n_rows;
   g.sp_cols = geo->n_cols / 2; g.sp_rows = geo->n_rows / 4;
@@ -146,9 +155,9 @@ int allen_velo_create(const allen_velo_geometry_t* geo, allen_velo_t** out) {
 
 size_t allen_velo_workspace_bytes(const allen_velo_t* h, uint32_t n_events, size_t raw_bytes) {
   if (!h) return 0;
-  // slab: two entries per raw word (a super-pixel holds at most two clusters' seed pixels)
+  // tracking scratch: two entries per raw word (a super-pixel holds at most two clusters)
   const size_t entries = raw_bytes / 2 + 4096;
-  return fixed_bytes(n_events, h->dev.n_layers) + entries * per_entry_bytes() + 16 * kAlign;
+  return fixed_bytes(n_events, h->dev.n_layers, h->n_mid_sms) + entries * per_entry_bytes() + 16 * kAlign;
 }
 
 int allen_velo_set_workspace(allen_velo_t* h, void* dev_ptr, size_t bytes) {
@@ -185,30 +194,23 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   }
 
   // ---- carve the workspace
-  const size_t fixed = fixed_bytes(n_events, L);
+  const size_t fixed = fixed_bytes(n_events, L, h->n_mid_sms);
   if (!h->ws || h->ws_bytes < fixed + 1024 * per_entry_bytes() + 16 * kAlign) return fail(h, ALLEN_VELO_ERR_WORKSPACE, "workspace too small");
   const uint32_t items = n_events * L;
   Carve cv{static_cast<unsigned char*>(h->ws)};
-  uint32_t* counts = cv.take<uint32_t>(items);
-  uint32_t* slab_base = cv.take<uint32_t>(items);
-  unsigned long long* scan_state = cv.take<unsigned long long>(scan_state_words(items));
+  // look-back words, then one word for the big-pool counter, then the mid masks: zeroed by one memset
+  const size_t state_bytes = ((size_t)items + 1) * 8 + (size_t)h->n_mid_sms * 4;
+  unsigned long long* state = reinterpret_cast<unsigned long long*>(cv.take<unsigned char>(state_bytes));
+  const uint32_t n_big = big_slots(items);
+  unsigned char* mid_pool = cv.take<unsigned char>((size_t)h->n_mid_sms * 32 * cluster_mid_slot_bytes());
+  unsigned char* big_pool = cv.take<unsigned char>((size_t)n_big * cluster_big_slot_bytes());
   unsigned long long* trk_counts = cv.take<unsigned long long>(n_events);
   unsigned long long* trk_offsets = cv.take<unsigned long long>((size_t)n_events + 1);
   unsigned long long* trk_scan_state = cv.take<unsigned long long>(scan_state_words(n_events));
+  uint8_t* trk_level = cv.take<uint8_t>(n_events);
   size_t entries = (h->ws_bytes - cv.used - 16 * kAlign) / per_entry_bytes();
   if (entries > 0x7FFFFFF0u) entries = 0x7FFFFFF0u;
-  ClusterSlab slab{};
-  slab.capacity = (uint32_t)entries;
-  slab.key = cv.take<uint32_t>(entries);
-  slab.n_pixels = cv.take<uint32_t>(entries);
-  slab.sum_col = cv.take<uint32_t>(entries);
-  slab.sum_row = cv.take<uint32_t>(entries);
-  slab.checksum = cv.take<uint32_t>(entries);
-  slab.x = cv.take<float>(entries);
-  slab.y = cv.take<float>(entries);
-  slab.z = cv.take<float>(entries);
-  slab.phi16 = cv.take<int16_t>(entries);
-  // tracking scratch is addressed by output cluster index; it shares the entry count with the slab
+  // tracking scratch is addressed by output cluster index
   uint16_t* link = cv.take<uint16_t>(entries);
   uint16_t* hits_slab = cv.take<uint16_t>(entries);
   uint32_t* trk_hitoff = cv.take<uint32_t>(entries / 3 + 1);
@@ -217,7 +219,8 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
 
   // ---- launch sequence
   err = cudaMemsetAsync(oc->status, 0, (size_t)n_events * 4, stream);
-  if (err != cudaSuccess) return fail(h, ALLEN_VELO_ERR_CUDA, "memset status", err);
+  if (err == cudaSuccess) err = cudaMemsetAsync(state, 0, state_bytes, stream);
+  if (err != cudaSuccess) return fail(h, ALLEN_VELO_ERR_CUDA, "memset", err);
   cudaEvent_t* ev = nullptr;
   if (h->timing_calls) ev = h->events.data() + (h->call_index++ % h->timing_calls) * (kKernels + 1);
   auto mark = [&](uint32_t i) { if (ev) cudaEventRecord(ev[i], stream); };
@@ -228,48 +231,39 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   cl.raw = static_cast<const uint32_t*>(raw_banks);
   cl.event_offsets = event_offsets;
   cl.n_events = n_events;
-  cl.slab = slab;
-  cl.counts = counts;
-  cl.slab_base = slab_base;
-  cl.status = oc->status;
+  cl.out = *oc;
+  cl.state = state;
+  cl.big_ctr = reinterpret_cast<uint32_t*>(state + items);
+  cl.mid_mask = reinterpret_cast<uint32_t*>(state + items + 1);
+  cl.mid_pool = mid_pool;
+  cl.big_pool = big_pool;
+  cl.n_mid_sms = h->n_mid_sms;
+  cl.n_big_slots = n_big;
   cl.with_checksum = oc->checksum != nullptr;
   if ((err = launch_cluster(cl, stream)) != cudaSuccess) return fail(h, ALLEN_VELO_ERR_CUDA, "cluster kernel", err);
   h->last_launches++;
   mark(1);
 
-  if ((err = launch_scan_u32(counts, oc->layer_offsets, items, scan_state, oc->event_offsets, L, stream)) != cudaSuccess)
-    return fail(h, ALLEN_VELO_ERR_CUDA, "cluster scan", err);
-  h->last_launches++;
-  mark(2);
-
-  CompactClustersLaunch cc{};
-  cc.geo = h->dev;
-  cc.n_events = n_events;
-  cc.slab = slab;
-  cc.slab_base = slab_base;
-  cc.out = *oc;
-  if ((err = launch_compact_clusters(cc, stream)) != cudaSuccess) return fail(h, ALLEN_VELO_ERR_CUDA, "cluster compaction", err);
-  h->last_launches++;
-  mark(3);
-
   TrackLaunch tl{};
   tl.geo = h->dev;
   tl.n_events = n_events;
   tl.clusters = *oc;
-  if (tl.clusters.capacity > slab.capacity) tl.clusters.capacity = slab.capacity;  // scratch is indexed by cluster
+  if (tl.clusters.capacity > entries) tl.clusters.capacity = (uint32_t)entries;  // scratch is indexed by cluster
   tl.link = link;
   tl.hits_slab = hits_slab;
   tl.trk_hitoff = trk_hitoff;
   tl.trk_fit = trk_fit;
   tl.counts = trk_counts;
-  if ((err = launch_track(tl, stream)) != cudaSuccess) return fail(h, ALLEN_VELO_ERR_CUDA, "track kernel", err);
-  h->last_launches++;
-  mark(4);
+  tl.level = trk_level;
+  uint32_t n_track_launches = 0;
+  if ((err = launch_track(tl, stream, &n_track_launches)) != cudaSuccess) return fail(h, ALLEN_VELO_ERR_CUDA, "track kernel", err);
+  h->last_launches += n_track_launches;
+  mark(2);
 
   if ((err = launch_scan_u64(trk_counts, trk_offsets, n_events, trk_scan_state, stream)) != cudaSuccess)
     return fail(h, ALLEN_VELO_ERR_CUDA, "track scan", err);
   h->last_launches++;
-  mark(5);
+  mark(3);
 
   CompactTracksLaunch ct{};
   ct.n_events = n_events;
@@ -281,7 +275,7 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   ct.out = *ot;
   if ((err = launch_compact_tracks(ct, stream)) != cudaSuccess) return fail(h, ALLEN_VELO_ERR_CUDA, "track compaction", err);
   h->last_launches++;
-  mark(6);
+  mark(4);
   return ALLEN_VELO_OK;
 }
 

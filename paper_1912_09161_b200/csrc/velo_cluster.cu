@@ -1,6 +1,7 @@
 // Kernel 1 of the VELO hot path: raw decode (A1), exact connected-component clustering (A2), centroid -> global
-// position and phi16 (A3) and the per-layer phi sort (A4) — SURVEY.md §8(a); definitions DESIGN.md R1-R4; paper
-// P:153 (decoding), P:179 (clustering as connected component labelling), P:183 (sort hits on every layer by phi).
+// position and phi16 (A3), the per-layer phi sort (A4) and the placement of the layer in the compacted output (A9) —
+// SURVEY.md §8(a); definitions DESIGN.md R1-R4; paper P:153 (decoding), P:179 (clustering as connected component
+// labelling), P:183 (sort hits on every layer by phi), P:136 (sizes stay on the device).
 //
 // Work decomposition: ONE WARP per (event, layer).  Clustering is independent per sensor (R2) and the sort is
 // independent per layer (R4), so a warp needs no block-level barrier: everything below synchronises with
@@ -8,49 +9,74 @@
 //
 // Clustering without a pixel grid: the nodes of the graph are "SP components" — a 2x4 super-pixel holds at most two
 // 8-connected components (pixels in adjacent rows of a 2-wide block always touch, so components are runs of occupied
-// rows).  Super-pixels of one sensor are put into a small open-addressing hash table in shared memory keyed by
-// (sp_col, sp_row); each SP looks up only its four "forward" neighbours (col+1: row-1,row,row+1; col: row+1), and only
-// those its border pixels can touch (about one probe per SP on minimum-bias occupancy).  Touching components become
-// edges; labels (node ids) are propagated over the edge list to the minimum until nothing changes, which is exact for
-// any cluster size.  Roots get cluster slots by warp ballot (no atomics); non-root components add their integer sums
-// to the root's slot with shared-memory atomics (commutative integer adds/min: deterministic).
+// rows).  The super-pixels of the layer's sensors are staged in shared memory and put into one open-addressing hash
+// table keyed by (sensor, sp_col, sp_row); each SP looks up only its four "forward" neighbours (col+1: row-1, row,
+// row+1; col: row+1), and only those its border pixels can touch.  Touching components become edges; labels (node
+// ids) are propagated over the edge list to the minimum until nothing changes, which is exact for any cluster size.
+// Roots get cluster slots by warp ballot (no atomics); non-root components add their integer sums to the root's slot
+// with shared-memory atomics (commutative integer adds / min: deterministic).
 //
-// The layer's clusters are then ranked by (phi16, key) with a 256-bucket counting sort on the top byte of phi plus an
-// exact in-bucket rank, and written in the normative order, coalesced, to the (event, layer) region of the slab.
+// The layer's clusters are ranked by (phi16, key) with a 256-bucket counting sort on the top byte of phi plus an exact
+// in-bucket rank.  The position of the layer in the compacted output comes from a decoupled look-back over the
+// (event, layer) items (one status word per item; the count is published before the sort so successors rarely wait),
+// and the layer is written once, coalesced, in its final place: no slab, no separate scan or compaction pass.
+//
+// Capacities.  FAST: the layer's SP words fit the warp's shared memory (256).  MID: they do not, but every sensor
+// does: one pass per sensor group in shared memory, cluster records and sort scratch in a pool slot in global memory.
+// BIG: everything in a (larger) pool slot in global memory.  Same code, same results, decreasing speed; a layer is
+// flagged STAGE_OVERFLOW only if it exceeds 8192 SP words or the BIG pool (counter-allocated) is exhausted.  MID
+// slots belong to resident warps (per-SM bit masks), so they never run out and nobody waits for one.
 #include "velo_common.cuh"
 
 namespace velo {
 namespace {
 
-constexpr int kWarps = 4;            // warps per CTA (independent work items)
-constexpr int kHashBits = 9;
-constexpr uint32_t kH = 1u << kHashBits;  // hash slots per sensor
-constexpr uint32_t kSpCap = 320;     // SP words per sensor the table takes (load factor <= 0.625)
-constexpr uint32_t kEdgeCap = kH;    // edges per sensor
-constexpr uint32_t kClCap = 768;     // clusters per (event, layer) staged in shared memory
+constexpr int kWarps = 4;  // warps per CTA (independent work items)
+// per-warp shared memory
+constexpr uint32_t kCapSp = 256, kHashBits = 9, kCapEdges = 256, kCapCl = 256;
+// pool slots in global memory
+constexpr uint32_t kMidCl = 1024;
+constexpr uint32_t kBigSp = 8192, kBigHashBits = 14, kBigEdges = 7 * kBigSp, kBigCl = 2 * kBigSp;
 
-// per-warp shared memory (bytes)
-constexpr uint32_t kScratchBytes = 12 * kH;  // tab u32[H] | lab u16[2H] | edges u32[H] (aliased: cidmap u16[2H])
-static_assert(1024 + 6 * kClCap <= kScratchBytes, "sort scratch must fit in the CCL scratch it aliases");
+constexpr unsigned long long kFlagAggregate = 1ull << 62, kFlagInclusive = 2ull << 62, kValueMask = (1ull << 62) - 1;
 
-template <bool kChecksum>
-struct WarpSmem {
-  uint32_t scratch[kScratchBytes / 4];
-  uint32_t ckey[kClCap], cn[kClCap], ccol[kClCap], crow[kClCap];
-  uint32_t ccks[kChecksum ? kClCap : 1];
-  uint32_t n_edges;
+__device__ __forceinline__ unsigned long long ld_status(const unsigned long long* p) {
+  unsigned long long v;
+  asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_status(unsigned long long* p, unsigned long long v) {
+  asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+
+// Storage of one clustering pass.  Staged SP word: hitmap | sp_row << 8 | sp_col << 14 | local sensor << 23; 0 = dead.
+struct Pass {
+  uint32_t* sp;     // [cap_sp]
+  uint32_t* tab;    // [1 << hash_bits] entries (key << 14) | (index + 1), 0 = empty; key = staged word bits 25:8
+  uint16_t* lab;    // [2 * cap_sp] label of node 2 * index + component
+  uint32_t* edges;  // [cap_edges] u | v << 16; reused as cidmap u16[2 * cap_sp] once the labels are final
+  uint32_t hash_bits, cap_sp, cap_edges;
+};
+struct ClusterStore {  // cluster records of the whole layer
+  uint32_t *key, *n, *col, *row, *cks;
+  uint32_t cap;
+};
+struct SortStore {
+  uint32_t* cnt256;             // [256]
+  uint16_t *tmp, *order, *phis; // [cap] each; phis = phi16 + 32768
 };
 
-__device__ __forceinline__ uint32_t hash_slot(uint32_t key) { return (key * 0x9E3779B1u) >> (32 - kHashBits); }
+__device__ __forceinline__ uint32_t hash_slot(uint32_t key, uint32_t bits) { return (key * 0x9E3779B1u) >> (32 - bits); }
 
-// Slot of `key` in the table, or -1.  Entries are (key << 8) | hitmap, 0 = empty.
-__device__ __forceinline__ int lookup(const uint32_t* tab, uint32_t key) {
-  uint32_t s = hash_slot(key);
+// Index of the staged SP with `key`, or -1.
+__device__ __forceinline__ int lookup(const uint32_t* tab, uint32_t bits, uint32_t key) {
+  const uint32_t mask = (1u << bits) - 1u;
+  uint32_t s = hash_slot(key, bits);
   for (;;) {
     const uint32_t e = tab[s];
     if (e == 0) return -1;
-    if ((e >> 8) == key) return (int)s;
-    s = (s + 1) & (kH - 1);
+    if ((e >> 14) == key) return (int)(e & 0x3FFFu) - 1;
+    s = (s + 1) & mask;
   }
 }
 
@@ -91,17 +117,367 @@ __device__ __forceinline__ Stats comp_stats(uint32_t m, uint32_t C, uint32_t R, 
   return s;
 }
 
+// One clustering pass over the sensors [k0, k1) of the layer (lane k holds sensor k's id and bank range): stage,
+// insert, find edges, propagate labels, give roots cluster ids from n_cl upwards and accumulate the cluster records.
+// Returns false if a capacity of `p` or `cs` is exceeded (the caller retries with larger storage).
 template <bool kChecksum>
-__global__ void __launch_bounds__(kWarps * 32) velo_cluster_kernel(const ClusterLaunch a) {
+__device__ __forceinline__ bool ccl_pass(const Pass& p, const ClusterStore& cs, const DeviceGeometry& g,
+                                         const uint32_t* __restrict__ spw, uint32_t my_sensor, uint32_t my_off,
+                                         uint32_t my_cnt, uint32_t k0, uint32_t k1, uint32_t& n_cl, bool& bad_sp,
+                                         uint32_t* n_edges_ctr) {
+  const uint32_t lane = lane_id();
+  const uint32_t bits = p.hash_bits;
+  // ---- stage the SP words of the group (R1: addresses outside the sensor are ignored and flagged)
+  uint32_t n = 0;
+  for (uint32_t k = k0; k < k1; ++k) {
+    const uint32_t off = __shfl_sync(kFull, my_off, k), cnt = __shfl_sync(kFull, my_cnt, k);
+    for (uint32_t i = lane; i < cnt; i += 32) {
+      const uint32_t w = __ldg(spw + off + i);
+      const uint32_t R = (w >> 8) & 0x3Fu, C = (w >> 14) & 0x1FFu;
+      uint32_t staged = (w & 0x7FFFFFu) | (k << 23);
+      if (C >= g.sp_cols || R >= g.sp_rows) { bad_sp = true; staged = 0; }
+      if ((w & 0xFFu) == 0) staged = 0;
+      p.sp[n + i] = staged;
+    }
+    n += cnt;
+  }
+  for (uint32_t s = lane; s < (1u << bits); s += 32) p.tab[s] = 0;
+  if (lane == 0) *n_edges_ctr = 0;
+  __syncwarp();
+
+  // ---- insert: entry = key << 14 | (index + 1); a repeated address merges its hitmap into the first one (R1)
+  const uint32_t mask = (1u << bits) - 1u;
+  for (uint32_t i = lane; i < n; i += 32) {
+    const uint32_t w = p.sp[i];
+    if (!w) continue;
+    const uint32_t key = (w >> 8) & 0x3FFFFu;
+    uint32_t s = hash_slot(key, bits);
+    for (;;) {
+      const uint32_t old = atomicCAS(p.tab + s, 0u, (key << 14) | (i + 1));
+      if (old == 0) break;
+      if ((old >> 14) == key) {
+        atomicOr(p.sp + (old & 0x3FFFu) - 1, w & 0xFFu);
+        p.sp[i] = 0;
+        break;
+      }
+      s = (s + 1) & mask;
+    }
+  }
+  __syncwarp();
+
+  // ---- edges to touching forward neighbours; node = 2 * index + component
+  for (uint32_t i = lane; i < n; i += 32) {
+    const uint32_t w = p.sp[i];
+    if (!w) continue;
+    const uint32_t h = w & 0xFFu, R = (w >> 8) & 0x3Fu, C = (w >> 14) & 0x1FFu;
+    const uint32_t key = (w >> 8) & 0x3FFFFu;
+    const Comps mine = split_rows(h);
+    const uint32_t nA = 2 * i, nB = 2 * i + 1;
+    p.lab[nA] = (uint16_t)nA;
+    p.lab[nB] = (uint16_t)nB;
+    auto push = [&](uint32_t u, uint32_t v) {
+      const uint32_t idx = atomicAdd(n_edges_ctr, 1u);
+      if (idx < p.cap_edges) p.edges[idx] = u | (v << 16);
+    };
+    const uint32_t r4 = mine.rA | mine.rB;
+    const uint32_t n_row3 = (mine.rA & 8u) ? nA : nB;  // our component holding row 3
+    // (C, R+1): our row 3 touches their row 0 whatever the columns
+    if ((r4 & 8u) && R + 1 < g.sp_rows) {
+      const int t = lookup(p.tab, bits, key + 1);
+      if (t >= 0) {
+        const uint32_t q = p.sp[t] & 0xFFu;
+        if ((q | (q >> 4)) & 1u) push(n_row3, 2 * t);
+      }
+    }
+    if (C + 1 < g.sp_cols) {
+      // (C+1, R): our column-1 pixels touch their column-0 pixels within one row
+      if (h & 0xF0u) {
+        const int t = lookup(p.tab, bits, key + 64);
+        if (t >= 0) {
+          const uint32_t q = p.sp[t] & 0xFFu;
+          const Comps theirs = split_rows(q);
+          const uint32_t gl = q & 0xFu;
+          const uint32_t hA = (h >> 4) & mine.rA, hB = (h >> 4) & mine.rB;
+          const uint32_t adjA = (hA | (hA << 1) | (hA >> 1)) & gl, adjB = (hB | (hB << 1) | (hB >> 1)) & gl;
+          if (adjA & theirs.rA) push(nA, 2 * t);
+          if (adjA & theirs.rB) push(nA, 2 * t + 1);
+          if (adjB & theirs.rA) push(nB, 2 * t);
+          if (adjB & theirs.rB) push(nB, 2 * t + 1);
+        }
+      }
+      // (C+1, R+1): our pixel (dc=1, dr=3) touches their pixel (dc=0, dr=0)
+      if ((h & 0x80u) && R + 1 < g.sp_rows) {
+        const int t = lookup(p.tab, bits, key + 65);
+        if (t >= 0 && (p.sp[t] & 1u)) push(n_row3, 2 * t);
+      }
+      // (C+1, R-1): our pixel (dc=1, dr=0) touches their pixel (dc=0, dr=3)
+      if ((h & 0x10u) && R >= 1) {
+        const int t = lookup(p.tab, bits, key + 63);
+        if (t >= 0 && (p.sp[t] & 8u)) {
+          const Comps theirs = split_rows(p.sp[t] & 0xFFu);
+          push(nA, (theirs.rA & 8u) ? 2 * t : 2 * t + 1);
+        }
+      }
+    }
+  }
+  __syncwarp();
+  const uint32_t n_edges = *n_edges_ctr;
+  if (n_edges > p.cap_edges) return false;
+
+  // ---- propagate the minimum node id over the edges until nothing changes (exact for any cluster size)
+  if (n_edges) {
+    for (;;) {
+      bool changed = false;
+      for (uint32_t j = lane; j < n_edges; j += 32) {
+        const uint32_t uv = p.edges[j];
+        const uint32_t u = uv & 0xFFFFu, v = uv >> 16;
+        const uint16_t lu = p.lab[u], lv = p.lab[v];
+        if (lu < lv) { p.lab[v] = lu; changed = true; }
+        else if (lv < lu) { p.lab[u] = lv; changed = true; }
+      }
+      __syncwarp();
+      if (!__any_sync(kFull, changed)) break;
+    }
+  }
+
+  // ---- roots take cluster ids (ballot order) and store their own sums; cidmap[node] = id
+  uint16_t* cidmap = reinterpret_cast<uint16_t*>(p.edges);
+  bool any_child = false;
+  for (uint32_t i0 = 0; i0 < n; i0 += 32) {
+    const uint32_t i = i0 + lane;
+    const uint32_t w = i < n ? p.sp[i] : 0u;
+    const bool live = w != 0;
+    const uint32_t h = w & 0xFFu, R = (w >> 8) & 0x3Fu, C = (w >> 14) & 0x1FFu;
+    const uint32_t sensor = __shfl_sync(kFull, my_sensor, (w >> 23) & 7u);
+    const Comps mine = split_rows(h);
+    const bool rootA = live && p.lab[2 * i] == 2 * i;
+    const bool rootB = live && mine.rB && p.lab[2 * i + 1] == 2 * i + 1;
+    const uint32_t ballotA = __ballot_sync(kFull, rootA), ballotB = __ballot_sync(kFull, rootB);
+    const uint32_t cidA = n_cl + __popc(ballotA & lanemask_lt());
+    const uint32_t cidB = n_cl + __popc(ballotA) + __popc(ballotB & lanemask_lt());
+    n_cl += __popc(ballotA) + __popc(ballotB);
+    any_child = any_child || (live && (!rootA || (mine.rB && !rootB)));
+    if (n_cl > cs.cap) return false;  // warp-uniform
+    if (rootA) {
+      const Stats s = comp_stats<kChecksum>(h & (mine.rA | (mine.rA << 4)), C, R, g.n_cols);
+      cs.key[cidA] = (sensor << 18) | s.minpix; cs.n[cidA] = s.n; cs.col[cidA] = s.sum_col; cs.row[cidA] = s.sum_row;
+      if (kChecksum) cs.cks[cidA] = s.cks;
+      cidmap[2 * i] = (uint16_t)cidA;
+    }
+    if (rootB) {
+      const Stats s = comp_stats<kChecksum>(h & (mine.rB | (mine.rB << 4)), C, R, g.n_cols);
+      cs.key[cidB] = (sensor << 18) | s.minpix; cs.n[cidB] = s.n; cs.col[cidB] = s.sum_col; cs.row[cidB] = s.sum_row;
+      if (kChecksum) cs.cks[cidB] = s.cks;
+      cidmap[2 * i + 1] = (uint16_t)cidB;
+    }
+  }
+  __syncwarp();
+  // ---- non-root components add their sums to the root's record
+  if (__any_sync(kFull, any_child)) {
+    for (uint32_t i = lane; i < n; i += 32) {
+      const uint32_t w = p.sp[i];
+      if (!w) continue;
+      const uint32_t h = w & 0xFFu, R = (w >> 8) & 0x3Fu, C = (w >> 14) & 0x1FFu;
+      const Comps mine = split_rows(h);
+#pragma unroll
+      for (int comp = 0; comp < 2; ++comp) {
+        const uint32_t rows = comp ? mine.rB : mine.rA;
+        const uint32_t node = 2 * i + comp;
+        if (!rows || p.lab[node] == node) continue;
+        const uint32_t cid = cidmap[p.lab[node]];
+        const Stats s = comp_stats<kChecksum>(h & (rows | (rows << 4)), C, R, g.n_cols);
+        atomicMin(&cs.key[cid], (cs.key[cid] & ~0x3FFFFu) | s.minpix);
+        atomicAdd(&cs.n[cid], s.n);
+        atomicAdd(&cs.col[cid], s.sum_col);
+        atomicAdd(&cs.row[cid], s.sum_row);
+        if (kChecksum) atomicAdd(&cs.cks[cid], s.cks);
+      }
+    }
+    __syncwarp();
+  }
+  return true;
+}
+
+// A3 + A4 + A9 for one layer whose n_cl cluster records are in `cs`: position and phi16, rank by (phi16, key),
+// look-back for the layer's place in the compacted output, coalesced write in the normative order.
+template <bool kChecksum>
+__device__ __forceinline__ void finish_layer(const ClusterLaunch& a, const ClusterStore& cs, const SortStore& ss,
+                                             uint32_t item, uint32_t e, uint32_t layer, uint32_t n_cl) {
+  const DeviceGeometry& g = a.geo;
+  const uint32_t lane = lane_id();
+  // the count goes out first: successors can add it up while this warp sorts
+  if (lane == 0) st_status(a.state + item, (item == 0 ? kFlagInclusive : kFlagAggregate) | n_cl);
+
+  for (uint32_t s = lane; s < 256; s += 32) ss.cnt256[s] = 0;
+  __syncwarp();
+  for (uint32_t c = lane; c < n_cl; c += 32) {
+    float x, y, z;
+    cluster_position(cs.n[c], cs.col[c], cs.row[c], g.pitch, g.ltg + 9 * (cs.key[c] >> 18), x, y, z);
+    const uint16_t p = (uint16_t)((uint16_t)phi16_of(x, y) ^ 0x8000u);
+    ss.phis[c] = p;
+    atomicAdd(&ss.cnt256[p >> 8], 1u);
+  }
+  __syncwarp();
+  {  // exclusive scan of the 256 bucket counts: 8 per lane + warp scan
+    uint32_t v[8], sum = 0;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) { v[q] = ss.cnt256[lane * 8 + q]; sum += v[q]; }
+    uint32_t incl = sum;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const uint32_t t = __shfl_up_sync(kFull, incl, d);
+      if (lane >= (uint32_t)d) incl += t;
+    }
+    uint32_t run = incl - sum;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) { ss.cnt256[lane * 8 + q] = run; run += v[q]; }
+  }
+  __syncwarp();
+  for (uint32_t c = lane; c < n_cl; c += 32) ss.tmp[atomicAdd(&ss.cnt256[ss.phis[c] >> 8], 1u)] = (uint16_t)c;
+  __syncwarp();
+  for (uint32_t j = lane; j < n_cl; j += 32) {
+    const uint32_t c = ss.tmp[j];
+    const uint32_t b = ss.phis[c] >> 8;
+    const uint32_t start = b ? ss.cnt256[b - 1] : 0, end = ss.cnt256[b];
+    const unsigned long long mine = ((unsigned long long)ss.phis[c] << 32) | cs.key[c];
+    uint32_t rank = 0;
+    for (uint32_t q = start; q < end; ++q) {
+      const uint32_t o = ss.tmp[q];
+      rank += (((unsigned long long)ss.phis[o] << 32) | cs.key[o]) < mine;
+    }
+    ss.order[start + rank] = (uint16_t)c;
+  }
+  __syncwarp();
+
+  // ---- decoupled look-back over the items before this one
+  unsigned long long exclusive = 0;
+  if (item > 0) {
+    long long look = (long long)item - 1;
+    for (;;) {
+      const long long idx = look - (long long)lane;
+      unsigned long long s = kFlagInclusive;  // items before the first count as an inclusive prefix of 0
+      if (idx >= 0) {
+        do { s = ld_status(a.state + idx); } while ((s >> 62) == 0);
+      }
+      const uint32_t incl_mask = __ballot_sync(kFull, (s >> 62) == 2);
+      const int first = incl_mask ? __ffs(incl_mask) - 1 : 32;
+      unsigned long long part = (int)lane <= first ? (s & kValueMask) : 0ull;
+#pragma unroll
+      for (int d = 16; d; d >>= 1) part += __shfl_xor_sync(kFull, part, d);
+      exclusive += part;
+      if (incl_mask) break;
+      look -= 32;
+    }
+    if (lane == 0) st_status(a.state + item, kFlagInclusive | (exclusive + n_cl));
+  }
+  const uint32_t base = (uint32_t)exclusive;
+  const uint32_t n_items = a.n_events * g.n_layers;
+  if (lane == 0) {
+    a.out.layer_offsets[item] = base;
+    if (layer == 0) a.out.event_offsets[e] = base;
+    if (item + 1 == n_items) {
+      a.out.layer_offsets[n_items] = base + n_cl;
+      a.out.event_offsets[a.n_events] = base + n_cl;
+    }
+  }
+  if (n_cl == 0) return;
+  if (exclusive + n_cl > a.out.capacity) {
+    if (lane == 0) atomicOr(a.out.status + e, ALLEN_VELO_STATUS_CLUSTER_CAPACITY);
+    return;
+  }
+  // ---- the layer in the normative order, in its final place
+  for (uint32_t j = lane; j < n_cl; j += 32) {
+    const uint32_t c = ss.order[j];
+    const uint32_t key = cs.key[c], n = cs.n[c], sc = cs.col[c], sr = cs.row[c];
+    float x, y, z;
+    cluster_position(n, sc, sr, g.pitch, g.ltg + 9 * (key >> 18), x, y, z);
+    const uint32_t o = base + j;
+    a.out.key[o] = key;
+    a.out.n_pixels[o] = n;
+    a.out.sum_col[o] = sc;
+    a.out.sum_row[o] = sr;
+    a.out.x[o] = x;
+    a.out.y[o] = y;
+    a.out.z[o] = z;
+    a.out.phi16[o] = (int16_t)(ss.phis[c] ^ 0x8000u);
+    if (kChecksum) a.out.checksum[o] = cs.cks[c];
+  }
+}
+
+// Out-of-line instances for storage in global memory (MID and BIG): generic pointers, rarely executed.
+template <bool kChecksum>
+__device__ __noinline__ bool ccl_pass_generic(const Pass& p, const ClusterStore& cs, const DeviceGeometry& g,
+                                              const uint32_t* __restrict__ spw, uint32_t my_sensor, uint32_t my_off,
+                                              uint32_t my_cnt, uint32_t k0, uint32_t k1, uint32_t& n_cl, bool& bad_sp,
+                                              uint32_t* n_edges_ctr) {
+  return ccl_pass<kChecksum>(p, cs, g, spw, my_sensor, my_off, my_cnt, k0, k1, n_cl, bad_sp, n_edges_ctr);
+}
+template <bool kChecksum>
+__device__ __noinline__ void finish_layer_generic(const ClusterLaunch& a, const ClusterStore& cs, const SortStore& ss,
+                                                  uint32_t item, uint32_t e, uint32_t layer, uint32_t n_cl) {
+  finish_layer<kChecksum>(a, cs, ss, item, e, layer, n_cl);
+}
+
+template <bool kChecksum>
+struct WarpSmem {
+  uint32_t sp[kCapSp];
+  uint32_t tab[1u << kHashBits];
+  uint16_t lab[2 * kCapSp];
+  uint32_t edges[kCapEdges];
+  uint32_t ckey[kCapCl], cn[kCapCl], ccol[kCapCl], crow[kCapCl];
+  uint32_t ccks[kChecksum ? kCapCl : 1];
+  uint32_t n_edges;
+};
+static_assert(1024 + 6 * kCapCl <= 4 * kCapSp + 4 * (1u << kHashBits), "sort scratch aliases sp + tab");
+
+// Layout of the pool slots (bytes from the slot base).
+struct MidSlot {
+  static constexpr size_t kStats = 0;                              // 5 x u32[kMidCl]
+  static constexpr size_t kCnt = kStats + 5 * 4 * (size_t)kMidCl;  // u32[256]
+  static constexpr size_t kSort = kCnt + 1024;                     // 3 x u16[kMidCl]
+  static constexpr size_t kBytes = (kSort + 3 * 2 * (size_t)kMidCl + 255) / 256 * 256;
+};
+struct BigSlot {
+  static constexpr size_t kSp = 0;
+  static constexpr size_t kTab = kSp + 4 * (size_t)kBigSp;
+  static constexpr size_t kLab = kTab + 4 * ((size_t)1 << kBigHashBits);
+  static constexpr size_t kEdges = kLab + 2 * 2 * (size_t)kBigSp;
+  static constexpr size_t kStats = kEdges + 4 * (size_t)kBigEdges;
+  static constexpr size_t kCnt = kStats + 5 * 4 * (size_t)kBigCl;
+  static constexpr size_t kSort = kCnt + 1024;
+  static constexpr size_t kCtr = kSort + 3 * 2 * (size_t)kBigCl;   // u32 edge counter
+  static constexpr size_t kBytes = (kCtr + 4 + 255) / 256 * 256;
+};
+
+__device__ __forceinline__ void stores_at(unsigned char* base, size_t stats, size_t cnt, size_t sort, uint32_t cap,
+                                          ClusterStore& cs, SortStore& ss) {
+  uint32_t* s = reinterpret_cast<uint32_t*>(base + stats);
+  cs.key = s; cs.n = s + cap; cs.col = s + 2 * cap; cs.row = s + 3 * cap; cs.cks = s + 4 * cap; cs.cap = cap;
+  ss.cnt256 = reinterpret_cast<uint32_t*>(base + cnt);
+  uint16_t* t = reinterpret_cast<uint16_t*>(base + sort);
+  ss.tmp = t; ss.order = t + cap; ss.phis = t + 2 * cap;
+}
+
+template <bool kChecksum>
+__global__ void __launch_bounds__(kWarps * 32) velo_cluster_kernel(const __grid_constant__ ClusterLaunch a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   using WS = WarpSmem<kChecksum>;
   WS& ws = reinterpret_cast<WS*>(smem_raw)[threadIdx.x >> 5];
   const DeviceGeometry& g = a.geo;
   const uint32_t lane = lane_id();
   const uint32_t L = g.n_layers;
+  // items are taken in blockIdx order: every predecessor of a running item is running or finished (look-back)
   const uint32_t item = blockIdx.x * kWarps + (threadIdx.x >> 5);
   if (item >= a.n_events * L) return;
   const uint32_t e = item / L, layer = item % L;
+
+  ClusterStore cs;
+  cs.key = ws.ckey; cs.n = ws.cn; cs.col = ws.ccol; cs.row = ws.crow; cs.cks = ws.ccks; cs.cap = kCapCl;
+  SortStore ss;
+  ss.cnt256 = ws.sp;
+  ss.tmp = reinterpret_cast<uint16_t*>(ws.tab);
+  ss.order = ss.tmp + kCapCl;
+  ss.phis = ss.order + kCapCl;
 
   // ---------------- A1: header, bank table (raw format v1, R1) ----------------
   const uint32_t byte0 = __ldg(a.event_offsets + e), byte1 = __ldg(a.event_offsets + e + 1);
@@ -116,26 +492,19 @@ __global__ void __launch_bounds__(kWarps * 32) velo_cluster_kernel(const Cluster
     bad = bad || need != n_words;
   }
   const uint32_t* tbl = ev + 4;
-  uint32_t before = 0;  // SP words of this event in layers below `layer` (slab placement)
   if (!bad) {
     for (uint32_t j = lane; j < g.n_sensors; j += 32) {
       const uint32_t o0 = __ldg(tbl + j), o1 = __ldg(tbl + j + 1);
       bad = bad || o0 > o1 || (j == 0 && o0 != 0) || (j + 1 == g.n_sensors && o1 != n_sp_total);
-      if (__ldg(g.sensor_layer + j) < layer) before += o1 - o0;
     }
   }
   bad = __any_sync(kFull, bad);
   if (bad) {
-    if (lane == 0) {
-      if (layer == 0) atomicOr(a.status + e, ALLEN_VELO_STATUS_BAD_HEADER);
-      a.counts[item] = 0;
-      a.slab_base[item] = 0;
-    }
+    if (lane == 0 && layer == 0) atomicOr(a.out.status + e, ALLEN_VELO_STATUS_BAD_HEADER);
+    finish_layer<kChecksum>(a, cs, ss, item, e, layer, 0);
     return;
   }
-  before = __reduce_add_sync(kFull, before);
-  const uint32_t* sp = tbl + g.table_words;
-  const uint32_t slab0 = 2u * ((byte0 >> 2) + 4u + g.table_words + before);
+  const uint32_t* spw = tbl + g.table_words;
 
   // sensors of this layer: lane k < K holds sensor k's bank range
   const uint32_t K = __ldg(g.layer_n_sensors + layer);
@@ -146,267 +515,100 @@ __global__ void __launch_bounds__(kWarps * 32) velo_cluster_kernel(const Cluster
     my_cnt = __ldg(tbl + my_sensor + 1) - my_off;
   }
   const uint32_t n_sp_layer = __reduce_add_sync(kFull, my_cnt);
-  bool overflow = (unsigned long long)slab0 + 2ull * n_sp_layer > a.slab.capacity;
+  const uint32_t max_cnt = __reduce_max_sync(kFull, my_cnt);
 
-  uint32_t* tab = ws.scratch;
-  uint16_t* lab = reinterpret_cast<uint16_t*>(ws.scratch + kH);
-  uint32_t* edges = ws.scratch + 2 * kH;
-  uint16_t* cidmap = reinterpret_cast<uint16_t*>(ws.scratch + 2 * kH);
+  Pass fast;
+  fast.sp = ws.sp; fast.tab = ws.tab; fast.lab = ws.lab; fast.edges = ws.edges;
+  fast.hash_bits = kHashBits; fast.cap_sp = kCapSp; fast.cap_edges = kCapEdges;
 
-  uint32_t n_cl = 0;  // clusters of this layer so far (warp-uniform)
-  bool bad_sp = false;
-
-  // ---------------- A2: clustering, sensor by sensor ----------------
-  for (uint32_t k = 0; k < K && !overflow; ++k) {
-    const uint32_t sensor = __shfl_sync(kFull, my_sensor, k);
-    const uint32_t off = __shfl_sync(kFull, my_off, k);
-    const uint32_t cnt = __shfl_sync(kFull, my_cnt, k);
-    if (cnt == 0) continue;
-    if (cnt > kSpCap) { overflow = true; break; }
-    for (uint32_t s = lane; s < kH; s += 32) tab[s] = 0;
-    if (lane == 0) ws.n_edges = 0;
-    __syncwarp();
-
-    // Phase A: insert SP words (entry = key << 8 | hitmap, key = sp_col << 6 | sp_row); a repeated address merges.
-    uint32_t absorbed = 0;  // bit per chunk: this lane's word needs no processing (invalid, empty or merged)
-    for (uint32_t i = lane, chunk = 0; i < cnt; i += 32, ++chunk) {
-      const uint32_t w = __ldg(sp + off + i);
-      const uint32_t h = w & 0xFFu, R = (w >> 8) & 0x3Fu, C = (w >> 14) & 0x1FFu;
-      if (C >= g.sp_cols || R >= g.sp_rows) { bad_sp = true; absorbed |= 1u << chunk; continue; }
-      if (h == 0) { absorbed |= 1u << chunk; continue; }
-      const uint32_t key = (C << 6) | R;
-      uint32_t s = hash_slot(key);
-      for (;;) {
-        const uint32_t old = atomicCAS(tab + s, 0u, (key << 8) | h);
-        if (old == 0) break;
-        if ((old >> 8) == key) { atomicOr(tab + s, h); absorbed |= 1u << chunk; break; }
-        s = (s + 1) & (kH - 1);
-      }
+  uint32_t n_cl = 0;
+  bool bad_sp = false, overflow = false;
+  int mode = n_sp_layer <= kCapSp ? 0 : (max_cnt <= kCapSp && n_sp_layer <= kMidCl) ? 1 : 2;
+  if (mode == 0) {
+    if (ccl_pass<kChecksum>(fast, cs, g, spw, my_sensor, my_off, my_cnt, 0, K, n_cl, bad_sp, &ws.n_edges)) {
+      if (__any_sync(kFull, bad_sp) && lane == 0) atomicOr(a.out.status + e, ALLEN_VELO_STATUS_BAD_SP);
+      finish_layer<kChecksum>(a, cs, ss, item, e, layer, n_cl);
+      return;
     }
-    __syncwarp();
-
-    // Phase B: every SP initialises its node labels and pushes edges to touching forward neighbours.
-    for (uint32_t i = lane, chunk = 0; i < cnt; i += 32, ++chunk) {
-      if (absorbed >> chunk & 1u) continue;
-      const uint32_t w = __ldg(sp + off + i);
-      const uint32_t R = (w >> 8) & 0x3Fu, C = (w >> 14) & 0x1FFu;
-      const uint32_t key = (C << 6) | R;
-      const uint32_t slot = (uint32_t)lookup(tab, key);
-      const uint32_t h = tab[slot] & 0xFFu;
-      const Comps mine = split_rows(h);
-      const uint32_t nA = 2 * slot, nB = 2 * slot + 1;
-      lab[nA] = (uint16_t)nA;
-      lab[nB] = (uint16_t)nB;
-      auto push = [&](uint32_t u, uint32_t v) {
-        const uint32_t idx = atomicAdd(&ws.n_edges, 1u);
-        if (idx < kEdgeCap) edges[idx] = u | (v << 16);
-      };
-      const uint32_t r4 = mine.rA | mine.rB;
-      const uint32_t n_row3 = (mine.rA & 8u) ? nA : nB;  // our component holding row 3
-      // (C, R+1): our row 3 touches their row 0 whatever the columns
-      if ((r4 & 8u) && R + 1 < g.sp_rows) {
-        const int t = lookup(tab, key + 1);
-        if (t >= 0) {
-          const uint32_t q = tab[t] & 0xFFu;
-          if ((q | (q >> 4)) & 1u) push(n_row3, 2 * t);
-        }
-      }
-      if (C + 1 < g.sp_cols) {
-        // (C+1, R): our column-1 pixels touch their column-0 pixels within one row
-        if (h & 0xF0u) {
-          const int t = lookup(tab, key + 64);
-          if (t >= 0) {
-            const uint32_t q = tab[t] & 0xFFu;
-            const Comps theirs = split_rows(q);
-            const uint32_t gl = q & 0xFu;
-            const uint32_t hA = (h >> 4) & mine.rA, hB = (h >> 4) & mine.rB;
-            const uint32_t adjA = (hA | (hA << 1) | (hA >> 1)) & gl, adjB = (hB | (hB << 1) | (hB >> 1)) & gl;
-            if (adjA & theirs.rA) push(nA, 2 * t);
-            if (adjA & theirs.rB) push(nA, 2 * t + 1);
-            if (adjB & theirs.rA) push(nB, 2 * t);
-            if (adjB & theirs.rB) push(nB, 2 * t + 1);
-          }
-        }
-        // (C+1, R+1): our pixel (dc=1, dr=3) touches their pixel (dc=0, dr=0)
-        if ((h & 0x80u) && R + 1 < g.sp_rows) {
-          const int t = lookup(tab, key + 65);
-          if (t >= 0 && (tab[t] & 1u)) push(n_row3, 2 * t);
-        }
-        // (C+1, R-1): our pixel (dc=1, dr=0) touches their pixel (dc=0, dr=3)
-        if ((h & 0x10u) && R >= 1) {
-          const int t = lookup(tab, key + 63);
-          if (t >= 0 && (tab[t] & 8u)) {
-            const Comps theirs = split_rows(tab[t] & 0xFFu);
-            push(nA, (theirs.rA & 8u) ? 2 * t : 2 * t + 1);
-          }
-        }
-      }
-    }
-    __syncwarp();
-    const uint32_t n_edges = ws.n_edges;
-    if (n_edges > kEdgeCap) { overflow = true; break; }
-
-    // Phase C: propagate the minimum node id over the edges until nothing changes (exact for any cluster size).
-    if (n_edges) {
-      for (;;) {
-        bool changed = false;
-        for (uint32_t j = lane; j < n_edges; j += 32) {
-          const uint32_t uv = edges[j];
-          const uint32_t u = uv & 0xFFFFu, v = uv >> 16;
-          const uint16_t lu = lab[u], lv = lab[v];
-          if (lu < lv) { lab[v] = lu; changed = true; }
-          else if (lv < lu) { lab[u] = lv; changed = true; }
-        }
-        __syncwarp();
-        if (!__any_sync(kFull, changed)) break;
-      }
-    }
-
-    // Phase D1: roots take cluster slots (ballot order) and store their own sums; cidmap[node] = slot.
-    const uint32_t n_cl_before = n_cl;
-    uint32_t has_child = 0;  // chunks in which this lane's SP has a non-root component
-    for (uint32_t i0 = 0, chunk = 0; i0 < cnt; i0 += 32, ++chunk) {
-      const uint32_t i = i0 + lane;
-      const bool live = i < cnt && !(absorbed >> chunk & 1u);
-      uint32_t slot = 0, h = 0, C = 0, R = 0;
-      Comps mine{0, 0};
-      if (live) {
-        const uint32_t w = __ldg(sp + off + i);
-        R = (w >> 8) & 0x3Fu; C = (w >> 14) & 0x1FFu;
-        slot = (uint32_t)lookup(tab, (C << 6) | R);
-        h = tab[slot] & 0xFFu;
-        mine = split_rows(h);
-      }
-      const bool rootA = live && lab[2 * slot] == 2 * slot;
-      const bool rootB = live && mine.rB && lab[2 * slot + 1] == 2 * slot + 1;
-      const uint32_t ballotA = __ballot_sync(kFull, rootA), ballotB = __ballot_sync(kFull, rootB);
-      const uint32_t cidA = n_cl + __popc(ballotA & lanemask_lt());
-      const uint32_t cidB = n_cl + __popc(ballotA) + __popc(ballotB & lanemask_lt());
-      n_cl += __popc(ballotA) + __popc(ballotB);
-      if (live && (!rootA || (mine.rB && !rootB))) has_child |= 1u << chunk;
-      if (n_cl > kClCap) { overflow = true; break; }
-      if (rootA) {
-        const Stats s = comp_stats<kChecksum>(h & (mine.rA | (mine.rA << 4)), C, R, g.n_cols);
-        ws.ckey[cidA] = (sensor << 18) | s.minpix; ws.cn[cidA] = s.n; ws.ccol[cidA] = s.sum_col; ws.crow[cidA] = s.sum_row;
-        if (kChecksum) ws.ccks[cidA] = s.cks;
-        cidmap[2 * slot] = (uint16_t)cidA;
-      }
-      if (rootB) {
-        const Stats s = comp_stats<kChecksum>(h & (mine.rB | (mine.rB << 4)), C, R, g.n_cols);
-        ws.ckey[cidB] = (sensor << 18) | s.minpix; ws.cn[cidB] = s.n; ws.ccol[cidB] = s.sum_col; ws.crow[cidB] = s.sum_row;
-        if (kChecksum) ws.ccks[cidB] = s.cks;
-        cidmap[2 * slot + 1] = (uint16_t)cidB;
-      }
-    }
-    if (overflow) break;
-    __syncwarp();
-    // Phase D2: non-root components add their sums to the root's slot.
-    const uint32_t any_child = __reduce_or_sync(kFull, has_child);
-    for (uint32_t i = lane, chunk = 0; i < cnt && (any_child >> chunk); i += 32, ++chunk) {
-      if (!(has_child >> chunk & 1u)) continue;
-      const uint32_t w = __ldg(sp + off + i);
-      const uint32_t R = (w >> 8) & 0x3Fu, C = (w >> 14) & 0x1FFu;
-      const uint32_t slot = (uint32_t)lookup(tab, (C << 6) | R);
-      const uint32_t h = tab[slot] & 0xFFu;
-      const Comps mine = split_rows(h);
-#pragma unroll
-      for (int comp = 0; comp < 2; ++comp) {
-        const uint32_t rows = comp ? mine.rB : mine.rA;
-        const uint32_t node = 2 * slot + comp;
-        if (!rows || lab[node] == node) continue;
-        const uint32_t cid = cidmap[lab[node]];
-        const Stats s = comp_stats<kChecksum>(h & (rows | (rows << 4)), C, R, g.n_cols);
-        atomicMin(&ws.ckey[cid], (sensor << 18) | s.minpix);
-        atomicAdd(&ws.cn[cid], s.n);
-        atomicAdd(&ws.ccol[cid], s.sum_col);
-        atomicAdd(&ws.crow[cid], s.sum_row);
-        if (kChecksum) atomicAdd(&ws.ccks[cid], s.cks);
-      }
-    }
-    __syncwarp();
-    (void)n_cl_before;
+    mode = 2;  // more clusters or edges than the warp's shared memory holds (not seen on physics-like input)
   }
-
-  if (__any_sync(kFull, bad_sp) && lane == 0) atomicOr(a.status + e, ALLEN_VELO_STATUS_BAD_SP);
-  if (overflow) {
+  uint32_t held = 0xFFFFFFFFu;  // mid slot of this warp (released at the end)
+  if (mode == 1) {
+    // one slot per resident warp: bit b of mid_mask[sm] <-> slot 32 * sm + b.  A kernel with at most 32 resident warps
+    // per SM always finds a free bit, so nobody ever waits for a slot (a wait could deadlock the look-back).
+    uint32_t slot = 0xFFFFFFFFu;
     if (lane == 0) {
-      atomicOr(a.status + e, ALLEN_VELO_STATUS_STAGE_OVERFLOW);
-      a.counts[item] = 0;
-      a.slab_base[item] = slab0;
+      uint32_t sm;
+      asm volatile("mov.u32 %0, %%smid;" : "=r"(sm));
+      if (sm < a.n_mid_sms) {
+        for (;;) {
+          const uint32_t free_bits = ~*reinterpret_cast<volatile uint32_t*>(a.mid_mask + sm);
+          if (!free_bits) break;
+          const uint32_t b = __ffs(free_bits) - 1;
+          if (!(atomicOr(a.mid_mask + sm, 1u << b) >> b & 1u)) { slot = 32 * sm + b; break; }
+        }
+      }
     }
-    return;
-  }
-
-  // ---------------- A3 + A4: position, phi16, rank by (phi16, key) ----------------
-  uint32_t* cnt256 = ws.scratch;                                            // u32[256]
-  uint16_t* tmp = reinterpret_cast<uint16_t*>(ws.scratch + 256);            // u16[kClCap]
-  uint16_t* order = tmp + kClCap;                                           // u16[kClCap]
-  uint16_t* phis = order + kClCap;                                          // u16[kClCap] phi16 + 32768
-  for (uint32_t s = lane; s < 256; s += 32) cnt256[s] = 0;
-  __syncwarp();
-  for (uint32_t c = lane; c < n_cl; c += 32) {
-    float x, y, z;
-    cluster_position(ws.cn[c], ws.ccol[c], ws.crow[c], g.pitch, g.ltg + 9 * (ws.ckey[c] >> 18), x, y, z);
-    const uint16_t p = (uint16_t)((uint16_t)phi16_of(x, y) ^ 0x8000u);
-    phis[c] = p;
-    atomicAdd(&cnt256[p >> 8], 1u);
-  }
-  __syncwarp();
-  {  // exclusive scan of the 256 bucket counts: 8 per lane + warp scan
-    uint32_t v[8], sum = 0;
-#pragma unroll
-    for (int q = 0; q < 8; ++q) { v[q] = cnt256[lane * 8 + q]; sum += v[q]; }
-    uint32_t incl = sum;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-      const uint32_t t = __shfl_up_sync(kFull, incl, d);
-      if (lane >= (uint32_t)d) incl += t;
+    slot = __shfl_sync(kFull, slot, 0);
+    if (slot == 0xFFFFFFFFu) {
+      mode = 2;
+    } else {
+      held = slot;
+      unsigned char* base = a.mid_pool + (size_t)slot * MidSlot::kBytes;
+      stores_at(base, MidSlot::kStats, MidSlot::kCnt, MidSlot::kSort, kMidCl, cs, ss);
+      n_cl = 0;
+      bad_sp = false;
+      bool ok = true;
+      for (uint32_t k0 = 0; k0 < K && ok;) {  // greedy groups of consecutive sensors that fit the shared memory
+        uint32_t k1 = k0, sum = 0;
+        while (k1 < K) {
+          const uint32_t cnt = __shfl_sync(kFull, my_cnt, k1);
+          if (sum + cnt > kCapSp) break;
+          sum += cnt;
+          ++k1;
+        }
+        ok = ccl_pass_generic<kChecksum>(fast, cs, g, spw, my_sensor, my_off, my_cnt, k0, k1, n_cl, bad_sp, &ws.n_edges);
+        k0 = k1;
+      }
+      if (!ok) mode = 2;
     }
-    uint32_t run = incl - sum;
-#pragma unroll
-    for (int q = 0; q < 8; ++q) { cnt256[lane * 8 + q] = run; run += v[q]; }
   }
-  __syncwarp();
-  for (uint32_t c = lane; c < n_cl; c += 32) tmp[atomicAdd(&cnt256[phis[c] >> 8], 1u)] = (uint16_t)c;
-  __syncwarp();
-  for (uint32_t j = lane; j < n_cl; j += 32) {
-    const uint32_t c = tmp[j];
-    const uint32_t b = phis[c] >> 8;
-    const uint32_t start = b ? cnt256[b - 1] : 0, end = cnt256[b];
-    const unsigned long long mine = ((unsigned long long)phis[c] << 32) | ws.ckey[c];
-    uint32_t rank = 0;
-    for (uint32_t q = start; q < end; ++q) {
-      const uint32_t o = tmp[q];
-      rank += (((unsigned long long)phis[o] << 32) | ws.ckey[o]) < mine;
+  if (mode == 2) {
+    uint32_t slot = 0;
+    if (lane == 0) slot = n_sp_layer <= kBigSp ? atomicAdd(a.big_ctr, 1u) : 0xFFFFFFFFu;
+    slot = __shfl_sync(kFull, slot, 0);
+    if (slot >= a.n_big_slots) {
+      overflow = true;
+    } else {
+      unsigned char* base = a.big_pool + (size_t)slot * BigSlot::kBytes;
+      Pass big;
+      big.sp = reinterpret_cast<uint32_t*>(base + BigSlot::kSp);
+      big.tab = reinterpret_cast<uint32_t*>(base + BigSlot::kTab);
+      big.lab = reinterpret_cast<uint16_t*>(base + BigSlot::kLab);
+      big.edges = reinterpret_cast<uint32_t*>(base + BigSlot::kEdges);
+      big.hash_bits = kBigHashBits; big.cap_sp = kBigSp; big.cap_edges = kBigEdges;
+      stores_at(base, BigSlot::kStats, BigSlot::kCnt, BigSlot::kSort, kBigCl, cs, ss);
+      n_cl = 0;
+      bad_sp = false;
+      overflow = !ccl_pass_generic<kChecksum>(big, cs, g, spw, my_sensor, my_off, my_cnt, 0, K, n_cl, bad_sp,
+                                              reinterpret_cast<uint32_t*>(base + BigSlot::kCtr));
     }
-    order[start + rank] = (uint16_t)c;
   }
+  if (overflow) {
+    if (lane == 0) atomicOr(a.out.status + e, ALLEN_VELO_STATUS_STAGE_OVERFLOW);
+    n_cl = 0;
+  } else if (__any_sync(kFull, bad_sp) && lane == 0) {
+    atomicOr(a.out.status + e, ALLEN_VELO_STATUS_BAD_SP);
+  }
+  finish_layer_generic<kChecksum>(a, cs, ss, item, e, layer, n_cl);
   __syncwarp();
-
-  // ---------------- write the layer in the normative order (coalesced) ----------------
-  for (uint32_t j = lane; j < n_cl; j += 32) {
-    const uint32_t c = order[j];
-    const uint32_t key = ws.ckey[c], n = ws.cn[c], sc = ws.ccol[c], sr = ws.crow[c];
-    float x, y, z;
-    cluster_position(n, sc, sr, g.pitch, g.ltg + 9 * (key >> 18), x, y, z);
-    const uint32_t o = slab0 + j;
-    a.slab.key[o] = key;
-    a.slab.n_pixels[o] = n;
-    a.slab.sum_col[o] = sc;
-    a.slab.sum_row[o] = sr;
-    a.slab.x[o] = x;
-    a.slab.y[o] = y;
-    a.slab.z[o] = z;
-    a.slab.phi16[o] = (int16_t)(phis[c] ^ 0x8000u);
-    if (kChecksum) a.slab.checksum[o] = ws.ccks[c];
-  }
-  if (lane == 0) {
-    a.counts[item] = n_cl;
-    a.slab_base[item] = slab0;
-  }
+  if (held != 0xFFFFFFFFu && lane == 0) atomicAnd(a.mid_mask + (held >> 5), ~(1u << (held & 31u)));
 }
 
 }  // namespace
+
+size_t cluster_mid_slot_bytes() { return MidSlot::kBytes; }
+size_t cluster_big_slot_bytes() { return BigSlot::kBytes; }
 
 cudaError_t launch_cluster(const ClusterLaunch& a, cudaStream_t stream) {
   const uint32_t items = a.n_events * a.geo.n_layers;

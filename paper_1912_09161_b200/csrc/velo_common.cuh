@@ -24,15 +24,6 @@ struct DeviceGeometry {
   allen_velo_params_t params;
 };
 
-// Unsorted-capacity slab the cluster kernel writes (sorted per layer) before compaction: structure of arrays with
-// `capacity` entries; region of (event, layer) starts at slab_base[item] and holds counts[item] clusters.
-struct ClusterSlab {
-  uint32_t capacity;
-  uint32_t *key, *n_pixels, *sum_col, *sum_row, *checksum;
-  float *x, *y, *z;
-  int16_t* phi16;
-};
-
 // ---- small device helpers -------------------------------------------------------------------
 __device__ __forceinline__ uint32_t lane_id() { return threadIdx.x & 31u; }
 __device__ __forceinline__ uint32_t lanemask_lt() {
@@ -100,35 +91,31 @@ __device__ __forceinline__ float scatter(float xa, float ya, float za, float xb,
 __device__ __forceinline__ int dphi16(int16_t a, int16_t b) { return (int16_t)(uint16_t)((uint16_t)a - (uint16_t)b); }
 
 // ---- kernel launchers (defined in the .cu files) -----------------------------------------------
+// Cluster kernel: one warp per (event, layer); writes the compacted cluster output directly (decoupled look-back over
+// the items through `state`).  Layers that exceed the warp's shared memory use slots of the two pools.
 struct ClusterLaunch {
   DeviceGeometry geo;
   const uint32_t* raw;
   const uint32_t* event_offsets;
   uint32_t n_events;
-  ClusterSlab slab;
-  uint32_t* counts;     // [n_events*n_layers] clusters per (event, layer)
-  uint32_t* slab_base;  // [n_events*n_layers] first slab entry of the (event, layer) region
-  uint32_t* status;     // [n_events], zeroed before
+  allen_velo_clusters_t out;
+  unsigned long long* state;  // [n_events*n_layers] look-back status words, zeroed before
+  uint32_t* big_ctr;          // slots handed out of the big pool, zeroed before
+  uint32_t* mid_mask;         // [n_mid_sms] busy bits of the mid slots of every SM, zeroed before
+  unsigned char* mid_pool;    // [32 * n_mid_sms] slots
+  unsigned char* big_pool;    // [n_big_slots] slots
+  uint32_t n_mid_sms, n_big_slots;
   bool with_checksum;
 };
 cudaError_t launch_cluster(const ClusterLaunch& a, cudaStream_t stream);
+size_t cluster_mid_slot_bytes();
+size_t cluster_big_slot_bytes();
 
 // Exclusive prefix sum of `in[n]` into `out[n+1]` (out[n] = total), single pass with decoupled look-back.
 // `tile_state` needs scan_state_words(n) u64 words, zeroed by the launcher.
 size_t scan_state_words(uint32_t n);
-cudaError_t launch_scan_u32(const uint32_t* in, uint32_t* out, uint32_t n, unsigned long long* tile_state,
-                            uint32_t* aux_out, uint32_t aux_stride, cudaStream_t stream);
 cudaError_t launch_scan_u64(const unsigned long long* in, unsigned long long* out, uint32_t n,
                             unsigned long long* tile_state, cudaStream_t stream);
-
-struct CompactClustersLaunch {
-  DeviceGeometry geo;
-  uint32_t n_events;
-  ClusterSlab slab;
-  const uint32_t* slab_base;
-  allen_velo_clusters_t out;  // layer_offsets / event_offsets already final
-};
-cudaError_t launch_compact_clusters(const CompactClustersLaunch& a, cudaStream_t stream);
 
 // Search by triplet + fit, one CTA per event.  Per-event slabs are addressed from the cluster offsets: an event
 // with clusters [co, co+n) owns hits_slab[co, co+n) (a hit belongs to at most one track) and track slots
@@ -142,8 +129,9 @@ struct TrackLaunch {
   uint32_t* trk_hitoff;            // [capacity/3+1] event-local first entry in hits_slab of every output track
   float4* trk_fit;                 // [capacity/3+1] x0, y0, tx, ty
   unsigned long long* counts;      // [n_events] (n_tracks << 32) | n_track_hits
+  uint8_t* level;                  // [n_events] kernel instance an event was handed to (0 = by its size alone)
 };
-cudaError_t launch_track(const TrackLaunch& a, cudaStream_t stream);
+cudaError_t launch_track(const TrackLaunch& a, cudaStream_t stream, uint32_t* n_launches);
 
 struct CompactTracksLaunch {
   uint32_t n_events;

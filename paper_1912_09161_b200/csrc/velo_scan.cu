@@ -1,10 +1,10 @@
-// Prefix-sum output compaction (A9 of SURVEY.md §8(a); only quantities that size later work ever need to
-// leave the device — here nothing does, the offsets are produced and consumed on the device).
+// Prefix-sum output compaction of the tracks (A9 of SURVEY.md §8(a); only quantities that size later work ever
+// need to leave the device — here nothing does, the offsets are produced and consumed on the device).
 //
 //  * scan_kernel: single-pass exclusive prefix sum with decoupled look-back (tile aggregates / inclusive prefixes
 //    published through one 64-bit status word per tile; tiles are claimed by an atomic ticket so that every
-//    predecessor of a running tile is itself running or finished).
-//  * compact_clusters_kernel: moves the per-(event, layer) slab regions to their final, gap-free position.
+//    predecessor of a running tile is itself running or finished).  The clusters need no such pass: the cluster
+//    kernel does its own look-back per (event, layer) and writes every layer in its final place.
 #include "velo_common.cuh"
 
 namespace velo {
@@ -102,41 +102,6 @@ __global__ void __launch_bounds__(kScanThreads) scan_kernel(const TIn* __restric
   }
 }
 
-// One CTA per event: copy the event's clusters from the slab regions of its layers to [event_offsets[e], ...).
-__global__ void __launch_bounds__(256) compact_clusters_kernel(const CompactClustersLaunch a) {
-  __shared__ uint32_t lo[kMaxLayers + 1];
-  __shared__ uint32_t src[kMaxLayers];
-  const uint32_t e = blockIdx.x, L = a.geo.n_layers;
-  for (uint32_t l = threadIdx.x; l <= L; l += blockDim.x) lo[l] = a.out.layer_offsets[e * L + l];
-  for (uint32_t l = threadIdx.x; l < L; l += blockDim.x) src[l] = a.slab_base[e * L + l];
-  __syncthreads();
-  const uint32_t first = lo[0], n = lo[L] - lo[0];
-  uint32_t flags = 0;
-  if (n > 65535u) flags |= ALLEN_VELO_STATUS_TOO_MANY_CLUSTERS;
-  if ((unsigned long long)first + n > a.out.capacity) flags |= ALLEN_VELO_STATUS_CLUSTER_CAPACITY;
-  if (flags && threadIdx.x == 0) atomicOr(a.out.status + e, flags);
-  if (flags & ALLEN_VELO_STATUS_CLUSTER_CAPACITY) return;
-  for (uint32_t j = threadIdx.x; j < n; j += blockDim.x) {
-    const uint32_t pos = first + j;
-    // layer of cluster j: the last l with lo[l] <= pos (binary search over <= 64 entries)
-    uint32_t a0 = 0, a1 = L;
-    while (a1 - a0 > 1) {
-      const uint32_t mid = (a0 + a1) >> 1;
-      if (lo[mid] <= pos) a0 = mid; else a1 = mid;
-    }
-    const uint32_t s = src[a0] + (pos - lo[a0]);
-    a.out.key[pos] = a.slab.key[s];
-    a.out.n_pixels[pos] = a.slab.n_pixels[s];
-    a.out.sum_col[pos] = a.slab.sum_col[s];
-    a.out.sum_row[pos] = a.slab.sum_row[s];
-    a.out.x[pos] = a.slab.x[s];
-    a.out.y[pos] = a.slab.y[s];
-    a.out.z[pos] = a.slab.z[s];
-    a.out.phi16[pos] = a.slab.phi16[s];
-    if (a.out.checksum) a.out.checksum[pos] = a.slab.checksum[s];
-  }
-}
-
 template <typename TIn, typename TOut>
 cudaError_t run_scan(const TIn* in, TOut* out, uint32_t n, unsigned long long* state, uint32_t* aux_out,
                      uint32_t aux_stride, cudaStream_t stream) {
@@ -152,20 +117,9 @@ cudaError_t run_scan(const TIn* in, TOut* out, uint32_t n, unsigned long long* s
 
 size_t scan_state_words(uint32_t n) { return 1 + (size_t)(n + kTile - 1) / kTile; }
 
-cudaError_t launch_scan_u32(const uint32_t* in, uint32_t* out, uint32_t n, unsigned long long* tile_state,
-                            uint32_t* aux_out, uint32_t aux_stride, cudaStream_t stream) {
-  return run_scan<uint32_t, uint32_t>(in, out, n, tile_state, aux_out, aux_stride ? aux_stride : 1, stream);
-}
-
 cudaError_t launch_scan_u64(const unsigned long long* in, unsigned long long* out, uint32_t n,
                             unsigned long long* tile_state, cudaStream_t stream) {
   return run_scan<unsigned long long, unsigned long long>(in, out, n, tile_state, nullptr, 1, stream);
-}
-
-cudaError_t launch_compact_clusters(const CompactClustersLaunch& a, cudaStream_t stream) {
-  if (a.n_events == 0) return cudaSuccess;
-  compact_clusters_kernel<<<a.n_events, 256, 0, stream>>>(a);
-  return cudaGetLastError();
 }
 
 }  // namespace velo

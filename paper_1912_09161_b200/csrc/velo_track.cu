@@ -4,288 +4,457 @@
 // on every layer by phi for fast look-up") and R6 of P:149 (straight lines).
 //
 // One CTA per event ("a single event is assigned to one block, while intra-event parallelism is mapped to the threads
-// within one block").  The 24 layer iterations are sequential; inside an iteration tracks (T1/T2) and middle
-// hits (T3/T4) are processed one per thread.  All conflict rules are order-independent minima, implemented as 64-bit
-// atomicMin on shared-memory claim words keyed (bits(S) << 32 | index): no "first thread wins" anywhere, so the
-// result is exactly the oracle's.  Track slots and output positions come from block-wide ballot/prefix scans, which
-// makes the output order deterministic (order of creation).
+// within one block").  The L-2 layer iterations are sequential.  Design for sm_100a:
+//  * the three layers of an iteration (plus the one being prefetched) live in shared memory as 16-byte hit records
+//    (x, y, z, phi16 | used << 16) in a ring of four slots: one LDS.128 per candidate; the next layer is brought in
+//    with cp.async one iteration ahead, so its DRAM latency hides behind the current iteration;
+//  * phi look-up uses a 128-bucket start table per layer, built while the layer is staged (no binary search);
+//  * seeding is flattened: S1 lists (b, a) doublets inside the phi window, S2 gives every doublet one thread that
+//    scans b's window on layer C; the per-b argmin is a 64-bit shared-memory atomicMin on (bits(S), a, c);
+//  * all conflict rules are order-independent minima on packed keys (bits(S) << 32 | index): no "first thread wins",
+//    so the result is exactly the oracle's whatever the thread schedule;
+//  * the kernel is instantiated for three staging capacities (256 / 512 / 1024 hits per layer); every event is taken
+//    by the smallest instance it fits, and an instance that runs out of track slots hands the event to the next one.
+#include <cuda_pipeline.h>
+
 #include "velo_common.cuh"
 
 namespace velo {
 namespace {
 
-constexpr int kThreads = 128;
-constexpr uint32_t kCapLayer = 768;    // hits of one layer staged (claims, used flags, triplets)
-constexpr uint32_t kCapTracks = 1024;  // tracks of one event kept in shared memory
 constexpr unsigned long long kNoClaim = ~0ull;
+constexpr int kBuckets = 128;
+constexpr int kBucketShift = 9;  // 65536 / 128
+constexpr uint32_t kUsedBit = 0x10000u;
 
-struct Smem {
-  unsigned long long claimA[kCapLayer], claimC[kCapLayer];
-  uint32_t tripS[kCapLayer];
-  uint16_t tripA[kCapLayer], tripC[kCapLayer];
-  float seedS[kCapTracks];
-  uint32_t choiceS[kCapTracks];
-  uint16_t choiceC[kCapTracks];
-  uint16_t newest[kCapTracks], previous[kCapTracks], seedB[kCapTracks];
-  uint8_t nhits[kCapTracks], missed[kCapTracks];  // missed == 0xFF: closed
-  uint8_t used[3][kCapLayer];
-  uint32_t lo[kMaxLayers + 1];
-  uint32_t warp_tot[kThreads / 32];
-  uint32_t overflow;
+struct __align__(16) Hit {
+  float x, y, z;
+  uint32_t w;  // phi16 (low 16 bits, two's complement) | used << 16
 };
 
-// Exclusive prefix of `v` over the block in thread order; returns the block total in `total`.
-__device__ __forceinline__ uint32_t block_scan(uint32_t v, uint32_t* warp_tot, uint32_t& total) {
-  const uint32_t lane = lane_id(), warp = threadIdx.x >> 5;
-  uint32_t incl = v;
-#pragma unroll
-  for (int d = 1; d < 32; d <<= 1) {
-    const uint32_t t = __shfl_up_sync(kFull, incl, d);
-    if (lane >= (uint32_t)d) incl += t;
-  }
-  __syncthreads();  // protects warp_tot against the previous use
-  if (lane == 31) warp_tot[warp] = incl;
-  __syncthreads();
-  uint32_t off = 0;
-  total = 0;
-#pragma unroll
-  for (int w = 0; w < kThreads / 32; ++w) {
-    if (w < (int)warp) off += warp_tot[w];
-    total += warp_tot[w];
-  }
-  return off + incl - v;
+template <int kThreads_, int kCap_, int kCapTracks_, int kCapDoublets_, int kLevel_, bool kLast_>
+struct Cfg {
+  static constexpr int kThreads = kThreads_;
+  static constexpr int kCap = kCap_;            // hits of one layer staged
+  static constexpr int kCapTracks = kCapTracks_;
+  static constexpr int kCapDoublets = kCapDoublets_;
+  static constexpr int kLevel = kLevel_;
+  static constexpr bool kLast = kLast_;
+  static constexpr int kWarps = kThreads / 32;
+  static constexpr int kRoundsB = (kCap + kThreads - 1) / kThreads;
+  static constexpr int kRoundsT = (kCapTracks + kThreads - 1) / kThreads;
+};
+using CfgS = Cfg<128, 256, 512, 512, 0, false>;
+using CfgM = Cfg<256, 512, 1024, 1024, 1, false>;
+using CfgL = Cfg<512, 1024, 2048, 2048, 2, true>;
+
+template <class C>
+struct Smem {
+  Hit rec[4][C::kCap];
+  unsigned long long best[C::kCap];  // T3: per-b argmin key; T1/T2: forward claims on layer C (aliased by phase)
+  unsigned long long claimA[C::kCap], claimC[C::kCap];
+  uint32_t doublets[C::kCapDoublets];  // b_local | a_local << 16
+  float ttx[C::kCapTracks], tty[C::kCapTracks];  // slopes of the last segment (older -> newest hit)
+  uint32_t tstate[C::kCapTracks];                // newest << 16 | weak_ok << 15 | nhits << 8 | missed (0xFF: closed)
+  uint16_t tseedB[C::kCapTracks];                // track_key: event-local index of the seed's middle hit
+  uint16_t bucket[4][kBuckets + 2];
+  uint32_t lo[kMaxLayers + 1];
+  uint32_t warp_tot[C::kRoundsB > C::kRoundsT ? C::kRoundsB : C::kRoundsT][C::kWarps];
+  uint32_t n_doublets;
+  uint32_t min_active[2];
+  uint32_t flags;
+};
+
+__device__ __forceinline__ int phi_of(uint32_t w) { return (int)(int16_t)(uint16_t)(w & 0xFFFFu); }
+
+// First index in [0, n) of the layer (sorted by signed phi16) with phi >= target, or n.
+__device__ __forceinline__ uint32_t lower_bound_phi(const uint16_t* __restrict__ bucket, const Hit* __restrict__ rec,
+                                                    uint32_t n, int target) {
+  uint32_t idx = bucket[((uint32_t)(target + 32768) & 0xFFFFu) >> kBucketShift];
+  while (idx < n && phi_of(rec[idx].w) < target) ++idx;
+  return idx;
 }
 
-// First index in [0, n) of the sorted (signed) phi array with phi >= target, or n.
-__device__ __forceinline__ uint32_t lower_bound_phi(const int16_t* __restrict__ phi, uint32_t n, int target) {
-  uint32_t a = 0, b = n;
-  while (a < b) {
-    const uint32_t mid = (a + b) >> 1;
-    if ((int)__ldg(phi + mid) < target) a = mid + 1; else b = mid;
+__device__ __forceinline__ int wrap16(int v) { return (int)(int16_t)(uint16_t)v; }
+
+template <class C>
+struct Ctx {
+  Smem<C>& sm;
+  const float* __restrict__ X;
+  const float* __restrict__ Y;
+  const float* __restrict__ Z;
+  const int16_t* __restrict__ PHI;
+  allen_velo_params_t P;
+};
+
+// Bring layer `l` into ring slot l & 3: x, y, z by cp.async (4-byte copies into the 16-byte records), the phi word and
+// the bucket table by this thread.  Completion: __pipeline_wait_prior(0) + __syncthreads() by the caller.
+template <class C>
+__device__ __forceinline__ void stage_layer(const Ctx<C>& c, uint32_t l) {
+  Smem<C>& sm = c.sm;
+  const uint32_t base = sm.lo[l], n = sm.lo[l + 1] - base;
+  Hit* rec = sm.rec[l & 3];
+  uint16_t* bucket = sm.bucket[l & 3];
+  if (n == 0) {
+    for (uint32_t b = threadIdx.x; b <= (uint32_t)kBuckets; b += C::kThreads) bucket[b] = 0;
+    return;
   }
-  return a;
+  for (uint32_t k = threadIdx.x; k < n; k += C::kThreads) {
+    __pipeline_memcpy_async(&rec[k].x, c.X + base + k, 4);
+    __pipeline_memcpy_async(&rec[k].y, c.Y + base + k, 4);
+    __pipeline_memcpy_async(&rec[k].z, c.Z + base + k, 4);
+    const uint32_t ph = (uint16_t)__ldg(c.PHI + base + k);
+    rec[k].w = ph;
+    const int bk = (int)((ph ^ 0x8000u) >> kBucketShift);
+    const int bp = k ? (int)((((uint32_t)(uint16_t)__ldg(c.PHI + base + k - 1)) ^ 0x8000u) >> kBucketShift) : -1;
+    for (int b = bp + 1; b <= bk; ++b) bucket[b] = (uint16_t)k;
+    if (k + 1 == n)
+      for (int b = bk + 1; b <= kBuckets; ++b) bucket[b] = (uint16_t)n;
+  }
+  __pipeline_commit();
 }
 
-__global__ void __launch_bounds__(kThreads) velo_track_kernel(const TrackLaunch a) {
+// One (b, a) doublet of T3: slopes of a -> b, slope cut, then the best unused c of layer C inside b's phi window.
+template <class C>
+__device__ __forceinline__ void process_doublet(const Ctx<C>& c, const Hit* __restrict__ recA,
+                                                const Hit* __restrict__ recB, const Hit* __restrict__ recC,
+                                                const uint16_t* __restrict__ bucketC, uint32_t nC, uint32_t kb,
+                                                uint32_t ia) {
+  const Hit hb = recB[kb], ha = recA[ia];
+  const float dz_ab = __fsub_rn(hb.z, ha.z);
+  const float tx = __fdiv_rn(__fsub_rn(hb.x, ha.x), dz_ab), ty = __fdiv_rn(__fsub_rn(hb.y, ha.y), dz_ab);
+  if (!(fabsf(tx) <= c.P.max_slope) || !(fabsf(ty) <= c.P.max_slope)) return;
+  const int w = c.P.w_seed_phi16, phb = phi_of(hb.w);
+  uint32_t ic = lower_bound_phi(bucketC, recC, nC, wrap16(phb - w));
+  unsigned long long best = kNoClaim;
+  for (uint32_t k = 0; k < nC; ++k, ++ic) {
+    if (ic >= nC) ic -= nC;
+    const Hit hc = recC[ic];
+    const int d = wrap16(phi_of(hc.w) - phb);
+    if (d > w || d < -w) break;
+    if (hc.w & kUsedBit) continue;
+    const float dz = __fsub_rn(hc.z, hb.z);
+    const float ex = __fsub_rn(__fmaf_rn(tx, dz, hb.x), hc.x);
+    const float ey = __fsub_rn(__fmaf_rn(ty, dz, hb.y), hc.y);
+    const float S = __fmaf_rn(ex, ex, __fmul_rn(ey, ey));
+    if (!(S <= c.P.s_seed)) continue;
+    // argmin over (bits(S), a, c): layer-local indices order like the event-local ones
+    const unsigned long long key = ((unsigned long long)__float_as_uint(S) << 32) | (ia << 16) | ic;
+    best = key < best ? key : best;
+  }
+  if (best != kNoClaim) atomicMin(&c.sm.best[kb], best);
+}
+
+template <class C>
+__global__ void __launch_bounds__(C::kThreads) velo_track_kernel(const __grid_constant__ TrackLaunch a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  Smem& sm = *reinterpret_cast<Smem*>(smem_raw);
+  Smem<C>& sm = *reinterpret_cast<Smem<C>*>(smem_raw);
   const DeviceGeometry& g = a.geo;
-  const allen_velo_params_t P = g.params;
   const uint32_t e = blockIdx.x, L = g.n_layers, tid = threadIdx.x;
+  const uint32_t lane = lane_id(), warp = tid >> 5;
 
   const uint32_t co = a.clusters.event_offsets[e];
   const uint32_t n_cl = a.clusters.event_offsets[e + 1] - co;
-  const uint32_t st = a.clusters.status[e];
+  const uint32_t st0 = a.clusters.status[e];
   // events whose clusters were not produced or not written take no part in tracking
-  const bool skip = (st & (ALLEN_VELO_STATUS_BAD_HEADER | ALLEN_VELO_STATUS_TOO_MANY_CLUSTERS |
-                           ALLEN_VELO_STATUS_CLUSTER_CAPACITY | ALLEN_VELO_STATUS_STAGE_OVERFLOW)) != 0;
-  if (skip || n_cl == 0) {
-    if (tid == 0) a.counts[e] = 0;
+  const bool skip = (st0 & (ALLEN_VELO_STATUS_BAD_HEADER | ALLEN_VELO_STATUS_TOO_MANY_CLUSTERS |
+                            ALLEN_VELO_STATUS_CLUSTER_CAPACITY | ALLEN_VELO_STATUS_STAGE_OVERFLOW)) != 0;
+  if (skip || n_cl == 0 || n_cl > 65535u || (unsigned long long)co + n_cl > a.clusters.capacity) {
+    if (C::kLevel == 0 && tid == 0) {
+      if (!skip && n_cl > 65535u) atomicOr(a.clusters.status + e, ALLEN_VELO_STATUS_TOO_MANY_CLUSTERS);  // hits are u16
+      else if (!skip && n_cl) atomicOr(a.clusters.status + e, ALLEN_VELO_STATUS_STAGE_OVERFLOW);  // scratch is per cluster
+      a.counts[e] = 0;
+    }
     return;
   }
-  if ((unsigned long long)co + n_cl > a.clusters.capacity) {  // tracking scratch is indexed by cluster
-    if (tid == 0) { atomicOr(a.clusters.status + e, ALLEN_VELO_STATUS_STAGE_OVERFLOW); a.counts[e] = 0; }
-    return;
-  }
-  for (uint32_t l = tid; l <= L; l += kThreads) sm.lo[l] = a.clusters.layer_offsets[e * L + l] - co;
-  if (tid == 0) sm.overflow = 0;
+  // ---- which instance takes this event: the smallest whose staging capacity holds its busiest layer, unless a
+  //      smaller instance ran out of track slots and passed it on (level[e])
+  if (tid == 0) sm.flags = 0;
+  for (uint32_t l = tid; l <= L; l += C::kThreads) sm.lo[l] = a.clusters.layer_offsets[e * L + l] - co;
   __syncthreads();
-  for (uint32_t l = tid; l < L; l += kThreads)
-    if (sm.lo[l + 1] - sm.lo[l] > kCapLayer) sm.overflow = 1;
-  for (uint32_t i = tid; i < 3 * kCapLayer; i += kThreads) (&sm.used[0][0])[i] = 0;
-  for (uint32_t i = tid; i < kCapLayer; i += kThreads) { sm.claimA[i] = kNoClaim; sm.claimC[i] = kNoClaim; }
+  {
+    uint32_t mx = 0;
+    for (uint32_t l = tid; l < L; l += C::kThreads) mx = max(mx, sm.lo[l + 1] - sm.lo[l]);
+    if (mx) atomicMax(&sm.flags, mx);
+  }
   __syncthreads();
-  if (sm.overflow) {
-    if (tid == 0) { atomicOr(a.clusters.status + e, ALLEN_VELO_STATUS_STAGE_OVERFLOW); a.counts[e] = 0; }
+  const uint32_t max_layer = sm.flags;
+  const uint32_t natural = max_layer <= (uint32_t)CfgS::kCap ? 0u : max_layer <= (uint32_t)CfgM::kCap ? 1u : 2u;
+  const uint32_t level = max(natural, (uint32_t)a.level[e]);  // level[e]: 0 unless raised by a smaller instance
+  const bool fits = max_layer <= (uint32_t)C::kCap;
+  if (level != (uint32_t)C::kLevel || !fits) {
+    if (C::kLast && !fits && tid == 0) {  // busiest layer beyond the largest staging capacity
+      atomicOr(a.clusters.status + e, ALLEN_VELO_STATUS_STAGE_OVERFLOW);
+      a.counts[e] = 0;
+    }
     return;
   }
+  __syncthreads();
+  if (tid == 0) { sm.flags = 0; sm.min_active[0] = 0; sm.min_active[1] = 0; }
 
-  const float* __restrict__ X = a.clusters.x + co;
-  const float* __restrict__ Y = a.clusters.y + co;
-  const float* __restrict__ Z = a.clusters.z + co;
-  const int16_t* __restrict__ PHI = a.clusters.phi16 + co;
+  Ctx<C> c{sm, a.clusters.x + co, a.clusters.y + co, a.clusters.z + co, a.clusters.phi16 + co, g.params};
+  const allen_velo_params_t& P = c.P;
   uint16_t* link = a.link + co;
 
-  uint32_t n_tracks = 0;  // block-uniform
+  for (uint32_t k = tid; k < (uint32_t)C::kCap; k += C::kThreads) {
+    sm.best[k] = kNoClaim; sm.claimA[k] = kNoClaim; sm.claimC[k] = kNoClaim;
+  }
+  stage_layer(c, L - 1);
+  stage_layer(c, L - 2);
+  stage_layer(c, L - 3);
+
+  uint32_t n_tracks = 0;        // block-uniform
+  uint32_t first_new = 0;       // n_tracks before the latest T4 (block-uniform)
 
   for (int i = (int)L - 1; i >= 2; --i) {
     const uint32_t A0 = sm.lo[i], A1 = sm.lo[i + 1], B0 = sm.lo[i - 1], C0 = sm.lo[i - 2];
     const uint32_t nA = A1 - A0, nB = A0 - B0, nC = B0 - C0;
-    uint8_t* usedA = sm.used[i % 3];
-    uint8_t* usedB = sm.used[(i - 1) % 3];
-    uint8_t* usedC = sm.used[(i - 2) % 3];
-    if (i != (int)L - 1) {  // layer C enters the window: nothing of it is used yet
-      for (uint32_t k = tid; k < nC; k += kThreads) usedC[k] = 0;
-      __syncthreads();
-    }
+    Hit* recA = sm.rec[i & 3];
+    Hit* recB = sm.rec[(i - 1) & 3];
+    Hit* recC = sm.rec[(i - 2) & 3];
+    const uint16_t* bucketA = sm.bucket[i & 3];
+    const uint16_t* bucketC = sm.bucket[(i - 2) & 3];
 
-    // ---- T1 forward: best unused hit of layer C per active track, claim it with (bits(S), track_key)
-    for (uint32_t t = tid; t < n_tracks; t += kThreads) {
-      sm.choiceC[t] = 0xFFFF;
-      if (sm.missed[t] == 0xFF || nC == 0) continue;
-      const uint32_t p = sm.previous[t], q = sm.newest[t];
-      const float xp = __ldg(X + p), yp = __ldg(Y + p), zp = __ldg(Z + p);
-      const float xq = __ldg(X + q), yq = __ldg(Y + q), zq = __ldg(Z + q);
-      const int16_t phq = __ldg(PHI + q);
+    __pipeline_wait_prior(0);
+    __syncthreads();  // B1: layer C staged; tracks created by the previous T4 visible; claims re-initialised
+    if (i >= 3) stage_layer(c, (uint32_t)i - 3);  // prefetch: needed at the top of the next iteration
+
+    // ---- T1 forward: best hit of layer C per active track (nothing of C is used yet); claim with (bits(S), key)
+    const uint32_t first = min(sm.min_active[i & 1], first_new);
+    if (tid == 0) { sm.min_active[(i - 1) & 1] = 0xFFFFFFFFu; sm.n_doublets = 0; }
+    unsigned long long fkey[C::kRoundsT];
+    uint32_t fc[C::kRoundsT];
+#pragma unroll
+    for (int r = 0; r < C::kRoundsT; ++r) {
+      fkey[r] = kNoClaim;
+      fc[r] = 0;
+      if (first + r * C::kThreads >= n_tracks) continue;  // uniform
+      const uint32_t t = first + r * C::kThreads + tid;
+      if (t >= n_tracks) continue;
+      const uint32_t st = sm.tstate[t];
+      if ((st & 0xFFu) == 0xFFu || nC == 0) continue;
+      const uint32_t q = st >> 16;
+      float xq, yq, zq;
+      int phq;
+      if (q < A1) {  // q on layer A or B (always, when max_skipped <= 1)
+        const Hit hq = q >= A0 ? recA[q - A0] : recB[q - B0];
+        xq = hq.x; yq = hq.y; zq = hq.z; phq = phi_of(hq.w);
+      } else {       // tracks that skipped more than one layer: their last hit left the ring
+        xq = __ldg(c.X + q); yq = __ldg(c.Y + q); zq = __ldg(c.Z + q); phq = (int)__ldg(c.PHI + q);
+      }
+      const float tx = sm.ttx[t], ty = sm.tty[t];
       const int w = P.w_fwd_phi16;
-      const uint32_t s0 = lower_bound_phi(PHI + C0, nC, (int)(int16_t)(uint16_t)((int)phq - w));
+      uint32_t ic = lower_bound_phi(bucketC, recC, nC, wrap16(phq - w));
       unsigned long long best = kNoClaim;
-      for (uint32_t k = 0; k < nC; ++k) {
-        uint32_t idx = s0 + k;
-        if (idx >= nC) idx -= nC;
-        const uint32_t c = C0 + idx;
-        const int d = dphi16(__ldg(PHI + c), phq);
+      for (uint32_t k = 0; k < nC; ++k, ++ic) {
+        if (ic >= nC) ic -= nC;
+        const Hit hc = recC[ic];
+        const int d = wrap16(phi_of(hc.w) - phq);
         if (d > w || d < -w) break;
-        if (usedC[idx]) continue;
-        const float S = scatter(xp, yp, zp, xq, yq, zq, __ldg(X + c), __ldg(Y + c), __ldg(Z + c));
+        const float dz = __fsub_rn(hc.z, zq);
+        const float ex = __fsub_rn(__fmaf_rn(tx, dz, xq), hc.x);
+        const float ey = __fsub_rn(__fmaf_rn(ty, dz, yq), hc.y);
+        const float S = __fmaf_rn(ex, ex, __fmul_rn(ey, ey));
         if (!(S <= P.s_fwd)) continue;
-        const unsigned long long key = ((unsigned long long)__float_as_uint(S) << 32) | c;
+        const unsigned long long key = ((unsigned long long)__float_as_uint(S) << 32) | ic;
         best = key < best ? key : best;
       }
       if (best != kNoClaim) {
-        const uint32_t c = (uint32_t)best, sb = (uint32_t)(best >> 32);
-        sm.choiceC[t] = (uint16_t)c;
-        sm.choiceS[t] = sb;
-        atomicMin(&sm.claimC[c - C0], ((unsigned long long)sb << 32) | sm.seedB[t]);
+        fc[r] = (uint32_t)best;
+        fkey[r] = (best & 0xFFFFFFFF00000000ull) | sm.tseedB[t];
+        atomicMin(&sm.best[fc[r]], fkey[r]);
       }
     }
-    __syncthreads();
+    __syncthreads();  // B2
     // ---- T2 resolve: the minimal claim wins the hit; everyone else counts a miss
-    for (uint32_t t = tid; t < n_tracks; t += kThreads) {
-      if (sm.missed[t] == 0xFF) continue;
-      const uint32_t c = sm.choiceC[t];
-      bool won = false;
-      if (c != 0xFFFF) won = sm.claimC[c - C0] == (((unsigned long long)sm.choiceS[t] << 32) | sm.seedB[t]);
+#pragma unroll
+    for (int r = 0; r < C::kRoundsT; ++r) {
+      if (first + r * C::kThreads >= n_tracks) continue;  // uniform
+      const uint32_t t = first + r * C::kThreads + tid;
+      if (t >= n_tracks) continue;
+      const uint32_t st = sm.tstate[t];
+      if ((st & 0xFFu) == 0xFFu) continue;
+      const bool won = fkey[r] != kNoClaim && sm.best[fc[r]] == fkey[r];
       if (won) {
-        link[c] = sm.newest[t];
-        sm.previous[t] = sm.newest[t];
-        sm.newest[t] = (uint16_t)c;
-        sm.nhits[t] += 1;
-        sm.missed[t] = 0;
-        usedC[c - C0] = 1;
-      } else {
-        const uint32_t m = sm.missed[t] + 1u;
-        sm.missed[t] = m > (uint32_t)P.max_skipped ? 0xFF : (uint8_t)m;
-      }
-    }
-    __syncthreads();
-    for (uint32_t k = tid; k < nC; k += kThreads) sm.claimC[k] = kNoClaim;
-    __syncthreads();
-
-    // ---- T3 seed: best (a, c) per unused middle hit b; claim a and c with (bits(S), b)
-    for (uint32_t kb = tid; kb < nB; kb += kThreads) {
-      sm.tripS[kb] = 0xFFFFFFFFu;
-      if (usedB[kb] || nA == 0 || nC == 0) continue;
-      const uint32_t b = B0 + kb;
-      const float xb = __ldg(X + b), yb = __ldg(Y + b), zb = __ldg(Z + b);
-      const int16_t phb = __ldg(PHI + b);
-      const int w = P.w_seed_phi16;
-      const int target = (int)(int16_t)(uint16_t)((int)phb - w);
-      const uint32_t sA = lower_bound_phi(PHI + A0, nA, target);
-      const uint32_t sC = lower_bound_phi(PHI + C0, nC, target);
-      uint32_t bestS = 0xFFFFFFFFu, bestA = 0, bestC = 0;
-      bool found = false;
-      for (uint32_t ka = 0; ka < nA; ++ka) {
-        uint32_t ia = sA + ka;
-        if (ia >= nA) ia -= nA;
-        const uint32_t ha = A0 + ia;
-        const int da = dphi16(__ldg(PHI + ha), phb);
-        if (da > w || da < -w) break;
-        if (usedA[ia]) continue;
-        const float xa = __ldg(X + ha), ya = __ldg(Y + ha), za = __ldg(Z + ha);
-        const float dz_ab = __fsub_rn(zb, za);
-        const float tx = __fdiv_rn(__fsub_rn(xb, xa), dz_ab), ty = __fdiv_rn(__fsub_rn(yb, ya), dz_ab);
-        if (!(fabsf(tx) <= P.max_slope) || !(fabsf(ty) <= P.max_slope)) continue;
-        for (uint32_t kc = 0; kc < nC; ++kc) {
-          uint32_t ic = sC + kc;
-          if (ic >= nC) ic -= nC;
-          const uint32_t hc = C0 + ic;
-          const int dc = dphi16(__ldg(PHI + hc), phb);
-          if (dc > w || dc < -w) break;
-          if (usedC[ic]) continue;
-          const float dz = __fsub_rn(__ldg(Z + hc), zb);
-          const float ex = __fsub_rn(__fmaf_rn(tx, dz, xb), __ldg(X + hc));
-          const float ey = __fsub_rn(__fmaf_rn(ty, dz, yb), __ldg(Y + hc));
-          const float S = __fmaf_rn(ex, ex, __fmul_rn(ey, ey));
-          if (!(S <= P.s_seed)) continue;
-          const uint32_t sb = __float_as_uint(S);
-          // argmin over (bits(S), a, c)
-          const bool better = !found || sb < bestS || (sb == bestS && (ha < bestA || (ha == bestA && hc < bestC)));
-          if (better) { bestS = sb; bestA = ha; bestC = hc; found = true; }
-        }
-      }
-      if (found) {
-        sm.tripS[kb] = bestS;
-        sm.tripA[kb] = (uint16_t)bestA;
-        sm.tripC[kb] = (uint16_t)bestC;
-        const unsigned long long key = ((unsigned long long)bestS << 32) | b;
-        atomicMin(&sm.claimA[bestA - A0], key);
-        atomicMin(&sm.claimC[bestC - C0], key);
-      }
-    }
-    __syncthreads();
-    // ---- T4 resolve: accepted iff the triplet holds the minimal key on both its a and its c; new tracks take
-    //      slots in ascending b (block prefix scan)
-    for (uint32_t base = 0; base < nB; base += kThreads) {
-      const uint32_t kb = base + tid;
-      bool accepted = false;
-      uint32_t ha = 0, hc = 0, sb = 0;
-      if (kb < nB && sm.tripS[kb] != 0xFFFFFFFFu) {
-        ha = sm.tripA[kb]; hc = sm.tripC[kb]; sb = sm.tripS[kb];
-        const unsigned long long key = ((unsigned long long)sb << 32) | (B0 + kb);
-        accepted = sm.claimA[ha - A0] == key && sm.claimC[hc - C0] == key;
-      }
-      uint32_t total;
-      const uint32_t slot = n_tracks + block_scan(accepted ? 1u : 0u, sm.warp_tot, total);
-      if (accepted) {
-        if (slot < kCapTracks) {
-          const uint32_t b = B0 + kb;
-          sm.newest[slot] = (uint16_t)hc;
-          sm.previous[slot] = (uint16_t)b;
-          sm.seedB[slot] = (uint16_t)b;
-          sm.seedS[slot] = __uint_as_float(sb);
-          sm.nhits[slot] = 3;
-          sm.missed[slot] = 0;
-          link[b] = (uint16_t)ha;
-          link[hc] = (uint16_t)b;
-          usedA[ha - A0] = 1;
-          usedB[kb] = 1;
-          usedC[hc - C0] = 1;
+        const uint32_t q = st >> 16, cg = C0 + fc[r];
+        float xq, yq, zq;
+        if (q < A1) {
+          const Hit hq = q >= A0 ? recA[q - A0] : recB[q - B0];
+          xq = hq.x; yq = hq.y; zq = hq.z;
         } else {
-          sm.overflow = 1;
+          xq = __ldg(c.X + q); yq = __ldg(c.Y + q); zq = __ldg(c.Z + q);
+        }
+        const Hit hc = recC[fc[r]];
+        const float dz = __fsub_rn(hc.z, zq);
+        sm.ttx[t] = __fdiv_rn(__fsub_rn(hc.x, xq), dz);
+        sm.tty[t] = __fdiv_rn(__fsub_rn(hc.y, yq), dz);
+        recC[fc[r]].w = hc.w | kUsedBit;
+        link[cg] = (uint16_t)q;
+        const uint32_t nh = ((st >> 8) & 0x7Fu) + 1u;
+        sm.tstate[t] = (cg << 16) | (st & 0x8000u) | (nh << 8);
+        atomicMin(&sm.min_active[(i - 1) & 1], t);
+      } else {
+        const uint32_t m = (st & 0xFFu) + 1u;
+        if (m > (uint32_t)P.max_skipped) {
+          sm.tstate[t] = st | 0xFFu;
+        } else {
+          sm.tstate[t] = (st & 0xFFFFFF00u) | m;
+          atomicMin(&sm.min_active[(i - 1) & 1], t);
         }
       }
-      n_tracks += total;
-      if (n_tracks > kCapTracks) n_tracks = kCapTracks;
     }
-    __syncthreads();
-    for (uint32_t k = tid; k < nA; k += kThreads) sm.claimA[k] = kNoClaim;
-    for (uint32_t k = tid; k < nC; k += kThreads) sm.claimC[k] = kNoClaim;
-    __syncthreads();
-  }
+    __syncthreads();  // B3
 
-  if (sm.overflow) {
-    if (tid == 0) { atomicOr(a.clusters.status + e, ALLEN_VELO_STATUS_STAGE_OVERFLOW); a.counts[e] = 0; }
+    // ---- T3/S1: every unused b lists the unused hits of layer A inside its phi window as (b, a) doublets
+    const bool seeding = nA != 0 && nB != 0 && nC != 0;
+#pragma unroll
+    for (int r = 0; r < C::kRoundsB; ++r) {
+      const uint32_t kb = r * C::kThreads + tid;
+      if (kb >= nB) continue;
+      sm.best[kb] = kNoClaim;  // forward claims are done with; from here on: per-b argmin
+      const uint32_t wb = recB[kb].w;
+      if (!seeding || (wb & kUsedBit)) continue;
+      const int w = P.w_seed_phi16, phb = phi_of(wb);
+      uint32_t ia = lower_bound_phi(bucketA, recA, nA, wrap16(phb - w));
+      for (uint32_t k = 0; k < nA; ++k, ++ia) {
+        if (ia >= nA) ia -= nA;
+        const uint32_t wa = recA[ia].w;
+        const int d = wrap16(phi_of(wa) - phb);
+        if (d > w || d < -w) break;
+        if (wa & kUsedBit) continue;
+        const uint32_t pos = atomicAdd(&sm.n_doublets, 1u);
+        if (pos < (uint32_t)C::kCapDoublets) sm.doublets[pos] = kb | (ia << 16);
+        else process_doublet(c, recA, recB, recC, bucketC, nC, kb, ia);  // list full: do it here (same result)
+      }
+    }
+    __syncthreads();  // B4
+    // ---- T3/S2: one thread per doublet
+    {
+      const uint32_t nd = min(sm.n_doublets, (uint32_t)C::kCapDoublets);
+      for (uint32_t d = tid; d < nd; d += C::kThreads) {
+        const uint32_t v = sm.doublets[d];
+        process_doublet(c, recA, recB, recC, bucketC, nC, v & 0xFFFFu, v >> 16);
+      }
+    }
+    __syncthreads();  // B5
+
+    // ---- T4a: every b with a triplet claims its a and its c with (bits(S), b)
+    unsigned long long tkey[C::kRoundsB];
+    uint32_t tac[C::kRoundsB];  // a_local << 16 | c_local
+#pragma unroll
+    for (int r = 0; r < C::kRoundsB; ++r) {
+      tkey[r] = kNoClaim;
+      tac[r] = 0;
+      const uint32_t kb = r * C::kThreads + tid;
+      if (kb >= nB || !seeding) continue;
+      const unsigned long long k = sm.best[kb];
+      if (k == kNoClaim) continue;
+      tac[r] = (uint32_t)k;
+      tkey[r] = (k & 0xFFFFFFFF00000000ull) | (B0 + kb);
+      atomicMin(&sm.claimA[tac[r] >> 16], tkey[r]);
+      atomicMin(&sm.claimC[tac[r] & 0xFFFFu], tkey[r]);
+    }
+    __syncthreads();  // B6
+    // ---- T4b: accepted iff the triplet holds the minimal key on both its a and its c; new tracks take slots in
+    //      ascending b (ballot + per-warp totals)
+    uint32_t acc_ballot[C::kRoundsB];
+#pragma unroll
+    for (int r = 0; r < C::kRoundsB; ++r) {
+      const bool accepted = tkey[r] != kNoClaim && sm.claimA[tac[r] >> 16] == tkey[r] &&
+                            sm.claimC[tac[r] & 0xFFFFu] == tkey[r];
+      acc_ballot[r] = __ballot_sync(kFull, accepted);
+      if (lane == 0) sm.warp_tot[r][warp] = __popc(acc_ballot[r]);
+    }
+    __syncthreads();  // B7
+    first_new = n_tracks;
+    {
+      uint32_t run = n_tracks;
+#pragma unroll
+      for (int r = 0; r < C::kRoundsB; ++r) {
+        uint32_t before = 0, total = 0;
+#pragma unroll
+        for (int w = 0; w < C::kWarps; ++w) {
+          const uint32_t v = sm.warp_tot[r][w];
+          if (w < (int)warp) before += v;
+          total += v;
+        }
+        if (acc_ballot[r] >> lane & 1u) {
+          const uint32_t slot = run + before + __popc(acc_ballot[r] & lanemask_lt());
+          if (slot < (uint32_t)C::kCapTracks) {
+            const uint32_t kb = r * C::kThreads + tid, ia = tac[r] >> 16, ic = tac[r] & 0xFFFFu;
+            const Hit hb = recB[kb], hc = recC[ic];
+            const float dz = __fsub_rn(hc.z, hb.z);
+            sm.ttx[slot] = __fdiv_rn(__fsub_rn(hc.x, hb.x), dz);
+            sm.tty[slot] = __fdiv_rn(__fsub_rn(hc.y, hb.y), dz);
+            const float S = __uint_as_float((uint32_t)(tkey[r] >> 32));
+            sm.tstate[slot] = ((C0 + ic) << 16) | (S <= P.s_weak ? 0x8000u : 0u) | (3u << 8);
+            sm.tseedB[slot] = (uint16_t)(B0 + kb);
+            link[B0 + kb] = (uint16_t)(A0 + ia);
+            link[C0 + ic] = (uint16_t)(B0 + kb);
+            recA[ia].w |= kUsedBit;
+            recB[kb].w = hb.w | kUsedBit;
+            recC[ic].w = hc.w | kUsedBit;
+          } else {
+            sm.flags = 1;  // out of track slots: a larger instance redoes the event
+          }
+        }
+        run += total;
+      }
+      n_tracks = min(run, (uint32_t)C::kCapTracks);
+    }
+    // claims back to "none" for the next iteration (its T1 starts after B1)
+    for (uint32_t k = tid; k < (uint32_t)C::kCap; k += C::kThreads) {
+      sm.best[k] = kNoClaim; sm.claimA[k] = kNoClaim; sm.claimC[k] = kNoClaim;
+    }
+  }
+  __pipeline_wait_prior(0);
+  __syncthreads();
+
+  if (sm.flags) {
+    if (tid == 0) {
+      if (C::kLast) { atomicOr(a.clusters.status + e, ALLEN_VELO_STATUS_STAGE_OVERFLOW); a.counts[e] = 0; }
+      else a.level[e] = (uint8_t)(C::kLevel + 1);
+    }
     return;
   }
 
-  // ---- T5 finalise + A8 fit: keep >= 4 hits, or 3 hits with S_seed <= s_weak; compact in order of creation
+  // ---- T5 finalise + A8 fit: keep >= 4 hits, or 3 hits with S_seed <= s_weak; output in order of creation
   uint32_t out_tracks = 0, out_hits = 0;
   const uint32_t trk0 = co / 3;
-  for (uint32_t base = 0; base < n_tracks; base += kThreads) {
+  const float* __restrict__ X = c.X;
+  const float* __restrict__ Y = c.Y;
+  const float* __restrict__ Z = c.Z;
+  for (uint32_t base = 0; base < n_tracks; base += C::kThreads) {
     const uint32_t t = base + tid;
-    uint32_t n = 0;
+    uint32_t n = 0, st = 0;
     if (t < n_tracks) {
-      n = sm.nhits[t];
-      if (n == 3 && !(sm.seedS[t] <= P.s_weak)) n = 0;
+      st = sm.tstate[t];
+      n = (st >> 8) & 0x7Fu;
+      if (n == 3 && !(st & 0x8000u)) n = 0;
     }
-    uint32_t total;
-    const uint32_t off = block_scan(n ? ((1u << 20) | n) : 0u, sm.warp_tot, total);
+    // block exclusive scan of (1 << 20 | n)
+    const uint32_t v = n ? ((1u << 20) | n) : 0u;
+    uint32_t incl = v;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const uint32_t u = __shfl_up_sync(kFull, incl, d);
+      if (lane >= (uint32_t)d) incl += u;
+    }
+    __syncthreads();
+    if (lane == 31) sm.warp_tot[0][warp] = incl;
+    __syncthreads();
+    uint32_t off = incl - v, total = 0;
+#pragma unroll
+    for (int w = 0; w < C::kWarps; ++w) {
+      const uint32_t u = sm.warp_tot[0][w];
+      if (w < (int)warp) off += u;
+      total += u;
+    }
     if (n) {
       const uint32_t ot = out_tracks + (off >> 20), oh = out_hits + (off & 0xFFFFFu);
       // hits in order of addition: walk the links from the newest hit backwards
       double sz = 0, sx = 0, sy = 0;
-      uint32_t h = sm.newest[t];
+      uint32_t h = st >> 16;
       for (int k = (int)n - 1; k >= 0; --k) {
         a.hits_slab[co + oh + k] = (uint16_t)h;
         sz += (double)__ldg(Z + h); sx += (double)__ldg(X + h); sy += (double)__ldg(Y + h);
@@ -294,7 +463,7 @@ __global__ void __launch_bounds__(kThreads) velo_track_kernel(const TrackLaunch 
       const double inv = 1.0 / (double)n;
       const double zm = sz * inv, xm = sx * inv, ym = sy * inv;
       double szz = 0, szx = 0, szy = 0;
-      h = sm.newest[t];
+      h = st >> 16;
       for (int k = (int)n - 1; k >= 0; --k) {
         const double dz = (double)__ldg(Z + h) - zm;
         szz += dz * dz;
@@ -339,15 +508,32 @@ __global__ void __launch_bounds__(128) compact_tracks_kernel(const CompactTracks
   if (threadIdx.x == 0 && e + 1 == a.n_events) a.out.hit_offsets[T0 + nT] = H0 + nH;
 }
 
+template <class C>
+cudaError_t launch_instance(const TrackLaunch& a, cudaStream_t stream) {
+  cudaError_t err = cudaFuncSetAttribute(velo_track_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)sizeof(Smem<C>));
+  static_assert(sizeof(Smem<C>) <= 227 * 1024, "shared memory of one CTA");
+  if (err != cudaSuccess) return err;
+  velo_track_kernel<C><<<a.n_events, C::kThreads, sizeof(Smem<C>), stream>>>(a);
+  return cudaGetLastError();
+}
+
 }  // namespace
 
-cudaError_t launch_track(const TrackLaunch& a, cudaStream_t stream) {
+// Three launches over all events: each CTA first decides whether its event belongs to this instance (see the header
+// comment); events of other instances cost one small read and an exit.
+cudaError_t launch_track(const TrackLaunch& a, cudaStream_t stream, uint32_t* n_launches) {
+  *n_launches = 0;
   if (a.n_events == 0) return cudaSuccess;
-  cudaError_t err = cudaFuncSetAttribute(velo_track_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)sizeof(Smem));
+  cudaError_t err = cudaMemsetAsync(a.level, 0, a.n_events, stream);
   if (err != cudaSuccess) return err;
-  velo_track_kernel<<<a.n_events, kThreads, sizeof(Smem), stream>>>(a);
-  return cudaGetLastError();
+  if ((err = launch_instance<CfgS>(a, stream)) != cudaSuccess) return err;
+  ++*n_launches;
+  if ((err = launch_instance<CfgM>(a, stream)) != cudaSuccess) return err;
+  ++*n_launches;
+  if ((err = launch_instance<CfgL>(a, stream)) != cudaSuccess) return err;
+  ++*n_launches;
+  return cudaSuccess;
 }
 
 cudaError_t launch_compact_tracks(const CompactTracksLaunch& a, cudaStream_t stream) {
