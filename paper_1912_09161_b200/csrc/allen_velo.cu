@@ -27,12 +27,15 @@ struct allen_velo {
 
 namespace {
 
-constexpr uint32_t kKernels = 4;  // timed segments; velo_track is three launches (one per staging capacity)
-const char* const kKernelNames[kKernels] = {"velo_cluster", "velo_track", "scan_tracks", "compact_tracks"};
+constexpr uint32_t kKernels = 5;  // timed segments; velo_track is three launches (one per staging capacity)
+const char* const kKernelNames[kKernels] = {"velo_cluster", "scan_clusters", "velo_track", "scan_tracks",
+                                            "compact_tracks"};
 constexpr size_t kAlign = 256;
 inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
-// tracking scratch per cluster (link, hits_slab) and per track slot (trk_hitoff, trk_fit; one slot per 3 clusters)
+// bytes per slab entry (cluster SoA incl. checksum), tracking scratch per cluster (link, hits_slab) and per track
+// slot (trk_hitoff, trk_fit; one slot per 3 clusters)
+constexpr size_t kSlabEntryBytes = 7 * 4 + 2 + 4;
 constexpr size_t kTrackScratchBytes = 2 + 2;
 constexpr size_t kTrackSlotBytes = 4 + 16;
 
@@ -53,7 +56,9 @@ uint32_t big_slots(uint32_t items) { return 16 + items / 4096; }
 size_t fixed_bytes(uint32_t n_events, uint32_t n_layers, uint32_t n_mid_sms) {
   const uint32_t items = n_events * n_layers;
   size_t b = 0;
-  b += align_up(((size_t)items + 1) * 8 + (size_t)n_mid_sms * 4);  // look-back state, big-pool counter, mid masks
+  b += align_up((size_t)items * 4) * 2;                           // counts, slab_base
+  b += align_up(scan_state_words(items) * 8);                     // scan state (clusters)
+  b += align_up(8 + (size_t)n_mid_sms * 4);                       // big-pool counter, mid masks
   b += align_up((size_t)n_mid_sms * 32 * cluster_mid_slot_bytes());
   b += align_up((size_t)big_slots(items) * cluster_big_slot_bytes());
   b += align_up((size_t)n_events * 8) + align_up(((size_t)n_events + 1) * 8);  // track counts, offsets
@@ -62,7 +67,7 @@ size_t fixed_bytes(uint32_t n_events, uint32_t n_layers, uint32_t n_mid_sms) {
   return b + 16 * kAlign;
 }
 
-size_t per_entry_bytes() { return kTrackScratchBytes + (kTrackSlotBytes + 2) / 3; }
+size_t per_entry_bytes() { return kSlabEntryBytes + kTrackScratchBytes + (kTrackSlotBytes + 2) / 3; }
 
 int fail(allen_velo* h, int code, const char* what, cudaError_t err = cudaSuccess) {
   if (h) {
@@ -155,7 +160,7 @@ int allen_velo_create(const allen_velo_geometry_t* geo, allen_velo_t** out) {
 
 size_t allen_velo_workspace_bytes(const allen_velo_t* h, uint32_t n_events, size_t raw_bytes) {
   if (!h) return 0;
-  // tracking scratch: two entries per raw word (a super-pixel holds at most two clusters)
+  // slab and tracking scratch: two entries per raw word (a super-pixel holds at most two clusters)
   const size_t entries = raw_bytes / 2 + 4096;
   return fixed_bytes(n_events, h->dev.n_layers, h->n_mid_sms) + entries * per_entry_bytes() + 16 * kAlign;
 }
@@ -198,8 +203,11 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   if (!h->ws || h->ws_bytes < fixed + 1024 * per_entry_bytes() + 16 * kAlign) return fail(h, ALLEN_VELO_ERR_WORKSPACE, "workspace too small");
   const uint32_t items = n_events * L;
   Carve cv{static_cast<unsigned char*>(h->ws)};
-  // look-back words, then one word for the big-pool counter, then the mid masks: zeroed by one memset
-  const size_t state_bytes = ((size_t)items + 1) * 8 + (size_t)h->n_mid_sms * 4;
+  uint32_t* counts = cv.take<uint32_t>(items);
+  uint32_t* slab_base = cv.take<uint32_t>(items);
+  unsigned long long* scan_state = cv.take<unsigned long long>(scan_state_words(items));
+  // one word for the big-pool counter, then the mid masks: zeroed by one memset
+  const size_t state_bytes = 8 + (size_t)h->n_mid_sms * 4;
   unsigned long long* state = reinterpret_cast<unsigned long long*>(cv.take<unsigned char>(state_bytes));
   const uint32_t n_big = big_slots(items);
   unsigned char* mid_pool = cv.take<unsigned char>((size_t)h->n_mid_sms * 32 * cluster_mid_slot_bytes());
@@ -210,7 +218,18 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   uint8_t* trk_level = cv.take<uint8_t>(n_events);
   size_t entries = (h->ws_bytes - cv.used - 16 * kAlign) / per_entry_bytes();
   if (entries > 0x7FFFFFF0u) entries = 0x7FFFFFF0u;
-  // tracking scratch is addressed by output cluster index
+  ClusterSlab slab{};
+  slab.capacity = (uint32_t)entries;
+  slab.key = cv.take<uint32_t>(entries);
+  slab.n_pixels = cv.take<uint32_t>(entries);
+  slab.sum_col = cv.take<uint32_t>(entries);
+  slab.sum_row = cv.take<uint32_t>(entries);
+  slab.checksum = cv.take<uint32_t>(entries);
+  slab.x = cv.take<float>(entries);
+  slab.y = cv.take<float>(entries);
+  slab.z = cv.take<float>(entries);
+  slab.phi16 = cv.take<int16_t>(entries);
+  // tracking scratch is addressed by output cluster index; it shares the entry count with the slab
   uint16_t* link = cv.take<uint16_t>(entries);
   uint16_t* hits_slab = cv.take<uint16_t>(entries);
   uint32_t* trk_hitoff = cv.take<uint32_t>(entries / 3 + 1);
@@ -231,10 +250,12 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   cl.raw = static_cast<const uint32_t*>(raw_banks);
   cl.event_offsets = event_offsets;
   cl.n_events = n_events;
-  cl.out = *oc;
-  cl.state = state;
-  cl.big_ctr = reinterpret_cast<uint32_t*>(state + items);
-  cl.mid_mask = reinterpret_cast<uint32_t*>(state + items + 1);
+  cl.slab = slab;
+  cl.counts = counts;
+  cl.slab_base = slab_base;
+  cl.status = oc->status;
+  cl.big_ctr = reinterpret_cast<uint32_t*>(state);
+  cl.mid_mask = reinterpret_cast<uint32_t*>(state + 1);
   cl.mid_pool = mid_pool;
   cl.big_pool = big_pool;
   cl.n_mid_sms = h->n_mid_sms;
@@ -244,10 +265,17 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   h->last_launches++;
   mark(1);
 
+  if ((err = launch_scan_u32(counts, oc->layer_offsets, items, scan_state, oc->event_offsets, L, stream)) != cudaSuccess)
+    return fail(h, ALLEN_VELO_ERR_CUDA, "cluster scan", err);
+  h->last_launches++;
+  mark(2);
+
   TrackLaunch tl{};
   tl.geo = h->dev;
   tl.n_events = n_events;
   tl.clusters = *oc;
+  tl.slab = slab;
+  tl.slab_base = slab_base;
   if (tl.clusters.capacity > entries) tl.clusters.capacity = (uint32_t)entries;  // scratch is indexed by cluster
   tl.link = link;
   tl.hits_slab = hits_slab;
@@ -258,12 +286,12 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   uint32_t n_track_launches = 0;
   if ((err = launch_track(tl, stream, &n_track_launches)) != cudaSuccess) return fail(h, ALLEN_VELO_ERR_CUDA, "track kernel", err);
   h->last_launches += n_track_launches;
-  mark(2);
+  mark(3);
 
   if ((err = launch_scan_u64(trk_counts, trk_offsets, n_events, trk_scan_state, stream)) != cudaSuccess)
     return fail(h, ALLEN_VELO_ERR_CUDA, "track scan", err);
   h->last_launches++;
-  mark(3);
+  mark(4);
 
   CompactTracksLaunch ct{};
   ct.n_events = n_events;
@@ -275,7 +303,7 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   ct.out = *ot;
   if ((err = launch_compact_tracks(ct, stream)) != cudaSuccess) return fail(h, ALLEN_VELO_ERR_CUDA, "track compaction", err);
   h->last_launches++;
-  mark(4);
+  mark(5);
   return ALLEN_VELO_OK;
 }
 

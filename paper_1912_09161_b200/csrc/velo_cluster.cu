@@ -17,9 +17,11 @@
 // with shared-memory atomics (commutative integer adds / min: deterministic).
 //
 // The layer's clusters are ranked by (phi16, key) with a 256-bucket counting sort on the top byte of phi plus an exact
-// in-bucket rank.  The position of the layer in the compacted output comes from a decoupled look-back over the
-// (event, layer) items (one status word per item; the count is published before the sort so successors rarely wait),
-// and the layer is written once, coalesced, in its final place: no slab, no separate scan or compaction pass.
+// in-bucket rank and written, coalesced and in the normative order, to the layer's region of a slab whose position
+// depends only on the event's bank table (2 entries per SP word before the layer): warps never wait for one another.
+// (A decoupled look-back over the 260 k (event, layer) items that wrote the compacted output directly was measured
+// first: in-order publication made every warp wait for its slowest predecessor — 66 % of the issued instructions
+// were the spin — so compaction moved into the track kernel, which reads every hit anyway; profiles/README.md.)
 //
 // Capacities.  FAST: the layer's SP words fit the warp's shared memory (256).  MID: they do not, but every sensor
 // does: one pass per sensor group in shared memory, cluster records and sort scratch in a pool slot in global memory.
@@ -37,17 +39,6 @@ constexpr uint32_t kCapSp = 256, kHashBits = 9, kCapEdges = 256, kCapCl = 256;
 // pool slots in global memory
 constexpr uint32_t kMidCl = 1024;
 constexpr uint32_t kBigSp = 8192, kBigHashBits = 14, kBigEdges = 7 * kBigSp, kBigCl = 2 * kBigSp;
-
-constexpr unsigned long long kFlagAggregate = 1ull << 62, kFlagInclusive = 2ull << 62, kValueMask = (1ull << 62) - 1;
-
-__device__ __forceinline__ unsigned long long ld_status(const unsigned long long* p) {
-  unsigned long long v;
-  asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
-  return v;
-}
-__device__ __forceinline__ void st_status(unsigned long long* p, unsigned long long v) {
-  asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
-}
 
 // Storage of one clustering pass.  Staged SP word: hitmap | sp_row << 8 | sp_col << 14 | local sensor << 23; 0 = dead.
 struct Pass {
@@ -298,16 +289,18 @@ __device__ __forceinline__ bool ccl_pass(const Pass& p, const ClusterStore& cs, 
   return true;
 }
 
-// A3 + A4 + A9 for one layer whose n_cl cluster records are in `cs`: position and phi16, rank by (phi16, key),
-// look-back for the layer's place in the compacted output, coalesced write in the normative order.
+// A3 + A4 for one layer whose n_cl cluster records are in `cs`: position and phi16, rank by (phi16, key), coalesced
+// write in the normative order to the slab region [slab0, slab0 + n_cl).
 template <bool kChecksum>
 __device__ __forceinline__ void finish_layer(const ClusterLaunch& a, const ClusterStore& cs, const SortStore& ss,
-                                             uint32_t item, uint32_t e, uint32_t layer, uint32_t n_cl) {
+                                             uint32_t item, uint32_t slab0, uint32_t n_cl) {
   const DeviceGeometry& g = a.geo;
   const uint32_t lane = lane_id();
-  // the count goes out first: successors can add it up while this warp sorts
-  if (lane == 0) st_status(a.state + item, (item == 0 ? kFlagInclusive : kFlagAggregate) | n_cl);
-
+  if (lane == 0) {
+    a.counts[item] = n_cl;
+    a.slab_base[item] = slab0;
+  }
+  if (n_cl == 0) return;
   for (uint32_t s = lane; s < 256; s += 32) ss.cnt256[s] = 0;
   __syncwarp();
   for (uint32_t c = lane; c < n_cl; c += 32) {
@@ -348,59 +341,21 @@ __device__ __forceinline__ void finish_layer(const ClusterLaunch& a, const Clust
     ss.order[start + rank] = (uint16_t)c;
   }
   __syncwarp();
-
-  // ---- decoupled look-back over the items before this one
-  unsigned long long exclusive = 0;
-  if (item > 0) {
-    long long look = (long long)item - 1;
-    for (;;) {
-      const long long idx = look - (long long)lane;
-      unsigned long long s = kFlagInclusive;  // items before the first count as an inclusive prefix of 0
-      if (idx >= 0) {
-        do { s = ld_status(a.state + idx); } while ((s >> 62) == 0);
-      }
-      const uint32_t incl_mask = __ballot_sync(kFull, (s >> 62) == 2);
-      const int first = incl_mask ? __ffs(incl_mask) - 1 : 32;
-      unsigned long long part = (int)lane <= first ? (s & kValueMask) : 0ull;
-#pragma unroll
-      for (int d = 16; d; d >>= 1) part += __shfl_xor_sync(kFull, part, d);
-      exclusive += part;
-      if (incl_mask) break;
-      look -= 32;
-    }
-    if (lane == 0) st_status(a.state + item, kFlagInclusive | (exclusive + n_cl));
-  }
-  const uint32_t base = (uint32_t)exclusive;
-  const uint32_t n_items = a.n_events * g.n_layers;
-  if (lane == 0) {
-    a.out.layer_offsets[item] = base;
-    if (layer == 0) a.out.event_offsets[e] = base;
-    if (item + 1 == n_items) {
-      a.out.layer_offsets[n_items] = base + n_cl;
-      a.out.event_offsets[a.n_events] = base + n_cl;
-    }
-  }
-  if (n_cl == 0) return;
-  if (exclusive + n_cl > a.out.capacity) {
-    if (lane == 0) atomicOr(a.out.status + e, ALLEN_VELO_STATUS_CLUSTER_CAPACITY);
-    return;
-  }
-  // ---- the layer in the normative order, in its final place
   for (uint32_t j = lane; j < n_cl; j += 32) {
     const uint32_t c = ss.order[j];
     const uint32_t key = cs.key[c], n = cs.n[c], sc = cs.col[c], sr = cs.row[c];
     float x, y, z;
     cluster_position(n, sc, sr, g.pitch, g.ltg + 9 * (key >> 18), x, y, z);
-    const uint32_t o = base + j;
-    a.out.key[o] = key;
-    a.out.n_pixels[o] = n;
-    a.out.sum_col[o] = sc;
-    a.out.sum_row[o] = sr;
-    a.out.x[o] = x;
-    a.out.y[o] = y;
-    a.out.z[o] = z;
-    a.out.phi16[o] = (int16_t)(ss.phis[c] ^ 0x8000u);
-    if (kChecksum) a.out.checksum[o] = cs.cks[c];
+    const uint32_t o = slab0 + j;
+    a.slab.key[o] = key;
+    a.slab.n_pixels[o] = n;
+    a.slab.sum_col[o] = sc;
+    a.slab.sum_row[o] = sr;
+    a.slab.x[o] = x;
+    a.slab.y[o] = y;
+    a.slab.z[o] = z;
+    a.slab.phi16[o] = (int16_t)(ss.phis[c] ^ 0x8000u);
+    if (kChecksum) a.slab.checksum[o] = cs.cks[c];
   }
 }
 
@@ -414,8 +369,8 @@ __device__ __noinline__ bool ccl_pass_generic(const Pass& p, const ClusterStore&
 }
 template <bool kChecksum>
 __device__ __noinline__ void finish_layer_generic(const ClusterLaunch& a, const ClusterStore& cs, const SortStore& ss,
-                                                  uint32_t item, uint32_t e, uint32_t layer, uint32_t n_cl) {
-  finish_layer<kChecksum>(a, cs, ss, item, e, layer, n_cl);
+                                                  uint32_t item, uint32_t slab0, uint32_t n_cl) {
+  finish_layer<kChecksum>(a, cs, ss, item, slab0, n_cl);
 }
 
 template <bool kChecksum>
@@ -466,7 +421,6 @@ __global__ void __launch_bounds__(kWarps * 32) velo_cluster_kernel(const __grid_
   const DeviceGeometry& g = a.geo;
   const uint32_t lane = lane_id();
   const uint32_t L = g.n_layers;
-  // items are taken in blockIdx order: every predecessor of a running item is running or finished (look-back)
   const uint32_t item = blockIdx.x * kWarps + (threadIdx.x >> 5);
   if (item >= a.n_events * L) return;
   const uint32_t e = item / L, layer = item % L;
@@ -492,19 +446,24 @@ __global__ void __launch_bounds__(kWarps * 32) velo_cluster_kernel(const __grid_
     bad = bad || need != n_words;
   }
   const uint32_t* tbl = ev + 4;
+  uint32_t before = 0;  // SP words of this event in layers below `layer` (slab placement)
   if (!bad) {
     for (uint32_t j = lane; j < g.n_sensors; j += 32) {
       const uint32_t o0 = __ldg(tbl + j), o1 = __ldg(tbl + j + 1);
       bad = bad || o0 > o1 || (j == 0 && o0 != 0) || (j + 1 == g.n_sensors && o1 != n_sp_total);
+      if (__ldg(g.sensor_layer + j) < layer) before += o1 - o0;
     }
   }
   bad = __any_sync(kFull, bad);
   if (bad) {
-    if (lane == 0 && layer == 0) atomicOr(a.out.status + e, ALLEN_VELO_STATUS_BAD_HEADER);
-    finish_layer<kChecksum>(a, cs, ss, item, e, layer, 0);
+    if (lane == 0 && layer == 0) atomicOr(a.status + e, ALLEN_VELO_STATUS_BAD_HEADER);
+    finish_layer<kChecksum>(a, cs, ss, item, 0, 0);
     return;
   }
+  before = __reduce_add_sync(kFull, before);
   const uint32_t* spw = tbl + g.table_words;
+  // two slab entries per SP word (a super-pixel holds at most two clusters), placed by the raw position of the layer
+  const uint32_t slab0 = 2u * ((byte0 >> 2) + 4u + g.table_words + before);
 
   // sensors of this layer: lane k < K holds sensor k's bank range
   const uint32_t K = __ldg(g.layer_n_sensors + layer);
@@ -516,6 +475,11 @@ __global__ void __launch_bounds__(kWarps * 32) velo_cluster_kernel(const __grid_
   }
   const uint32_t n_sp_layer = __reduce_add_sync(kFull, my_cnt);
   const uint32_t max_cnt = __reduce_max_sync(kFull, my_cnt);
+  if ((unsigned long long)slab0 + 2ull * n_sp_layer > a.slab.capacity) {  // workspace smaller than workspace_bytes()
+    if (lane == 0) atomicOr(a.status + e, ALLEN_VELO_STATUS_STAGE_OVERFLOW);
+    finish_layer<kChecksum>(a, cs, ss, item, slab0, 0);
+    return;
+  }
 
   Pass fast;
   fast.sp = ws.sp; fast.tab = ws.tab; fast.lab = ws.lab; fast.edges = ws.edges;
@@ -526,8 +490,8 @@ __global__ void __launch_bounds__(kWarps * 32) velo_cluster_kernel(const __grid_
   int mode = n_sp_layer <= kCapSp ? 0 : (max_cnt <= kCapSp && n_sp_layer <= kMidCl) ? 1 : 2;
   if (mode == 0) {
     if (ccl_pass<kChecksum>(fast, cs, g, spw, my_sensor, my_off, my_cnt, 0, K, n_cl, bad_sp, &ws.n_edges)) {
-      if (__any_sync(kFull, bad_sp) && lane == 0) atomicOr(a.out.status + e, ALLEN_VELO_STATUS_BAD_SP);
-      finish_layer<kChecksum>(a, cs, ss, item, e, layer, n_cl);
+      if (__any_sync(kFull, bad_sp) && lane == 0) atomicOr(a.status + e, ALLEN_VELO_STATUS_BAD_SP);
+      finish_layer<kChecksum>(a, cs, ss, item, slab0, n_cl);
       return;
     }
     mode = 2;  // more clusters or edges than the warp's shared memory holds (not seen on physics-like input)
@@ -535,7 +499,7 @@ __global__ void __launch_bounds__(kWarps * 32) velo_cluster_kernel(const __grid_
   uint32_t held = 0xFFFFFFFFu;  // mid slot of this warp (released at the end)
   if (mode == 1) {
     // one slot per resident warp: bit b of mid_mask[sm] <-> slot 32 * sm + b.  A kernel with at most 32 resident warps
-    // per SM always finds a free bit, so nobody ever waits for a slot (a wait could deadlock the look-back).
+    // per SM always finds a free bit, so nobody ever waits for a slot.
     uint32_t slot = 0xFFFFFFFFu;
     if (lane == 0) {
       uint32_t sm;
@@ -595,12 +559,12 @@ __global__ void __launch_bounds__(kWarps * 32) velo_cluster_kernel(const __grid_
     }
   }
   if (overflow) {
-    if (lane == 0) atomicOr(a.out.status + e, ALLEN_VELO_STATUS_STAGE_OVERFLOW);
+    if (lane == 0) atomicOr(a.status + e, ALLEN_VELO_STATUS_STAGE_OVERFLOW);
     n_cl = 0;
   } else if (__any_sync(kFull, bad_sp) && lane == 0) {
-    atomicOr(a.out.status + e, ALLEN_VELO_STATUS_BAD_SP);
+    atomicOr(a.status + e, ALLEN_VELO_STATUS_BAD_SP);
   }
-  finish_layer_generic<kChecksum>(a, cs, ss, item, e, layer, n_cl);
+  finish_layer_generic<kChecksum>(a, cs, ss, item, slab0, n_cl);
   __syncwarp();
   if (held != 0xFFFFFFFFu && lane == 0) atomicAnd(a.mid_mask + (held >> 5), ~(1u << (held & 31u)));
 }

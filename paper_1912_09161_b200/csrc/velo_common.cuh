@@ -24,6 +24,15 @@ struct DeviceGeometry {
   allen_velo_params_t params;
 };
 
+// Slab the cluster kernel writes: structure of arrays with `capacity` entries; the region of (event, layer) starts at
+// slab_base[item] and holds counts[item] clusters in the normative order.  The track kernel moves it to the output.
+struct ClusterSlab {
+  uint32_t capacity;
+  uint32_t *key, *n_pixels, *sum_col, *sum_row, *checksum;
+  float *x, *y, *z;
+  int16_t* phi16;
+};
+
 // ---- small device helpers -------------------------------------------------------------------
 __device__ __forceinline__ uint32_t lane_id() { return threadIdx.x & 31u; }
 __device__ __forceinline__ uint32_t lanemask_lt() {
@@ -91,15 +100,17 @@ __device__ __forceinline__ float scatter(float xa, float ya, float za, float xb,
 __device__ __forceinline__ int dphi16(int16_t a, int16_t b) { return (int16_t)(uint16_t)((uint16_t)a - (uint16_t)b); }
 
 // ---- kernel launchers (defined in the .cu files) -----------------------------------------------
-// Cluster kernel: one warp per (event, layer); writes the compacted cluster output directly (decoupled look-back over
-// the items through `state`).  Layers that exceed the warp's shared memory use slots of the two pools.
+// Cluster kernel: one warp per (event, layer); writes the layer, sorted, to its slab region.  Layers that exceed the
+// warp's shared memory use slots of the two pools.
 struct ClusterLaunch {
   DeviceGeometry geo;
   const uint32_t* raw;
   const uint32_t* event_offsets;
   uint32_t n_events;
-  allen_velo_clusters_t out;
-  unsigned long long* state;  // [n_events*n_layers] look-back status words, zeroed before
+  ClusterSlab slab;
+  uint32_t* counts;           // [n_events*n_layers] clusters per (event, layer)
+  uint32_t* slab_base;        // [n_events*n_layers] first slab entry of the (event, layer) region
+  uint32_t* status;           // [n_events], zeroed before
   uint32_t* big_ctr;          // slots handed out of the big pool, zeroed before
   uint32_t* mid_mask;         // [n_mid_sms] busy bits of the mid slots of every SM, zeroed before
   unsigned char* mid_pool;    // [32 * n_mid_sms] slots
@@ -114,6 +125,8 @@ size_t cluster_big_slot_bytes();
 // Exclusive prefix sum of `in[n]` into `out[n+1]` (out[n] = total), single pass with decoupled look-back.
 // `tile_state` needs scan_state_words(n) u64 words, zeroed by the launcher.
 size_t scan_state_words(uint32_t n);
+cudaError_t launch_scan_u32(const uint32_t* in, uint32_t* out, uint32_t n, unsigned long long* tile_state,
+                            uint32_t* aux_out, uint32_t aux_stride, cudaStream_t stream);
 cudaError_t launch_scan_u64(const unsigned long long* in, unsigned long long* out, uint32_t n,
                             unsigned long long* tile_state, cudaStream_t stream);
 
@@ -123,7 +136,9 @@ cudaError_t launch_scan_u64(const unsigned long long* in, unsigned long long* ou
 struct TrackLaunch {
   DeviceGeometry geo;
   uint32_t n_events;
-  allen_velo_clusters_t clusters;  // final compacted clusters (inputs to the search)
+  allen_velo_clusters_t clusters;  // compacted cluster output: offsets final; the arrays are filled by this kernel
+  ClusterSlab slab;                // sorted layers as the cluster kernel left them
+  const uint32_t* slab_base;       // [n_events*n_layers]
   uint16_t* link;                  // [cluster capacity] scratch: previous (older) hit of the same track, per hit
   uint16_t* hits_slab;             // [cluster capacity] hit lists of the event's output tracks, back to back
   uint32_t* trk_hitoff;            // [capacity/3+1] event-local first entry in hits_slab of every output track

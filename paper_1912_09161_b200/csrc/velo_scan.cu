@@ -3,8 +3,9 @@
 //
 //  * scan_kernel: single-pass exclusive prefix sum with decoupled look-back (tile aggregates / inclusive prefixes
 //    published through one 64-bit status word per tile; tiles are claimed by an atomic ticket so that every
-//    predecessor of a running tile is itself running or finished).  The clusters need no such pass: the cluster
-//    kernel does its own look-back per (event, layer) and writes every layer in its final place.
+//    predecessor of a running tile is itself running or finished).  Used for the cluster counts per
+//    (event, layer) -> layer_offsets / event_offsets and for the (tracks, hits) counts per event.  The data moves are
+//    fused into the track kernel (clusters) and compact_tracks_kernel (tracks).
 #include "velo_common.cuh"
 
 namespace velo {
@@ -116,6 +117,11 @@ cudaError_t run_scan(const TIn* in, TOut* out, uint32_t n, unsigned long long* s
 }  // namespace
 
 size_t scan_state_words(uint32_t n) { return 1 + (size_t)(n + kTile - 1) / kTile; }
+
+cudaError_t launch_scan_u32(const uint32_t* in, uint32_t* out, uint32_t n, unsigned long long* tile_state,
+                            uint32_t* aux_out, uint32_t aux_stride, cudaStream_t stream) {
+  return run_scan<uint32_t, uint32_t>(in, out, n, tile_state, aux_out, aux_stride ? aux_stride : 1, stream);
+}
 
 cudaError_t launch_scan_u64(const unsigned long long* in, unsigned long long* out, uint32_t n,
                             unsigned long long* tile_state, cudaStream_t stream) {

@@ -13,6 +13,8 @@
 //    scans b's window on layer C; the per-b argmin is a 64-bit shared-memory atomicMin on (bits(S), a, c);
 //  * all conflict rules are order-independent minima on packed keys (bits(S) << 32 | index): no "first thread wins",
 //    so the result is exactly the oracle's whatever the thread schedule;
+//  * compaction of the clusters (A9) rides along: in the first instance a fifth warp copies the event's layers from
+//    the cluster kernel's slab to their final place while the four tracking warps (own named barrier) search;
 //  * the kernel is instantiated for three staging capacities (256 / 512 / 1024 hits per layer); every event is taken
 //    by the smallest instance it fits, and an instance that runs out of track slots hands the event to the next one.
 #include <cuda_pipeline.h>
@@ -32,7 +34,7 @@ struct __align__(16) Hit {
   uint32_t w;  // phi16 (low 16 bits, two's complement) | used << 16
 };
 
-template <int kThreads_, int kCap_, int kCapTracks_, int kCapDoublets_, int kLevel_, bool kLast_>
+template <int kThreads_, int kCap_, int kCapTracks_, int kCapDoublets_, int kLevel_, bool kLast_, bool kCopier_>
 struct Cfg {
   static constexpr int kThreads = kThreads_;
   static constexpr int kCap = kCap_;            // hits of one layer staged
@@ -40,13 +42,15 @@ struct Cfg {
   static constexpr int kCapDoublets = kCapDoublets_;
   static constexpr int kLevel = kLevel_;
   static constexpr bool kLast = kLast_;
+  static constexpr bool kCopier = kCopier_;      // an extra warp moves the event's clusters from the slab to the output
+  static constexpr int kBlock = kThreads + (kCopier ? 32 : 0);
   static constexpr int kWarps = kThreads / 32;
   static constexpr int kRoundsB = (kCap + kThreads - 1) / kThreads;
   static constexpr int kRoundsT = (kCapTracks + kThreads - 1) / kThreads;
 };
-using CfgS = Cfg<128, 256, 512, 512, 0, false>;
-using CfgM = Cfg<256, 512, 1024, 1024, 1, false>;
-using CfgL = Cfg<512, 1024, 2048, 2048, 2, true>;
+using CfgS = Cfg<128, 256, 512, 512, 0, false, true>;
+using CfgM = Cfg<256, 512, 1024, 1024, 1, false, false>;
+using CfgL = Cfg<512, 1024, 2048, 2048, 2, true, false>;
 
 template <class C>
 struct Smem {
@@ -59,6 +63,7 @@ struct Smem {
   uint16_t tseedB[C::kCapTracks];                // track_key: event-local index of the seed's middle hit
   uint16_t bucket[4][kBuckets + 2];
   uint32_t lo[kMaxLayers + 1];
+  uint32_t src[kMaxLayers];  // first entry of every layer in the arrays X, Y, Z, PHI are read from
   uint32_t warp_tot[C::kRoundsB > C::kRoundsT ? C::kRoundsB : C::kRoundsT][C::kWarps];
   uint32_t n_doublets;
   uint32_t min_active[2];
@@ -77,6 +82,13 @@ __device__ __forceinline__ uint32_t lower_bound_phi(const uint16_t* __restrict__
 
 __device__ __forceinline__ int wrap16(int v) { return (int)(int16_t)(uint16_t)v; }
 
+// Barrier over the tracking threads only (the copier warp, if any, runs on its own).
+template <class C>
+__device__ __forceinline__ void tsync() {
+  if (C::kCopier) asm volatile("bar.sync 1, %0;" ::"n"(C::kThreads) : "memory");
+  else __syncthreads();
+}
+
 template <class C>
 struct Ctx {
   Smem<C>& sm;
@@ -92,7 +104,7 @@ struct Ctx {
 template <class C>
 __device__ __forceinline__ void stage_layer(const Ctx<C>& c, uint32_t l) {
   Smem<C>& sm = c.sm;
-  const uint32_t base = sm.lo[l], n = sm.lo[l + 1] - base;
+  const uint32_t base = sm.src[l], n = sm.lo[l + 1] - sm.lo[l];
   Hit* rec = sm.rec[l & 3];
   uint16_t* bucket = sm.bucket[l & 3];
   if (n == 0) {
@@ -145,8 +157,23 @@ __device__ __forceinline__ void process_doublet(const Ctx<C>& c, const Hit* __re
   if (best != kNoClaim) atomicMin(&c.sm.best[kb], best);
 }
 
+// Copy clusters [k0, k1) of layer l (layer-local indices) from the slab to the compacted output.
+__device__ __forceinline__ void copy_clusters(const TrackLaunch& a, uint32_t src, uint32_t dst, uint32_t n,
+                                              uint32_t first, uint32_t step) {
+  for (uint32_t k = first; k < n; k += step) {
+    const uint32_t s = src + k, d = dst + k;
+    const uint32_t key = __ldg(a.slab.key + s), np = __ldg(a.slab.n_pixels + s);
+    const uint32_t sc = __ldg(a.slab.sum_col + s), sr = __ldg(a.slab.sum_row + s);
+    const float x = __ldg(a.slab.x + s), y = __ldg(a.slab.y + s), z = __ldg(a.slab.z + s);
+    const int16_t ph = __ldg(a.slab.phi16 + s);
+    a.clusters.key[d] = key; a.clusters.n_pixels[d] = np; a.clusters.sum_col[d] = sc; a.clusters.sum_row[d] = sr;
+    a.clusters.x[d] = x; a.clusters.y[d] = y; a.clusters.z[d] = z; a.clusters.phi16[d] = ph;
+    if (a.clusters.checksum) a.clusters.checksum[d] = __ldg(a.slab.checksum + s);
+  }
+}
+
 template <class C>
-__global__ void __launch_bounds__(C::kThreads) velo_track_kernel(const __grid_constant__ TrackLaunch a) {
+__global__ void __launch_bounds__(C::kBlock) velo_track_kernel(const __grid_constant__ TrackLaunch a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   Smem<C>& sm = *reinterpret_cast<Smem<C>*>(smem_raw);
   const DeviceGeometry& g = a.geo;
@@ -156,25 +183,30 @@ __global__ void __launch_bounds__(C::kThreads) velo_track_kernel(const __grid_co
   const uint32_t co = a.clusters.event_offsets[e];
   const uint32_t n_cl = a.clusters.event_offsets[e + 1] - co;
   const uint32_t st0 = a.clusters.status[e];
-  // events whose clusters were not produced or not written take no part in tracking
-  const bool skip = (st0 & (ALLEN_VELO_STATUS_BAD_HEADER | ALLEN_VELO_STATUS_TOO_MANY_CLUSTERS |
-                            ALLEN_VELO_STATUS_CLUSTER_CAPACITY | ALLEN_VELO_STATUS_STAGE_OVERFLOW)) != 0;
-  if (skip || n_cl == 0 || n_cl > 65535u || (unsigned long long)co + n_cl > a.clusters.capacity) {
+  if (n_cl == 0) {
+    if (C::kLevel == 0 && tid == 0) a.counts[e] = 0;
+    return;
+  }
+  if ((unsigned long long)co + n_cl > a.clusters.capacity) {  // the output (or the per-cluster scratch) cannot hold it
     if (C::kLevel == 0 && tid == 0) {
-      if (!skip && n_cl > 65535u) atomicOr(a.clusters.status + e, ALLEN_VELO_STATUS_TOO_MANY_CLUSTERS);  // hits are u16
-      else if (!skip && n_cl) atomicOr(a.clusters.status + e, ALLEN_VELO_STATUS_STAGE_OVERFLOW);  // scratch is per cluster
+      atomicOr(a.clusters.status + e, ALLEN_VELO_STATUS_CLUSTER_CAPACITY);
       a.counts[e] = 0;
     }
     return;
   }
+  // events whose clusters are incomplete, or too many for 16-bit hit indices, take no part in tracking
+  const bool skip = (st0 & (ALLEN_VELO_STATUS_BAD_HEADER | ALLEN_VELO_STATUS_STAGE_OVERFLOW)) != 0 || n_cl > 65535u;
   // ---- which instance takes this event: the smallest whose staging capacity holds its busiest layer, unless a
   //      smaller instance ran out of track slots and passed it on (level[e])
   if (tid == 0) sm.flags = 0;
-  for (uint32_t l = tid; l <= L; l += C::kThreads) sm.lo[l] = a.clusters.layer_offsets[e * L + l] - co;
+  for (uint32_t l = tid; l <= L; l += C::kBlock) sm.lo[l] = a.clusters.layer_offsets[e * L + l] - co;
+  // the instance with the copier reads the slab the cluster kernel wrote; the others the output it has filled
+  for (uint32_t l = tid; l < L; l += C::kBlock)
+    sm.src[l] = C::kCopier ? a.slab_base[e * L + l] : a.clusters.layer_offsets[e * L + l];
   __syncthreads();
   {
     uint32_t mx = 0;
-    for (uint32_t l = tid; l < L; l += C::kThreads) mx = max(mx, sm.lo[l + 1] - sm.lo[l]);
+    for (uint32_t l = tid; l < L; l += C::kBlock) mx = max(mx, sm.lo[l + 1] - sm.lo[l]);
     if (mx) atomicMax(&sm.flags, mx);
   }
   __syncthreads();
@@ -182,17 +214,34 @@ __global__ void __launch_bounds__(C::kThreads) velo_track_kernel(const __grid_co
   const uint32_t natural = max_layer <= (uint32_t)CfgS::kCap ? 0u : max_layer <= (uint32_t)CfgM::kCap ? 1u : 2u;
   const uint32_t level = max(natural, (uint32_t)a.level[e]);  // level[e]: 0 unless raised by a smaller instance
   const bool fits = max_layer <= (uint32_t)C::kCap;
-  if (level != (uint32_t)C::kLevel || !fits) {
-    if (C::kLast && !fits && tid == 0) {  // busiest layer beyond the largest staging capacity
-      atomicOr(a.clusters.status + e, ALLEN_VELO_STATUS_STAGE_OVERFLOW);
-      a.counts[e] = 0;
+  const bool take = !skip && level == (uint32_t)C::kLevel && fits;
+  __syncthreads();  // everyone has read sm.flags
+  if (!take) {
+    if (C::kCopier)  // the output is still to be filled: the whole CTA moves the event
+      for (uint32_t l = 0; l < L; ++l)
+        copy_clusters(a, sm.src[l], co + sm.lo[l], sm.lo[l + 1] - sm.lo[l], tid, C::kBlock);
+    if (tid == 0) {
+      if (C::kLevel == 0 && n_cl > 65535u) atomicOr(a.clusters.status + e, ALLEN_VELO_STATUS_TOO_MANY_CLUSTERS);
+      if (C::kLevel == 0 && skip) a.counts[e] = 0;
+      if (C::kLast && !skip && !fits) {  // busiest layer beyond the largest staging capacity
+        atomicOr(a.clusters.status + e, ALLEN_VELO_STATUS_STAGE_OVERFLOW);
+        a.counts[e] = 0;
+      }
     }
     return;
   }
-  __syncthreads();
+  if (C::kCopier && tid >= (uint32_t)C::kThreads) {
+    // copier warp: layers in the order the search stages them (their slab lines are then in L2 for both readers)
+    for (int l = (int)L - 1; l >= 0; --l)
+      copy_clusters(a, sm.src[l], co + sm.lo[l], sm.lo[l + 1] - sm.lo[l], lane, 32);
+    __syncthreads();  // pairs with the barrier before the fit: the output arrays are complete
+    return;
+  }
   if (tid == 0) { sm.flags = 0; sm.min_active[0] = 0; sm.min_active[1] = 0; }
 
-  Ctx<C> c{sm, a.clusters.x + co, a.clusters.y + co, a.clusters.z + co, a.clusters.phi16 + co, g.params};
+  Ctx<C> c{sm,
+           C::kCopier ? a.slab.x : a.clusters.x, C::kCopier ? a.slab.y : a.clusters.y,
+           C::kCopier ? a.slab.z : a.clusters.z, C::kCopier ? a.slab.phi16 : a.clusters.phi16, g.params};
   const allen_velo_params_t& P = c.P;
   uint16_t* link = a.link + co;
 
@@ -216,7 +265,7 @@ __global__ void __launch_bounds__(C::kThreads) velo_track_kernel(const __grid_co
     const uint16_t* bucketC = sm.bucket[(i - 2) & 3];
 
     __pipeline_wait_prior(0);
-    __syncthreads();  // B1: layer C staged; tracks created by the previous T4 visible; claims re-initialised
+    tsync<C>();  // B1: layer C staged; tracks created by the previous T4 visible; claims re-initialised
     if (i >= 3) stage_layer(c, (uint32_t)i - 3);  // prefetch: needed at the top of the next iteration
 
     // ---- T1 forward: best hit of layer C per active track (nothing of C is used yet); claim with (bits(S), key)
@@ -240,7 +289,10 @@ __global__ void __launch_bounds__(C::kThreads) velo_track_kernel(const __grid_co
         const Hit hq = q >= A0 ? recA[q - A0] : recB[q - B0];
         xq = hq.x; yq = hq.y; zq = hq.z; phq = phi_of(hq.w);
       } else {       // tracks that skipped more than one layer: their last hit left the ring
-        xq = __ldg(c.X + q); yq = __ldg(c.Y + q); zq = __ldg(c.Z + q); phq = (int)__ldg(c.PHI + q);
+        uint32_t l = (uint32_t)i + 1;
+        while (q >= sm.lo[l + 1]) ++l;
+        const uint32_t s = sm.src[l] + (q - sm.lo[l]);
+        xq = __ldg(c.X + s); yq = __ldg(c.Y + s); zq = __ldg(c.Z + s); phq = (int)__ldg(c.PHI + s);
       }
       const float tx = sm.ttx[t], ty = sm.tty[t];
       const int w = P.w_fwd_phi16;
@@ -265,7 +317,7 @@ __global__ void __launch_bounds__(C::kThreads) velo_track_kernel(const __grid_co
         atomicMin(&sm.best[fc[r]], fkey[r]);
       }
     }
-    __syncthreads();  // B2
+    tsync<C>();  // B2
     // ---- T2 resolve: the minimal claim wins the hit; everyone else counts a miss
 #pragma unroll
     for (int r = 0; r < C::kRoundsT; ++r) {
@@ -282,7 +334,10 @@ __global__ void __launch_bounds__(C::kThreads) velo_track_kernel(const __grid_co
           const Hit hq = q >= A0 ? recA[q - A0] : recB[q - B0];
           xq = hq.x; yq = hq.y; zq = hq.z;
         } else {
-          xq = __ldg(c.X + q); yq = __ldg(c.Y + q); zq = __ldg(c.Z + q);
+          uint32_t l = (uint32_t)i + 1;
+          while (q >= sm.lo[l + 1]) ++l;
+          const uint32_t s = sm.src[l] + (q - sm.lo[l]);
+          xq = __ldg(c.X + s); yq = __ldg(c.Y + s); zq = __ldg(c.Z + s);
         }
         const Hit hc = recC[fc[r]];
         const float dz = __fsub_rn(hc.z, zq);
@@ -303,7 +358,7 @@ __global__ void __launch_bounds__(C::kThreads) velo_track_kernel(const __grid_co
         }
       }
     }
-    __syncthreads();  // B3
+    tsync<C>();  // B3
 
     // ---- T3/S1: every unused b lists the unused hits of layer A inside its phi window as (b, a) doublets
     const bool seeding = nA != 0 && nB != 0 && nC != 0;
@@ -327,7 +382,7 @@ __global__ void __launch_bounds__(C::kThreads) velo_track_kernel(const __grid_co
         else process_doublet(c, recA, recB, recC, bucketC, nC, kb, ia);  // list full: do it here (same result)
       }
     }
-    __syncthreads();  // B4
+    tsync<C>();  // B4
     // ---- T3/S2: one thread per doublet
     {
       const uint32_t nd = min(sm.n_doublets, (uint32_t)C::kCapDoublets);
@@ -336,7 +391,7 @@ __global__ void __launch_bounds__(C::kThreads) velo_track_kernel(const __grid_co
         process_doublet(c, recA, recB, recC, bucketC, nC, v & 0xFFFFu, v >> 16);
       }
     }
-    __syncthreads();  // B5
+    tsync<C>();  // B5
 
     // ---- T4a: every b with a triplet claims its a and its c with (bits(S), b)
     unsigned long long tkey[C::kRoundsB];
@@ -354,7 +409,7 @@ __global__ void __launch_bounds__(C::kThreads) velo_track_kernel(const __grid_co
       atomicMin(&sm.claimA[tac[r] >> 16], tkey[r]);
       atomicMin(&sm.claimC[tac[r] & 0xFFFFu], tkey[r]);
     }
-    __syncthreads();  // B6
+    tsync<C>();  // B6
     // ---- T4b: accepted iff the triplet holds the minimal key on both its a and its c; new tracks take slots in
     //      ascending b (ballot + per-warp totals)
     uint32_t acc_ballot[C::kRoundsB];
@@ -365,7 +420,7 @@ __global__ void __launch_bounds__(C::kThreads) velo_track_kernel(const __grid_co
       acc_ballot[r] = __ballot_sync(kFull, accepted);
       if (lane == 0) sm.warp_tot[r][warp] = __popc(acc_ballot[r]);
     }
-    __syncthreads();  // B7
+    tsync<C>();  // B7
     first_new = n_tracks;
     {
       uint32_t run = n_tracks;
@@ -421,9 +476,11 @@ __global__ void __launch_bounds__(C::kThreads) velo_track_kernel(const __grid_co
   // ---- T5 finalise + A8 fit: keep >= 4 hits, or 3 hits with S_seed <= s_weak; output in order of creation
   uint32_t out_tracks = 0, out_hits = 0;
   const uint32_t trk0 = co / 3;
-  const float* __restrict__ X = c.X;
-  const float* __restrict__ Y = c.Y;
-  const float* __restrict__ Z = c.Z;
+  // the fit reads the compacted output (complete: the copier warp passed the barrier above, or an earlier kernel
+  // filled it); __ldcg because these lines may have been written during this kernel
+  const float* X = a.clusters.x + co;
+  const float* Y = a.clusters.y + co;
+  const float* Z = a.clusters.z + co;
   for (uint32_t base = 0; base < n_tracks; base += C::kThreads) {
     const uint32_t t = base + tid;
     uint32_t n = 0, st = 0;
@@ -440,9 +497,9 @@ __global__ void __launch_bounds__(C::kThreads) velo_track_kernel(const __grid_co
       const uint32_t u = __shfl_up_sync(kFull, incl, d);
       if (lane >= (uint32_t)d) incl += u;
     }
-    __syncthreads();
+    tsync<C>();
     if (lane == 31) sm.warp_tot[0][warp] = incl;
-    __syncthreads();
+    tsync<C>();
     uint32_t off = incl - v, total = 0;
 #pragma unroll
     for (int w = 0; w < C::kWarps; ++w) {
@@ -457,7 +514,7 @@ __global__ void __launch_bounds__(C::kThreads) velo_track_kernel(const __grid_co
       uint32_t h = st >> 16;
       for (int k = (int)n - 1; k >= 0; --k) {
         a.hits_slab[co + oh + k] = (uint16_t)h;
-        sz += (double)__ldg(Z + h); sx += (double)__ldg(X + h); sy += (double)__ldg(Y + h);
+        sz += (double)__ldcg(Z + h); sx += (double)__ldcg(X + h); sy += (double)__ldcg(Y + h);
         if (k) h = link[h];
       }
       const double inv = 1.0 / (double)n;
@@ -465,10 +522,10 @@ __global__ void __launch_bounds__(C::kThreads) velo_track_kernel(const __grid_co
       double szz = 0, szx = 0, szy = 0;
       h = st >> 16;
       for (int k = (int)n - 1; k >= 0; --k) {
-        const double dz = (double)__ldg(Z + h) - zm;
+        const double dz = (double)__ldcg(Z + h) - zm;
         szz += dz * dz;
-        szx += dz * ((double)__ldg(X + h) - xm);
-        szy += dz * ((double)__ldg(Y + h) - ym);
+        szx += dz * ((double)__ldcg(X + h) - xm);
+        szy += dz * ((double)__ldcg(Y + h) - ym);
         if (k) h = link[h];
       }
       const double tx = szx / szz, ty = szy / szz;
@@ -514,7 +571,7 @@ cudaError_t launch_instance(const TrackLaunch& a, cudaStream_t stream) {
                                          (int)sizeof(Smem<C>));
   static_assert(sizeof(Smem<C>) <= 227 * 1024, "shared memory of one CTA");
   if (err != cudaSuccess) return err;
-  velo_track_kernel<C><<<a.n_events, C::kThreads, sizeof(Smem<C>), stream>>>(a);
+  velo_track_kernel<C><<<a.n_events, C::kBlock, sizeof(Smem<C>), stream>>>(a);
   return cudaGetLastError();
 }
 
