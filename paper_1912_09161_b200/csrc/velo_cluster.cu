@@ -63,6 +63,7 @@ __device__ __forceinline__ uint32_t hash_slot(uint32_t key, uint32_t bits) { ret
 __device__ __forceinline__ int lookup(const uint32_t* tab, uint32_t bits, uint32_t key) {
   const uint32_t mask = (1u << bits) - 1u;
   uint32_t s = hash_slot(key, bits);
+#pragma unroll 1
   for (;;) {
     const uint32_t e = tab[s];
     if (e == 0) return -1;
@@ -99,6 +100,7 @@ __device__ __forceinline__ Stats comp_stats(uint32_t m, uint32_t C, uint32_t R, 
   s.cks = 0;
   if (kChecksum) {
     uint32_t mm = m;
+#pragma unroll 1
     while (mm) {
       const uint32_t b = __ffs(mm) - 1;
       mm &= mm - 1;
@@ -120,8 +122,10 @@ __device__ __forceinline__ bool ccl_pass(const Pass& p, const ClusterStore& cs, 
   const uint32_t bits = p.hash_bits;
   // ---- stage the SP words of the group (R1: addresses outside the sensor are ignored and flagged)
   uint32_t n = 0;
+#pragma unroll 1
   for (uint32_t k = k0; k < k1; ++k) {
     const uint32_t off = __shfl_sync(kFull, my_off, k), cnt = __shfl_sync(kFull, my_cnt, k);
+#pragma unroll 1
     for (uint32_t i = lane; i < cnt; i += 32) {
       const uint32_t w = __ldg(spw + off + i);
       const uint32_t R = (w >> 8) & 0x3Fu, C = (w >> 14) & 0x1FFu;
@@ -132,17 +136,20 @@ __device__ __forceinline__ bool ccl_pass(const Pass& p, const ClusterStore& cs, 
     }
     n += cnt;
   }
+#pragma unroll 1
   for (uint32_t s = lane; s < (1u << bits); s += 32) p.tab[s] = 0;
   if (lane == 0) *n_edges_ctr = 0;
   __syncwarp();
 
   // ---- insert: entry = key << 14 | (index + 1); a repeated address merges its hitmap into the first one (R1)
   const uint32_t mask = (1u << bits) - 1u;
+#pragma unroll 1
   for (uint32_t i = lane; i < n; i += 32) {
     const uint32_t w = p.sp[i];
     if (!w) continue;
     const uint32_t key = (w >> 8) & 0x3FFFFu;
     uint32_t s = hash_slot(key, bits);
+#pragma unroll 1
     for (;;) {
       const uint32_t old = atomicCAS(p.tab + s, 0u, (key << 14) | (i + 1));
       if (old == 0) break;
@@ -157,6 +164,7 @@ __device__ __forceinline__ bool ccl_pass(const Pass& p, const ClusterStore& cs, 
   __syncwarp();
 
   // ---- edges to touching forward neighbours; node = 2 * index + component
+#pragma unroll 1
   for (uint32_t i = lane; i < n; i += 32) {
     const uint32_t w = p.sp[i];
     if (!w) continue;
@@ -217,8 +225,10 @@ __device__ __forceinline__ bool ccl_pass(const Pass& p, const ClusterStore& cs, 
 
   // ---- propagate the minimum node id over the edges until nothing changes (exact for any cluster size)
   if (n_edges) {
+#pragma unroll 1
     for (;;) {
       bool changed = false;
+#pragma unroll 1
       for (uint32_t j = lane; j < n_edges; j += 32) {
         const uint32_t uv = p.edges[j];
         const uint32_t u = uv & 0xFFFFu, v = uv >> 16;
@@ -234,6 +244,7 @@ __device__ __forceinline__ bool ccl_pass(const Pass& p, const ClusterStore& cs, 
   // ---- roots take cluster ids (ballot order) and store their own sums; cidmap[node] = id
   uint16_t* cidmap = reinterpret_cast<uint16_t*>(p.edges);
   bool any_child = false;
+#pragma unroll 1
   for (uint32_t i0 = 0; i0 < n; i0 += 32) {
     const uint32_t i = i0 + lane;
     const uint32_t w = i < n ? p.sp[i] : 0u;
@@ -265,6 +276,7 @@ __device__ __forceinline__ bool ccl_pass(const Pass& p, const ClusterStore& cs, 
   __syncwarp();
   // ---- non-root components add their sums to the root's record
   if (__any_sync(kFull, any_child)) {
+#pragma unroll 1
     for (uint32_t i = lane; i < n; i += 32) {
       const uint32_t w = p.sp[i];
       if (!w) continue;
@@ -301,8 +313,10 @@ __device__ __forceinline__ void finish_layer(const ClusterLaunch& a, const Clust
     a.slab_base[item] = slab0;
   }
   if (n_cl == 0) return;
+#pragma unroll 1
   for (uint32_t s = lane; s < 256; s += 32) ss.cnt256[s] = 0;
   __syncwarp();
+#pragma unroll 1
   for (uint32_t c = lane; c < n_cl; c += 32) {
     float x, y, z;
     cluster_position(cs.n[c], cs.col[c], cs.row[c], g.pitch, g.ltg + 9 * (cs.key[c] >> 18), x, y, z);
@@ -326,14 +340,17 @@ __device__ __forceinline__ void finish_layer(const ClusterLaunch& a, const Clust
     for (int q = 0; q < 8; ++q) { ss.cnt256[lane * 8 + q] = run; run += v[q]; }
   }
   __syncwarp();
+#pragma unroll 1
   for (uint32_t c = lane; c < n_cl; c += 32) ss.tmp[atomicAdd(&ss.cnt256[ss.phis[c] >> 8], 1u)] = (uint16_t)c;
   __syncwarp();
+#pragma unroll 1
   for (uint32_t j = lane; j < n_cl; j += 32) {
     const uint32_t c = ss.tmp[j];
     const uint32_t b = ss.phis[c] >> 8;
     const uint32_t start = b ? ss.cnt256[b - 1] : 0, end = ss.cnt256[b];
     const unsigned long long mine = ((unsigned long long)ss.phis[c] << 32) | cs.key[c];
     uint32_t rank = 0;
+#pragma unroll 1
     for (uint32_t q = start; q < end; ++q) {
       const uint32_t o = ss.tmp[q];
       rank += (((unsigned long long)ss.phis[o] << 32) | cs.key[o]) < mine;
@@ -341,6 +358,7 @@ __device__ __forceinline__ void finish_layer(const ClusterLaunch& a, const Clust
     ss.order[start + rank] = (uint16_t)c;
   }
   __syncwarp();
+#pragma unroll 1
   for (uint32_t j = lane; j < n_cl; j += 32) {
     const uint32_t c = ss.order[j];
     const uint32_t key = cs.key[c], n = cs.n[c], sc = cs.col[c], sr = cs.row[c];
@@ -448,6 +466,7 @@ __global__ void __launch_bounds__(kWarps * 32) velo_cluster_kernel(const __grid_
   const uint32_t* tbl = ev + 4;
   uint32_t before = 0;  // SP words of this event in layers below `layer` (slab placement)
   if (!bad) {
+#pragma unroll 1
     for (uint32_t j = lane; j < g.n_sensors; j += 32) {
       const uint32_t o0 = __ldg(tbl + j), o1 = __ldg(tbl + j + 1);
       bad = bad || o0 > o1 || (j == 0 && o0 != 0) || (j + 1 == g.n_sensors && o1 != n_sp_total);
@@ -505,6 +524,7 @@ __global__ void __launch_bounds__(kWarps * 32) velo_cluster_kernel(const __grid_
       uint32_t sm;
       asm volatile("mov.u32 %0, %%smid;" : "=r"(sm));
       if (sm < a.n_mid_sms) {
+#pragma unroll 1
         for (;;) {
           const uint32_t free_bits = ~*reinterpret_cast<volatile uint32_t*>(a.mid_mask + sm);
           if (!free_bits) break;
@@ -523,8 +543,10 @@ __global__ void __launch_bounds__(kWarps * 32) velo_cluster_kernel(const __grid_
       n_cl = 0;
       bad_sp = false;
       bool ok = true;
+#pragma unroll 1
       for (uint32_t k0 = 0; k0 < K && ok;) {  // greedy groups of consecutive sensors that fit the shared memory
         uint32_t k1 = k0, sum = 0;
+#pragma unroll 1
         while (k1 < K) {
           const uint32_t cnt = __shfl_sync(kFull, my_cnt, k1);
           if (sum + cnt > kCapSp) break;

@@ -76,6 +76,7 @@ __device__ __forceinline__ int phi_of(uint32_t w) { return (int)(int16_t)(uint16
 __device__ __forceinline__ uint32_t lower_bound_phi(const uint16_t* __restrict__ bucket, const Hit* __restrict__ rec,
                                                     uint32_t n, int target) {
   uint32_t idx = bucket[((uint32_t)(target + 32768) & 0xFFFFu) >> kBucketShift];
+#pragma unroll 1
   while (idx < n && phi_of(rec[idx].w) < target) ++idx;
   return idx;
 }
@@ -108,9 +109,11 @@ __device__ __forceinline__ void stage_layer(const Ctx<C>& c, uint32_t l) {
   Hit* rec = sm.rec[l & 3];
   uint16_t* bucket = sm.bucket[l & 3];
   if (n == 0) {
+#pragma unroll 1
     for (uint32_t b = threadIdx.x; b <= (uint32_t)kBuckets; b += C::kThreads) bucket[b] = 0;
     return;
   }
+#pragma unroll 1
   for (uint32_t k = threadIdx.x; k < n; k += C::kThreads) {
     __pipeline_memcpy_async(&rec[k].x, c.X + base + k, 4);
     __pipeline_memcpy_async(&rec[k].y, c.Y + base + k, 4);
@@ -119,8 +122,10 @@ __device__ __forceinline__ void stage_layer(const Ctx<C>& c, uint32_t l) {
     rec[k].w = ph;
     const int bk = (int)((ph ^ 0x8000u) >> kBucketShift);
     const int bp = k ? (int)((((uint32_t)(uint16_t)__ldg(c.PHI + base + k - 1)) ^ 0x8000u) >> kBucketShift) : -1;
+#pragma unroll 1
     for (int b = bp + 1; b <= bk; ++b) bucket[b] = (uint16_t)k;
     if (k + 1 == n)
+#pragma unroll 1
       for (int b = bk + 1; b <= kBuckets; ++b) bucket[b] = (uint16_t)n;
   }
   __pipeline_commit();
@@ -139,6 +144,7 @@ __device__ __forceinline__ void process_doublet(const Ctx<C>& c, const Hit* __re
   const int w = c.P.w_seed_phi16, phb = phi_of(hb.w);
   uint32_t ic = lower_bound_phi(bucketC, recC, nC, wrap16(phb - w));
   unsigned long long best = kNoClaim;
+#pragma unroll 1
   for (uint32_t k = 0; k < nC; ++k, ++ic) {
     if (ic >= nC) ic -= nC;
     const Hit hc = recC[ic];
@@ -160,6 +166,7 @@ __device__ __forceinline__ void process_doublet(const Ctx<C>& c, const Hit* __re
 // Copy clusters [k0, k1) of layer l (layer-local indices) from the slab to the compacted output.
 __device__ __forceinline__ void copy_clusters(const TrackLaunch& a, uint32_t src, uint32_t dst, uint32_t n,
                                               uint32_t first, uint32_t step) {
+#pragma unroll 1
   for (uint32_t k = first; k < n; k += step) {
     const uint32_t s = src + k, d = dst + k;
     const uint32_t key = __ldg(a.slab.key + s), np = __ldg(a.slab.n_pixels + s);
@@ -199,13 +206,16 @@ __global__ void __launch_bounds__(C::kBlock) velo_track_kernel(const __grid_cons
   // ---- which instance takes this event: the smallest whose staging capacity holds its busiest layer, unless a
   //      smaller instance ran out of track slots and passed it on (level[e])
   if (tid == 0) sm.flags = 0;
+#pragma unroll 1
   for (uint32_t l = tid; l <= L; l += C::kBlock) sm.lo[l] = a.clusters.layer_offsets[e * L + l] - co;
   // the instance with the copier reads the slab the cluster kernel wrote; the others the output it has filled
+#pragma unroll 1
   for (uint32_t l = tid; l < L; l += C::kBlock)
     sm.src[l] = C::kCopier ? a.slab_base[e * L + l] : a.clusters.layer_offsets[e * L + l];
   __syncthreads();
   {
     uint32_t mx = 0;
+#pragma unroll 1
     for (uint32_t l = tid; l < L; l += C::kBlock) mx = max(mx, sm.lo[l + 1] - sm.lo[l]);
     if (mx) atomicMax(&sm.flags, mx);
   }
@@ -218,6 +228,7 @@ __global__ void __launch_bounds__(C::kBlock) velo_track_kernel(const __grid_cons
   __syncthreads();  // everyone has read sm.flags
   if (!take) {
     if (C::kCopier)  // the output is still to be filled: the whole CTA moves the event
+#pragma unroll 1
       for (uint32_t l = 0; l < L; ++l)
         copy_clusters(a, sm.src[l], co + sm.lo[l], sm.lo[l + 1] - sm.lo[l], tid, C::kBlock);
     if (tid == 0) {
@@ -232,6 +243,7 @@ __global__ void __launch_bounds__(C::kBlock) velo_track_kernel(const __grid_cons
   }
   if (C::kCopier && tid >= (uint32_t)C::kThreads) {
     // copier warp: layers in the order the search stages them (their slab lines are then in L2 for both readers)
+#pragma unroll 1
     for (int l = (int)L - 1; l >= 0; --l)
       copy_clusters(a, sm.src[l], co + sm.lo[l], sm.lo[l + 1] - sm.lo[l], lane, 32);
     __syncthreads();  // pairs with the barrier before the fit: the output arrays are complete
@@ -245,6 +257,7 @@ __global__ void __launch_bounds__(C::kBlock) velo_track_kernel(const __grid_cons
   const allen_velo_params_t& P = c.P;
   uint16_t* link = a.link + co;
 
+#pragma unroll 1
   for (uint32_t k = tid; k < (uint32_t)C::kCap; k += C::kThreads) {
     sm.best[k] = kNoClaim; sm.claimA[k] = kNoClaim; sm.claimC[k] = kNoClaim;
   }
@@ -255,6 +268,7 @@ __global__ void __launch_bounds__(C::kBlock) velo_track_kernel(const __grid_cons
   uint32_t n_tracks = 0;        // block-uniform
   uint32_t first_new = 0;       // n_tracks before the latest T4 (block-uniform)
 
+#pragma unroll 1
   for (int i = (int)L - 1; i >= 2; --i) {
     const uint32_t A0 = sm.lo[i], A1 = sm.lo[i + 1], B0 = sm.lo[i - 1], C0 = sm.lo[i - 2];
     const uint32_t nA = A1 - A0, nB = A0 - B0, nC = B0 - C0;
@@ -290,6 +304,7 @@ __global__ void __launch_bounds__(C::kBlock) velo_track_kernel(const __grid_cons
         xq = hq.x; yq = hq.y; zq = hq.z; phq = phi_of(hq.w);
       } else {       // tracks that skipped more than one layer: their last hit left the ring
         uint32_t l = (uint32_t)i + 1;
+#pragma unroll 1
         while (q >= sm.lo[l + 1]) ++l;
         const uint32_t s = sm.src[l] + (q - sm.lo[l]);
         xq = __ldg(c.X + s); yq = __ldg(c.Y + s); zq = __ldg(c.Z + s); phq = (int)__ldg(c.PHI + s);
@@ -298,6 +313,7 @@ __global__ void __launch_bounds__(C::kBlock) velo_track_kernel(const __grid_cons
       const int w = P.w_fwd_phi16;
       uint32_t ic = lower_bound_phi(bucketC, recC, nC, wrap16(phq - w));
       unsigned long long best = kNoClaim;
+#pragma unroll 1
       for (uint32_t k = 0; k < nC; ++k, ++ic) {
         if (ic >= nC) ic -= nC;
         const Hit hc = recC[ic];
@@ -335,6 +351,7 @@ __global__ void __launch_bounds__(C::kBlock) velo_track_kernel(const __grid_cons
           xq = hq.x; yq = hq.y; zq = hq.z;
         } else {
           uint32_t l = (uint32_t)i + 1;
+#pragma unroll 1
           while (q >= sm.lo[l + 1]) ++l;
           const uint32_t s = sm.src[l] + (q - sm.lo[l]);
           xq = __ldg(c.X + s); yq = __ldg(c.Y + s); zq = __ldg(c.Z + s);
@@ -371,6 +388,7 @@ __global__ void __launch_bounds__(C::kBlock) velo_track_kernel(const __grid_cons
       if (!seeding || (wb & kUsedBit)) continue;
       const int w = P.w_seed_phi16, phb = phi_of(wb);
       uint32_t ia = lower_bound_phi(bucketA, recA, nA, wrap16(phb - w));
+#pragma unroll 1
       for (uint32_t k = 0; k < nA; ++k, ++ia) {
         if (ia >= nA) ia -= nA;
         const uint32_t wa = recA[ia].w;
@@ -386,6 +404,7 @@ __global__ void __launch_bounds__(C::kBlock) velo_track_kernel(const __grid_cons
     // ---- T3/S2: one thread per doublet
     {
       const uint32_t nd = min(sm.n_doublets, (uint32_t)C::kCapDoublets);
+#pragma unroll 1
       for (uint32_t d = tid; d < nd; d += C::kThreads) {
         const uint32_t v = sm.doublets[d];
         process_doublet(c, recA, recB, recC, bucketC, nC, v & 0xFFFFu, v >> 16);
@@ -458,6 +477,7 @@ __global__ void __launch_bounds__(C::kBlock) velo_track_kernel(const __grid_cons
       n_tracks = min(run, (uint32_t)C::kCapTracks);
     }
     // claims back to "none" for the next iteration (its T1 starts after B1)
+#pragma unroll 1
     for (uint32_t k = tid; k < (uint32_t)C::kCap; k += C::kThreads) {
       sm.best[k] = kNoClaim; sm.claimA[k] = kNoClaim; sm.claimC[k] = kNoClaim;
     }
@@ -481,6 +501,7 @@ __global__ void __launch_bounds__(C::kBlock) velo_track_kernel(const __grid_cons
   const float* X = a.clusters.x + co;
   const float* Y = a.clusters.y + co;
   const float* Z = a.clusters.z + co;
+#pragma unroll 1
   for (uint32_t base = 0; base < n_tracks; base += C::kThreads) {
     const uint32_t t = base + tid;
     uint32_t n = 0, st = 0;
@@ -512,6 +533,7 @@ __global__ void __launch_bounds__(C::kBlock) velo_track_kernel(const __grid_cons
       // hits in order of addition: walk the links from the newest hit backwards
       double sz = 0, sx = 0, sy = 0;
       uint32_t h = st >> 16;
+#pragma unroll 1
       for (int k = (int)n - 1; k >= 0; --k) {
         a.hits_slab[co + oh + k] = (uint16_t)h;
         sz += (double)__ldcg(Z + h); sx += (double)__ldcg(X + h); sy += (double)__ldcg(Y + h);
@@ -521,6 +543,7 @@ __global__ void __launch_bounds__(C::kBlock) velo_track_kernel(const __grid_cons
       const double zm = sz * inv, xm = sx * inv, ym = sy * inv;
       double szz = 0, szx = 0, szy = 0;
       h = st >> 16;
+#pragma unroll 1
       for (int k = (int)n - 1; k >= 0; --k) {
         const double dz = (double)__ldcg(Z + h) - zm;
         szz += dz * dz;
@@ -556,11 +579,13 @@ __global__ void __launch_bounds__(128) compact_tracks_kernel(const CompactTracks
   }
   const uint32_t co = a.clusters.event_offsets[e];
   const uint32_t trk0 = co / 3;
+#pragma unroll 1
   for (uint32_t t = threadIdx.x; t < nT; t += blockDim.x) {
     const float4 f = a.trk_fit[trk0 + t];
     a.out.x0[T0 + t] = f.x; a.out.y0[T0 + t] = f.y; a.out.tx[T0 + t] = f.z; a.out.ty[T0 + t] = f.w;
     a.out.hit_offsets[T0 + t] = H0 + a.trk_hitoff[trk0 + t];
   }
+#pragma unroll 1
   for (uint32_t k = threadIdx.x; k < nH; k += blockDim.x) a.out.hits[H0 + k] = a.hits_slab[co + k];
   if (threadIdx.x == 0 && e + 1 == a.n_events) a.out.hit_offsets[T0 + nT] = H0 + nH;
 }
