@@ -12,7 +12,7 @@ from dataclasses import dataclass
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "_allen_velo.so")
+LIB_PATH = os.environ.get("ALLEN_VELO_LIB") or os.path.join(_HERE, "_allen_velo.so")  # override: an alternative build
 
 OK, ERR_INVALID, ERR_CUDA, ERR_WORKSPACE = 0, -1, -2, -3
 STATUS_BAD_HEADER, STATUS_BAD_SP, STATUS_TOO_MANY_CLUSTERS = 1, 2, 4

@@ -120,21 +120,41 @@ __device__ __forceinline__ bool ccl_pass(const Pass& p, const ClusterStore& cs, 
                                          uint32_t* n_edges_ctr) {
   const uint32_t lane = lane_id();
   const uint32_t bits = p.hash_bits;
-  // ---- stage the SP words of the group (R1: addresses outside the sensor are ignored and flagged)
-  uint32_t n = 0;
+  // ---- stage the SP words of the group (R1: addresses outside the sensor are ignored and flagged).  The group is
+  //      one flat index range; four loads per lane are in flight before the first is used.
+  const uint32_t in_group = (lane >= k0 && lane < k1) ? my_cnt : 0u;
+  uint32_t incl = in_group;
+#pragma unroll
+  for (int d = 1; d < 8; d <<= 1) {  // at most kMaxSensorsPerLayer = 8 lanes carry counts
+    const uint32_t t = __shfl_up_sync(kFull, incl, d);
+    if (lane >= (uint32_t)d) incl += t;
+  }
+  const uint32_t my_start = incl - in_group;                 // first staged index of sensor `lane`
+  const uint32_t n = __shfl_sync(kFull, incl, (k1 - 1) & 31);  // staged words of the group
 #pragma unroll 1
-  for (uint32_t k = k0; k < k1; ++k) {
-    const uint32_t off = __shfl_sync(kFull, my_off, k), cnt = __shfl_sync(kFull, my_cnt, k);
+  for (uint32_t i0 = 0; i0 < n; i0 += 128) {
+    uint32_t w[4], ks[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const uint32_t i = i0 + 32 * u + lane;
+      uint32_t k = k0;
 #pragma unroll 1
-    for (uint32_t i = lane; i < cnt; i += 32) {
-      const uint32_t w = __ldg(spw + off + i);
-      const uint32_t R = (w >> 8) & 0x3Fu, C = (w >> 14) & 0x1FFu;
-      uint32_t staged = (w & 0x7FFFFFu) | (k << 23);
-      if (C >= g.sp_cols || R >= g.sp_rows) { bad_sp = true; staged = 0; }
-      if ((w & 0xFFu) == 0) staged = 0;
-      p.sp[n + i] = staged;
+      for (uint32_t kk = k0 + 1; kk < k1; ++kk) k += i >= __shfl_sync(kFull, my_start, kk);
+      const uint32_t src = __shfl_sync(kFull, my_off, k) + (i - __shfl_sync(kFull, my_start, k));
+      ks[u] = k;
+      w[u] = i < n ? __ldg(spw + src) : 0u;
     }
-    n += cnt;
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const uint32_t i = i0 + 32 * u + lane;
+      const uint32_t R = (w[u] >> 8) & 0x3Fu, C = (w[u] >> 14) & 0x1FFu;
+      uint32_t staged = (w[u] & 0x7FFFFFu) | (ks[u] << 23);
+      if ((w[u] & 0xFFu) == 0) staged = 0;
+      if (i < n) {
+        if (C >= g.sp_cols || R >= g.sp_rows) { bad_sp = true; staged = 0; }
+        p.sp[i] = staged;
+      }
+    }
   }
 #pragma unroll 1
   for (uint32_t s = lane; s < (1u << bits); s += 32) p.tab[s] = 0;

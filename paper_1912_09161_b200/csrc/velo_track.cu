@@ -48,7 +48,16 @@ struct Cfg {
   static constexpr int kRoundsB = (kCap + kThreads - 1) / kThreads;
   static constexpr int kRoundsT = (kCapTracks + kThreads - 1) / kThreads;
 };
-using CfgS = Cfg<128, 256, 512, 512, 0, false, true>;
+#ifndef VELO_TRK_S_THREADS
+#define VELO_TRK_S_THREADS 128
+#endif
+#ifndef VELO_TRK_S_TRACKS
+#define VELO_TRK_S_TRACKS 384
+#endif
+#ifndef VELO_TRK_S_DOUBLETS
+#define VELO_TRK_S_DOUBLETS 256
+#endif
+using CfgS = Cfg<VELO_TRK_S_THREADS, 256, VELO_TRK_S_TRACKS, VELO_TRK_S_DOUBLETS, 0, false, true>;
 using CfgM = Cfg<256, 512, 1024, 1024, 1, false, false>;
 using CfgL = Cfg<512, 1024, 2048, 2048, 2, true, false>;
 
@@ -285,15 +294,12 @@ __global__ void __launch_bounds__(C::kBlock) velo_track_kernel(const __grid_cons
     // ---- T1 forward: best hit of layer C per active track (nothing of C is used yet); claim with (bits(S), key)
     const uint32_t first = min(sm.min_active[i & 1], first_new);
     if (tid == 0) { sm.min_active[(i - 1) & 1] = 0xFFFFFFFFu; sm.n_doublets = 0; }
-    unsigned long long fkey[C::kRoundsT];
-    uint32_t fc[C::kRoundsT];
-#pragma unroll
-    for (int r = 0; r < C::kRoundsT; ++r) {
-      fkey[r] = kNoClaim;
-      fc[r] = 0;
-      if (first + r * C::kThreads >= n_tracks) continue;  // uniform
-      const uint32_t t = first + r * C::kThreads + tid;
-      if (t >= n_tracks) continue;
+#pragma unroll 1
+    for (uint32_t k = tid; k < max(nA, nC); k += C::kThreads) { sm.claimA[k] = kNoClaim; sm.claimC[k] = kNoClaim; }
+    uint16_t* fsel = reinterpret_cast<uint16_t*>(sm.doublets);  // hit of layer C chosen by every track (T1 -> T2)
+#pragma unroll 1
+    for (uint32_t t = first + tid; t < n_tracks; t += C::kThreads) {
+      fsel[t] = 0xFFFFu;
       const uint32_t st = sm.tstate[t];
       if ((st & 0xFFu) == 0xFFu || nC == 0) continue;
       const uint32_t q = st >> 16;
@@ -328,23 +334,22 @@ __global__ void __launch_bounds__(C::kBlock) velo_track_kernel(const __grid_cons
         best = key < best ? key : best;
       }
       if (best != kNoClaim) {
-        fc[r] = (uint32_t)best;
-        fkey[r] = (best & 0xFFFFFFFF00000000ull) | sm.tseedB[t];
-        atomicMin(&sm.best[fc[r]], fkey[r]);
+        const uint32_t ic_best = (uint32_t)best;
+        fsel[t] = (uint16_t)ic_best;
+        atomicMin(&sm.best[ic_best], (best & 0xFFFFFFFF00000000ull) | sm.tseedB[t]);
       }
     }
     tsync<C>();  // B2
-    // ---- T2 resolve: the minimal claim wins the hit; everyone else counts a miss
-#pragma unroll
-    for (int r = 0; r < C::kRoundsT; ++r) {
-      if (first + r * C::kThreads >= n_tracks) continue;  // uniform
-      const uint32_t t = first + r * C::kThreads + tid;
-      if (t >= n_tracks) continue;
+    // ---- T2 resolve: the minimal claim wins the hit (track keys are unique, so the low half of the claim names the
+    //      winner); everyone else counts a miss
+#pragma unroll 1
+    for (uint32_t t = first + tid; t < n_tracks; t += C::kThreads) {
       const uint32_t st = sm.tstate[t];
       if ((st & 0xFFu) == 0xFFu) continue;
-      const bool won = fkey[r] != kNoClaim && sm.best[fc[r]] == fkey[r];
+      const uint32_t fc = fsel[t];
+      const bool won = fc != 0xFFFFu && (uint16_t)sm.best[fc] == sm.tseedB[t];
       if (won) {
-        const uint32_t q = st >> 16, cg = C0 + fc[r];
+        const uint32_t q = st >> 16, cg = C0 + fc;
         float xq, yq, zq;
         if (q < A1) {
           const Hit hq = q >= A0 ? recA[q - A0] : recB[q - B0];
@@ -356,11 +361,11 @@ __global__ void __launch_bounds__(C::kBlock) velo_track_kernel(const __grid_cons
           const uint32_t s = sm.src[l] + (q - sm.lo[l]);
           xq = __ldg(c.X + s); yq = __ldg(c.Y + s); zq = __ldg(c.Z + s);
         }
-        const Hit hc = recC[fc[r]];
+        const Hit hc = recC[fc];
         const float dz = __fsub_rn(hc.z, zq);
         sm.ttx[t] = __fdiv_rn(__fsub_rn(hc.x, xq), dz);
         sm.tty[t] = __fdiv_rn(__fsub_rn(hc.y, yq), dz);
-        recC[fc[r]].w = hc.w | kUsedBit;
+        recC[fc].w = hc.w | kUsedBit;
         link[cg] = (uint16_t)q;
         const uint32_t nh = ((st >> 8) & 0x7Fu) + 1u;
         sm.tstate[t] = (cg << 16) | (st & 0x8000u) | (nh << 8);
@@ -379,10 +384,10 @@ __global__ void __launch_bounds__(C::kBlock) velo_track_kernel(const __grid_cons
 
     // ---- T3/S1: every unused b lists the unused hits of layer A inside its phi window as (b, a) doublets
     const bool seeding = nA != 0 && nB != 0 && nC != 0;
-#pragma unroll
-    for (int r = 0; r < C::kRoundsB; ++r) {
-      const uint32_t kb = r * C::kThreads + tid;
-      if (kb >= nB) continue;
+#pragma unroll 1
+    for (uint32_t k = nB + tid; k < nC; k += C::kThreads) sm.best[k] = kNoClaim;  // forward claims beyond layer B's size
+#pragma unroll 1
+    for (uint32_t kb = tid; kb < nB; kb += C::kThreads) {
       sm.best[kb] = kNoClaim;  // forward claims are done with; from here on: per-b argmin
       const uint32_t wb = recB[kb].w;
       if (!seeding || (wb & kUsedBit)) continue;
@@ -413,38 +418,41 @@ __global__ void __launch_bounds__(C::kBlock) velo_track_kernel(const __grid_cons
     tsync<C>();  // B5
 
     // ---- T4a: every b with a triplet claims its a and its c with (bits(S), b)
-    unsigned long long tkey[C::kRoundsB];
-    uint32_t tac[C::kRoundsB];  // a_local << 16 | c_local
-#pragma unroll
-    for (int r = 0; r < C::kRoundsB; ++r) {
-      tkey[r] = kNoClaim;
-      tac[r] = 0;
-      const uint32_t kb = r * C::kThreads + tid;
-      if (kb >= nB || !seeding) continue;
+    const uint32_t roundsB = seeding ? (nB + C::kThreads - 1) / C::kThreads : 0;  // block-uniform
+#pragma unroll 1
+    for (uint32_t kb = tid; kb < nB && seeding; kb += C::kThreads) {
       const unsigned long long k = sm.best[kb];
       if (k == kNoClaim) continue;
-      tac[r] = (uint32_t)k;
-      tkey[r] = (k & 0xFFFFFFFF00000000ull) | (B0 + kb);
-      atomicMin(&sm.claimA[tac[r] >> 16], tkey[r]);
-      atomicMin(&sm.claimC[tac[r] & 0xFFFFu], tkey[r]);
+      const uint32_t ac = (uint32_t)k;  // a_local << 16 | c_local
+      const unsigned long long tkey = (k & 0xFFFFFFFF00000000ull) | (B0 + kb);
+      atomicMin(&sm.claimA[ac >> 16], tkey);
+      atomicMin(&sm.claimC[ac & 0xFFFFu], tkey);
     }
     tsync<C>();  // B6
     // ---- T4b: accepted iff the triplet holds the minimal key on both its a and its c; new tracks take slots in
-    //      ascending b (ballot + per-warp totals)
-    uint32_t acc_ballot[C::kRoundsB];
-#pragma unroll
-    for (int r = 0; r < C::kRoundsB; ++r) {
-      const bool accepted = tkey[r] != kNoClaim && sm.claimA[tac[r] >> 16] == tkey[r] &&
-                            sm.claimC[tac[r] & 0xFFFFu] == tkey[r];
-      acc_ballot[r] = __ballot_sync(kFull, accepted);
-      if (lane == 0) sm.warp_tot[r][warp] = __popc(acc_ballot[r]);
+    //      ascending b (ballot + per-warp totals).  best[] and the claims stay untouched until the end of T4b, so
+    //      both halves re-derive "accepted" instead of carrying it in registers.
+    auto accepted_of = [&](uint32_t kb, uint32_t& ac, unsigned long long& tkey) -> bool {
+      if (kb >= nB) return false;
+      const unsigned long long k = sm.best[kb];
+      if (k == kNoClaim) return false;
+      ac = (uint32_t)k;
+      tkey = (k & 0xFFFFFFFF00000000ull) | (B0 + kb);
+      return sm.claimA[ac >> 16] == tkey && sm.claimC[ac & 0xFFFFu] == tkey;
+    };
+#pragma unroll 1
+    for (uint32_t r = 0; r < roundsB; ++r) {
+      uint32_t ac = 0;
+      unsigned long long tkey = 0;
+      const uint32_t ballot = __ballot_sync(kFull, accepted_of(r * C::kThreads + tid, ac, tkey));
+      if (lane == 0) sm.warp_tot[r][warp] = __popc(ballot);
     }
     tsync<C>();  // B7
     first_new = n_tracks;
     {
       uint32_t run = n_tracks;
-#pragma unroll
-      for (int r = 0; r < C::kRoundsB; ++r) {
+#pragma unroll 1
+      for (uint32_t r = 0; r < roundsB; ++r) {
         uint32_t before = 0, total = 0;
 #pragma unroll
         for (int w = 0; w < C::kWarps; ++w) {
@@ -452,34 +460,37 @@ __global__ void __launch_bounds__(C::kBlock) velo_track_kernel(const __grid_cons
           if (w < (int)warp) before += v;
           total += v;
         }
-        if (acc_ballot[r] >> lane & 1u) {
-          const uint32_t slot = run + before + __popc(acc_ballot[r] & lanemask_lt());
-          if (slot < (uint32_t)C::kCapTracks) {
-            const uint32_t kb = r * C::kThreads + tid, ia = tac[r] >> 16, ic = tac[r] & 0xFFFFu;
-            const Hit hb = recB[kb], hc = recC[ic];
-            const float dz = __fsub_rn(hc.z, hb.z);
-            sm.ttx[slot] = __fdiv_rn(__fsub_rn(hc.x, hb.x), dz);
-            sm.tty[slot] = __fdiv_rn(__fsub_rn(hc.y, hb.y), dz);
-            const float S = __uint_as_float((uint32_t)(tkey[r] >> 32));
-            sm.tstate[slot] = ((C0 + ic) << 16) | (S <= P.s_weak ? 0x8000u : 0u) | (3u << 8);
-            sm.tseedB[slot] = (uint16_t)(B0 + kb);
-            link[B0 + kb] = (uint16_t)(A0 + ia);
-            link[C0 + ic] = (uint16_t)(B0 + kb);
-            recA[ia].w |= kUsedBit;
-            recB[kb].w = hb.w | kUsedBit;
-            recC[ic].w = hc.w | kUsedBit;
-          } else {
-            sm.flags = 1;  // out of track slots: a larger instance redoes the event
+        const uint32_t kb = r * C::kThreads + tid;
+        if (total) {  // block-uniform
+          uint32_t ac = 0;
+          unsigned long long tkey = 0;
+          const bool acc = accepted_of(kb, ac, tkey);
+          const uint32_t ballot = __ballot_sync(kFull, acc);
+          if (acc) {
+            const uint32_t slot = run + before + __popc(ballot & lanemask_lt());
+            if (slot < (uint32_t)C::kCapTracks) {
+              const uint32_t ia = ac >> 16, ic = ac & 0xFFFFu;
+              const Hit hb = recB[kb], hc = recC[ic];
+              const float dz = __fsub_rn(hc.z, hb.z);
+              sm.ttx[slot] = __fdiv_rn(__fsub_rn(hc.x, hb.x), dz);
+              sm.tty[slot] = __fdiv_rn(__fsub_rn(hc.y, hb.y), dz);
+              const float S = __uint_as_float((uint32_t)(tkey >> 32));
+              sm.tstate[slot] = ((C0 + ic) << 16) | (S <= P.s_weak ? 0x8000u : 0u) | (3u << 8);
+              sm.tseedB[slot] = (uint16_t)(B0 + kb);
+              link[B0 + kb] = (uint16_t)(A0 + ia);
+              link[C0 + ic] = (uint16_t)(B0 + kb);
+              // layer A leaves the ring after this iteration: its used flags are never read again
+              recB[kb].w = hb.w | kUsedBit;
+              recC[ic].w = hc.w | kUsedBit;
+            } else {
+              sm.flags = 1;  // out of track slots: a larger instance redoes the event
+            }
           }
         }
+        if (kb < nB) sm.best[kb] = kNoClaim;  // only this thread reads best[kb] in T4b; the next T1 needs "none"
         run += total;
       }
       n_tracks = min(run, (uint32_t)C::kCapTracks);
-    }
-    // claims back to "none" for the next iteration (its T1 starts after B1)
-#pragma unroll 1
-    for (uint32_t k = tid; k < (uint32_t)C::kCap; k += C::kThreads) {
-      sm.best[k] = kNoClaim; sm.claimA[k] = kNoClaim; sm.claimC[k] = kNoClaim;
     }
   }
   __pipeline_wait_prior(0);
