@@ -18,6 +18,9 @@ struct allen_velo {
   size_t ws_bytes = 0;
   uint32_t last_launches = 0;
   uint32_t n_mid_sms = 0;      // SM ids the mid-slot pool of the cluster kernel covers
+  uint32_t n_sms = 0;
+  cudaStream_t side[2] = {nullptr, nullptr};  // the larger track-kernel instances run beside the first one
+  cudaEvent_t fork_join[3] = {nullptr, nullptr, nullptr};
   std::string last_error;
   // optional per-kernel timing: a ring of (kKernels + 1) events per call
   std::vector<cudaEvent_t> events;
@@ -27,7 +30,7 @@ struct allen_velo {
 
 namespace {
 
-constexpr uint32_t kKernels = 5;  // timed segments; velo_track is three launches (one per staging capacity)
+constexpr uint32_t kKernels = 5;  // timed segments; velo_track is six launches (classification, three staging capacities, second pass)
 const char* const kKernelNames[kKernels] = {"velo_cluster", "scan_clusters", "velo_track", "scan_tracks",
                                             "compact_tracks"};
 constexpr size_t kAlign = 256;
@@ -63,7 +66,8 @@ size_t fixed_bytes(uint32_t n_events, uint32_t n_layers, uint32_t n_mid_sms) {
   b += align_up((size_t)big_slots(items) * cluster_big_slot_bytes());
   b += align_up((size_t)n_events * 8) + align_up(((size_t)n_events + 1) * 8);  // track counts, offsets
   b += align_up(scan_state_words(n_events) * 8);                  // scan state (tracks)
-  b += align_up(n_events);                                        // track kernel instance per event
+  b += align_up(n_events);                                        // class of every event
+  b += align_up((size_t)n_events * 4) * 4 + align_up(8 * 4);      // event lists of the larger instances, counters
   return b + 16 * kAlign;
 }
 
@@ -143,7 +147,12 @@ int allen_velo_create(const allen_velo_geometry_t* geo, allen_velo_t** out) {
   if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n_sm <= 0) {
     cudaFree(h->dev_block); delete h; return ALLEN_VELO_ERR_CUDA;
   }
+  h->n_sms = (uint32_t)n_sm;
   h->n_mid_sms = (uint32_t)n_sm + 16;  // %smid is below the SM count on the parts seen; margin for gaps in the numbering
+  for (int i = 0; i < 2; ++i)
+    if (cudaStreamCreateWithFlags(&h->side[i], cudaStreamNonBlocking) != cudaSuccess) { allen_velo_destroy(h); return ALLEN_VELO_ERR_CUDA; }
+  for (int i = 0; i < 3; ++i)
+    if (cudaEventCreateWithFlags(&h->fork_join[i], cudaEventDisableTiming) != cudaSuccess) { allen_velo_destroy(h); return ALLEN_VELO_ERR_CUDA; }
   DeviceGeometry& g = h->dev;
   g.n_sensors = S; g.n_layers = L; g.n_cols = geo->n_cols; g.n_rows = geo->n_rows;
   g.sp_cols = geo->n_cols / 2; g.sp_rows = geo->n_rows / 4;
@@ -216,6 +225,9 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   unsigned long long* trk_offsets = cv.take<unsigned long long>((size_t)n_events + 1);
   unsigned long long* trk_scan_state = cv.take<unsigned long long>(scan_state_words(n_events));
   uint8_t* trk_level = cv.take<uint8_t>(n_events);
+  uint32_t* trk_lists[4];
+  for (uint32_t*& p : trk_lists) p = cv.take<uint32_t>(n_events);
+  uint32_t* trk_counters = cv.take<uint32_t>(8);
   size_t entries = (h->ws_bytes - cv.used - 16 * kAlign) / per_entry_bytes();
   if (entries > 0x7FFFFFF0u) entries = 0x7FFFFFF0u;
   ClusterSlab slab{};
@@ -283,8 +295,11 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   tl.trk_fit = trk_fit;
   tl.counts = trk_counts;
   tl.level = trk_level;
+  tl.ev_list[0] = trk_lists[0]; tl.ev_list[1] = trk_lists[1];
+  tl.redo_list[0] = trk_lists[2]; tl.redo_list[1] = trk_lists[3];
+  tl.counters = trk_counters;
   uint32_t n_track_launches = 0;
-  if ((err = launch_track(tl, stream, &n_track_launches)) != cudaSuccess) return fail(h, ALLEN_VELO_ERR_CUDA, "track kernel", err);
+  if ((err = launch_track(tl, stream, h->side, h->fork_join, h->n_sms, &n_track_launches)) != cudaSuccess) return fail(h, ALLEN_VELO_ERR_CUDA, "track kernel", err);
   h->last_launches += n_track_launches;
   mark(3);
 
@@ -342,6 +357,8 @@ const char* allen_velo_last_error(const allen_velo_t* h) { return h ? h->last_er
 void allen_velo_destroy(allen_velo_t* h) {
   if (!h) return;
   for (cudaEvent_t e : h->events) cudaEventDestroy(e);
+  for (cudaStream_t st : h->side) if (st) cudaStreamDestroy(st);
+  for (cudaEvent_t e : h->fork_join) if (e) cudaEventDestroy(e);
   if (h->dev_block) cudaFree(h->dev_block);
   delete h;
 }

@@ -144,9 +144,13 @@ struct TrackLaunch {
   uint32_t* trk_hitoff;            // [capacity/3+1] event-local first entry in hits_slab of every output track
   float4* trk_fit;                 // [capacity/3+1] x0, y0, tx, ty
   unsigned long long* counts;      // [n_events] (n_tracks << 32) | n_track_hits
-  uint8_t* level;                  // [n_events] kernel instance an event was handed to (0 = by its size alone)
+  uint8_t* level;                  // [n_events] class of the event: searching instance 0..2, 254 copy only, 255 nothing
+  uint32_t* ev_list[2];            // [n_events] each: events of level 1 / 2
+  uint32_t* redo_list[2];          // [n_events] each: events level 0 / 1 ran out of track slots on (second pass)
+  uint32_t* counters;              // [8] list sizes and cursors, zeroed by the launcher
 };
-cudaError_t launch_track(const TrackLaunch& a, cudaStream_t stream, uint32_t* n_launches);
+cudaError_t launch_track(const TrackLaunch& a, cudaStream_t stream, cudaStream_t* side, cudaEvent_t* ev,
+                         uint32_t n_sms, uint32_t* n_launches);
 
 struct CompactTracksLaunch {
   uint32_t n_events;

@@ -58,8 +58,15 @@ struct Cfg {
 #define VELO_TRK_S_DOUBLETS 256
 #endif
 using CfgS = Cfg<VELO_TRK_S_THREADS, 256, VELO_TRK_S_TRACKS, VELO_TRK_S_DOUBLETS, 0, false, true>;
-using CfgM = Cfg<256, 512, 1024, 1024, 1, false, false>;
-using CfgL = Cfg<512, 1024, 2048, 2048, 2, true, false>;
+using CfgM = Cfg<256, 512, 1024, 1024, 1, false, true>;
+using CfgL = Cfg<512, 1024, 2048, 2048, 2, true, true>;
+// second pass for events a smaller instance ran out of track slots on: their clusters are already in the output
+using CfgMr = Cfg<256, 512, 1024, 1024, 1, false, false>;
+using CfgLr = Cfg<512, 1024, 2048, 2048, 2, true, false>;
+
+// class of an event (TrackLaunch::level), set by classify_events_kernel
+constexpr uint8_t kClsSkip = 255;  // nothing to do (no clusters, or the output cannot hold them)
+constexpr uint8_t kClsCopy = 254;  // clusters are moved to the output, no tracking (incomplete or > 65535 clusters)
 
 template <class C>
 struct Smem {
@@ -77,6 +84,7 @@ struct Smem {
   uint32_t n_doublets;
   uint32_t min_active[2];
   uint32_t flags;
+  uint32_t next_event;
 };
 
 __device__ __forceinline__ int phi_of(uint32_t w) { return (int)(int16_t)(uint16_t)(w & 0xFFFFu); }
@@ -188,68 +196,28 @@ __device__ __forceinline__ void copy_clusters(const TrackLaunch& a, uint32_t src
   }
 }
 
+// Offsets of the event's layers: lo[] relative to the event's first cluster, src[] absolute in the arrays the hits
+// are read from (the slab for instances with a copier warp, else the output a previous kernel has filled).
 template <class C>
-__global__ void __launch_bounds__(C::kBlock) velo_track_kernel(const __grid_constant__ TrackLaunch a) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  Smem<C>& sm = *reinterpret_cast<Smem<C>*>(smem_raw);
-  const DeviceGeometry& g = a.geo;
-  const uint32_t e = blockIdx.x, L = g.n_layers, tid = threadIdx.x;
-  const uint32_t lane = lane_id(), warp = tid >> 5;
-
-  const uint32_t co = a.clusters.event_offsets[e];
-  const uint32_t n_cl = a.clusters.event_offsets[e + 1] - co;
-  const uint32_t st0 = a.clusters.status[e];
-  if (n_cl == 0) {
-    if (C::kLevel == 0 && tid == 0) a.counts[e] = 0;
-    return;
-  }
-  if ((unsigned long long)co + n_cl > a.clusters.capacity) {  // the output (or the per-cluster scratch) cannot hold it
-    if (C::kLevel == 0 && tid == 0) {
-      atomicOr(a.clusters.status + e, ALLEN_VELO_STATUS_CLUSTER_CAPACITY);
-      a.counts[e] = 0;
-    }
-    return;
-  }
-  // events whose clusters are incomplete, or too many for 16-bit hit indices, take no part in tracking
-  const bool skip = (st0 & (ALLEN_VELO_STATUS_BAD_HEADER | ALLEN_VELO_STATUS_STAGE_OVERFLOW)) != 0 || n_cl > 65535u;
-  // ---- which instance takes this event: the smallest whose staging capacity holds its busiest layer, unless a
-  //      smaller instance ran out of track slots and passed it on (level[e])
-  if (tid == 0) sm.flags = 0;
+__device__ __forceinline__ void load_offsets(const TrackLaunch& a, uint32_t e, Smem<C>& sm, uint32_t co) {
+  const uint32_t L = a.geo.n_layers;
 #pragma unroll 1
-  for (uint32_t l = tid; l <= L; l += C::kBlock) sm.lo[l] = a.clusters.layer_offsets[e * L + l] - co;
-  // the instance with the copier reads the slab the cluster kernel wrote; the others the output it has filled
+  for (uint32_t l = threadIdx.x; l <= L; l += C::kBlock) sm.lo[l] = a.clusters.layer_offsets[e * L + l] - co;
 #pragma unroll 1
-  for (uint32_t l = tid; l < L; l += C::kBlock)
+  for (uint32_t l = threadIdx.x; l < L; l += C::kBlock)
     sm.src[l] = C::kCopier ? a.slab_base[e * L + l] : a.clusters.layer_offsets[e * L + l];
+}
+
+// Search by triplet, fit and (with a copier warp) cluster compaction for event e; the whole CTA calls it.
+template <class C>
+__device__ __forceinline__ void track_event(const TrackLaunch& a, uint32_t e, Smem<C>& sm) {
+  const DeviceGeometry& g = a.geo;
+  const uint32_t L = g.n_layers, tid = threadIdx.x;
+  const uint32_t lane = lane_id(), warp = tid >> 5;
+  const uint32_t co = a.clusters.event_offsets[e];
+  load_offsets<C>(a, e, sm, co);
+  if (tid == 0) { sm.flags = 0; sm.min_active[0] = 0; sm.min_active[1] = 0; }
   __syncthreads();
-  {
-    uint32_t mx = 0;
-#pragma unroll 1
-    for (uint32_t l = tid; l < L; l += C::kBlock) mx = max(mx, sm.lo[l + 1] - sm.lo[l]);
-    if (mx) atomicMax(&sm.flags, mx);
-  }
-  __syncthreads();
-  const uint32_t max_layer = sm.flags;
-  const uint32_t natural = max_layer <= (uint32_t)CfgS::kCap ? 0u : max_layer <= (uint32_t)CfgM::kCap ? 1u : 2u;
-  const uint32_t level = max(natural, (uint32_t)a.level[e]);  // level[e]: 0 unless raised by a smaller instance
-  const bool fits = max_layer <= (uint32_t)C::kCap;
-  const bool take = !skip && level == (uint32_t)C::kLevel && fits;
-  __syncthreads();  // everyone has read sm.flags
-  if (!take) {
-    if (C::kCopier)  // the output is still to be filled: the whole CTA moves the event
-#pragma unroll 1
-      for (uint32_t l = 0; l < L; ++l)
-        copy_clusters(a, sm.src[l], co + sm.lo[l], sm.lo[l + 1] - sm.lo[l], tid, C::kBlock);
-    if (tid == 0) {
-      if (C::kLevel == 0 && n_cl > 65535u) atomicOr(a.clusters.status + e, ALLEN_VELO_STATUS_TOO_MANY_CLUSTERS);
-      if (C::kLevel == 0 && skip) a.counts[e] = 0;
-      if (C::kLast && !skip && !fits) {  // busiest layer beyond the largest staging capacity
-        atomicOr(a.clusters.status + e, ALLEN_VELO_STATUS_STAGE_OVERFLOW);
-        a.counts[e] = 0;
-      }
-    }
-    return;
-  }
   if (C::kCopier && tid >= (uint32_t)C::kThreads) {
     // copier warp: layers in the order the search stages them (their slab lines are then in L2 for both readers)
 #pragma unroll 1
@@ -258,7 +226,6 @@ __global__ void __launch_bounds__(C::kBlock) velo_track_kernel(const __grid_cons
     __syncthreads();  // pairs with the barrier before the fit: the output arrays are complete
     return;
   }
-  if (tid == 0) { sm.flags = 0; sm.min_active[0] = 0; sm.min_active[1] = 0; }
 
   Ctx<C> c{sm,
            C::kCopier ? a.slab.x : a.clusters.x, C::kCopier ? a.slab.y : a.clusters.y,
@@ -496,10 +463,10 @@ __global__ void __launch_bounds__(C::kBlock) velo_track_kernel(const __grid_cons
   __pipeline_wait_prior(0);
   __syncthreads();
 
-  if (sm.flags) {
+  if (sm.flags) {  // out of track slots: the next larger instance redoes the event in the second pass
     if (tid == 0) {
       if (C::kLast) { atomicOr(a.clusters.status + e, ALLEN_VELO_STATUS_STAGE_OVERFLOW); a.counts[e] = 0; }
-      else a.level[e] = (uint8_t)(C::kLevel + 1);
+      else a.redo_list[C::kLevel][atomicAdd(a.counters + 2 + C::kLevel, 1u)] = e;
     }
     return;
   }
@@ -601,30 +568,136 @@ __global__ void __launch_bounds__(128) compact_tracks_kernel(const CompactTracks
   if (threadIdx.x == 0 && e + 1 == a.n_events) a.out.hit_offsets[T0 + nT] = H0 + nH;
 }
 
+// One thread per event: class of the event (which instance searches it, or copy only / nothing) and the event lists
+// of the two larger instances.  counters: [0], [1] events of level 1, 2; [2], [3] second-pass events; [4..7] cursors.
+__global__ void __launch_bounds__(256) classify_events_kernel(const __grid_constant__ TrackLaunch a) {
+  const uint32_t e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= a.n_events) return;
+  const uint32_t L = a.geo.n_layers;
+  const uint32_t co = a.clusters.event_offsets[e];
+  const uint32_t n_cl = a.clusters.event_offsets[e + 1] - co;
+  const uint32_t st0 = a.clusters.status[e];
+  uint8_t cls;
+  if (n_cl == 0) {
+    cls = kClsSkip;
+  } else if ((unsigned long long)co + n_cl > a.clusters.capacity) {  // the output (or the per-cluster scratch) is full
+    atomicOr(a.clusters.status + e, ALLEN_VELO_STATUS_CLUSTER_CAPACITY);
+    cls = kClsSkip;
+  } else if ((st0 & (ALLEN_VELO_STATUS_BAD_HEADER | ALLEN_VELO_STATUS_STAGE_OVERFLOW)) != 0) {
+    cls = kClsCopy;  // incomplete clusters take no part in tracking
+  } else if (n_cl > 65535u) {
+    atomicOr(a.clusters.status + e, ALLEN_VELO_STATUS_TOO_MANY_CLUSTERS);  // hit indices are 16 bit
+    cls = kClsCopy;
+  } else {
+    uint32_t mx = 0, prev = co;
+#pragma unroll 1
+    for (uint32_t l = 1; l <= L; ++l) {
+      const uint32_t o = a.clusters.layer_offsets[e * L + l];
+      mx = max(mx, o - prev);
+      prev = o;
+    }
+    if (mx <= (uint32_t)CfgS::kCap) cls = 0;
+    else if (mx <= (uint32_t)CfgM::kCap) cls = 1;
+    else if (mx <= (uint32_t)CfgL::kCap) cls = 2;
+    else {  // busiest layer beyond the largest staging capacity
+      atomicOr(a.clusters.status + e, ALLEN_VELO_STATUS_STAGE_OVERFLOW);
+      cls = kClsCopy;
+    }
+    if (cls == 1 || cls == 2) a.ev_list[cls - 1][atomicAdd(a.counters + (cls - 1), 1u)] = e;
+  }
+  a.level[e] = cls;
+  if (cls >= kClsCopy) a.counts[e] = 0;
+}
+
+// First instance: one CTA per event of class 0; it also moves the clusters of copy-only events.
 template <class C>
-cudaError_t launch_instance(const TrackLaunch& a, cudaStream_t stream) {
-  cudaError_t err = cudaFuncSetAttribute(velo_track_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)sizeof(Smem<C>));
+__global__ void __launch_bounds__(C::kBlock) velo_track_kernel(const __grid_constant__ TrackLaunch a) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  Smem<C>& sm = *reinterpret_cast<Smem<C>*>(smem_raw);
+  const uint32_t e = blockIdx.x;
+  const uint8_t cls = a.level[e];
+  if (cls == kClsCopy) {
+    const uint32_t co = a.clusters.event_offsets[e], L = a.geo.n_layers;
+    load_offsets<C>(a, e, sm, co);
+    __syncthreads();
+#pragma unroll 1
+    for (uint32_t l = 0; l < L; ++l)
+      copy_clusters(a, sm.src[l], co + sm.lo[l], sm.lo[l + 1] - sm.lo[l], threadIdx.x, C::kBlock);
+    return;
+  }
+  if (cls != 0) return;
+  track_event<C>(a, e, sm);
+}
+
+// Larger instances: a few resident CTAs take events from a list (most batches have few or none of them).
+template <class C>
+__global__ void __launch_bounds__(C::kBlock) velo_track_list_kernel(const __grid_constant__ TrackLaunch a,
+                                                                    const uint32_t* __restrict__ list,
+                                                                    const uint32_t* __restrict__ count,
+                                                                    uint32_t* cursor) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  Smem<C>& sm = *reinterpret_cast<Smem<C>*>(smem_raw);
+  const uint32_t n = *count;
+#pragma unroll 1
+  for (;;) {
+    if (threadIdx.x == 0) sm.next_event = atomicAdd(cursor, 1u);
+    __syncthreads();
+    const uint32_t idx = sm.next_event;
+    if (idx >= n) return;
+    track_event<C>(a, list[idx], sm);
+    __syncthreads();
+  }
+}
+
+template <class C>
+cudaError_t launch_list(const TrackLaunch& a, uint32_t which, uint32_t grid, cudaStream_t stream) {
   static_assert(sizeof(Smem<C>) <= 227 * 1024, "shared memory of one CTA");
+  cudaError_t err = cudaFuncSetAttribute(velo_track_list_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)sizeof(Smem<C>));
   if (err != cudaSuccess) return err;
-  velo_track_kernel<C><<<a.n_events, C::kBlock, sizeof(Smem<C>), stream>>>(a);
+  const uint32_t* list = which < 2 ? a.ev_list[which] : a.redo_list[which - 2];
+  velo_track_list_kernel<C><<<grid, C::kBlock, sizeof(Smem<C>), stream>>>(a, list, a.counters + which,
+                                                                          a.counters + 4 + which);
   return cudaGetLastError();
 }
 
 }  // namespace
 
-// Three launches over all events: each CTA first decides whether its event belongs to this instance (see the header
-// comment); events of other instances cost one small read and an exit.
-cudaError_t launch_track(const TrackLaunch& a, cudaStream_t stream, uint32_t* n_launches) {
+// classify -> [first instance over all events | level-1 list | level-2 list, on three streams] -> second pass for
+// events that ran out of track slots (level 1, then level 2).  `side`/`ev`: two extra streams and three events owned
+// by the handle; everything is ordered after and before the work on `stream` by events, nothing synchronises.
+cudaError_t launch_track(const TrackLaunch& a, cudaStream_t stream, cudaStream_t* side, cudaEvent_t* ev,
+                         uint32_t n_sms, uint32_t* n_launches) {
   *n_launches = 0;
   if (a.n_events == 0) return cudaSuccess;
-  cudaError_t err = cudaMemsetAsync(a.level, 0, a.n_events, stream);
+  cudaError_t err = cudaMemsetAsync(a.counters, 0, 8 * sizeof(uint32_t), stream);
   if (err != cudaSuccess) return err;
-  if ((err = launch_instance<CfgS>(a, stream)) != cudaSuccess) return err;
+  classify_events_kernel<<<(a.n_events + 255) / 256, 256, 0, stream>>>(a);
+  if ((err = cudaGetLastError()) != cudaSuccess) return err;
   ++*n_launches;
-  if ((err = launch_instance<CfgM>(a, stream)) != cudaSuccess) return err;
+  if ((err = cudaEventRecord(ev[0], stream)) != cudaSuccess) return err;
+  if ((err = cudaStreamWaitEvent(side[0], ev[0], 0)) != cudaSuccess) return err;
+  if ((err = cudaStreamWaitEvent(side[1], ev[0], 0)) != cudaSuccess) return err;
+
+  static_assert(sizeof(Smem<CfgS>) <= 227 * 1024, "shared memory of one CTA");
+  err = cudaFuncSetAttribute(velo_track_kernel<CfgS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)sizeof(Smem<CfgS>));
+  if (err != cudaSuccess) return err;
+  velo_track_kernel<CfgS><<<a.n_events, CfgS::kBlock, sizeof(Smem<CfgS>), stream>>>(a);
+  if ((err = cudaGetLastError()) != cudaSuccess) return err;
   ++*n_launches;
-  if ((err = launch_instance<CfgL>(a, stream)) != cudaSuccess) return err;
+  const uint32_t grid_m = min(a.n_events, 3 * n_sms), grid_l = min(a.n_events, n_sms);
+  if ((err = launch_list<CfgM>(a, 0, grid_m, side[0])) != cudaSuccess) return err;
+  ++*n_launches;
+  if ((err = launch_list<CfgL>(a, 1, grid_l, side[1])) != cudaSuccess) return err;
+  ++*n_launches;
+  if ((err = cudaEventRecord(ev[1], side[0])) != cudaSuccess) return err;
+  if ((err = cudaEventRecord(ev[2], side[1])) != cudaSuccess) return err;
+  if ((err = cudaStreamWaitEvent(stream, ev[1], 0)) != cudaSuccess) return err;
+  if ((err = cudaStreamWaitEvent(stream, ev[2], 0)) != cudaSuccess) return err;
+  if ((err = launch_list<CfgMr>(a, 2, min(grid_m, 2 * n_sms), stream)) != cudaSuccess) return err;
+  ++*n_launches;
+  if ((err = launch_list<CfgLr>(a, 3, grid_l, stream)) != cudaSuccess) return err;
   ++*n_launches;
   return cudaSuccess;
 }
