@@ -161,3 +161,39 @@ def test_deterministic_across_runs(velo, oracle_of):
         for k in d0:
             if isinstance(d0[k], np.ndarray):
                 assert np.array_equal(d0[k], d1[k]), k
+
+
+@pytest.mark.parametrize("params", [
+    # very loose cuts: hundreds of (fake) tracks per event -> the first instance runs out of track slots and the
+    # second pass (larger instances, reading the already compacted clusters) redoes those events
+    dict(w_seed_phi16=3000, w_fwd_phi16=3000, s_seed=4.0, s_fwd=4.0, s_weak=4.0, max_slope=2.0),
+    # tracks may skip two layers: their last hit leaves the three-layer ring of the search
+    dict(max_skipped=2),
+    dict(max_skipped=4, w_fwd_phi16=1500, s_fwd=0.5),
+    # tight windows, no weak tracks
+    dict(w_seed_phi16=100, w_fwd_phi16=60, s_weak=0.0),
+])
+def test_parity_with_other_cuts(geometry, batch_of, params):
+    import oracle
+    from paper_1912_09161_b200 import binding
+    from tests.helpers import compare_clusters, compare_tracks
+
+    batch = batch_of(2, 96)
+    ref = oracle.reconstruct(geometry, batch.raw, batch.event_offsets, params=params, n_threads=8)
+    v = binding.AllenVelo(geometry, params=params)
+    try:
+        clusters, tracks = binding.reconstruct_batch(v, batch.raw, batch.event_offsets)
+    finally:
+        v.destroy()
+    c, t = as_oracle_types(clusters, tracks)
+    assert not compare_clusters(c, ref.clusters)
+    rep = compare_tracks(t, ref.tracks, ref.near_cut_per_event)
+    assert rep["n_got"] == rep["n_ref"] and rep["mismatched_tracks"] == 0 and rep["bad_fits"] == 0, rep
+    assert np.array_equal(t.hits, ref.tracks.hits)
+    assert not clusters["status"].any()
+
+
+def test_parity_on_a_larger_batch(velo, oracle_of):
+    """2000 nu=6 events: several waves of CTAs per SM, events of every size class in one batch."""
+    batch, ref = oracle_of(2, 2000)
+    check_parity(velo, batch, ref)
