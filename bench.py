@@ -42,6 +42,24 @@ def peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def ncu_counters(workload_key):
+    """Per-kernel counters of one launch from the newest profiles/*_counters.csv (written from an `ncu --set full`
+    capture of this very command; the file names the command).  {} if there is none for this workload."""
+    import csv
+    import glob
+
+    out = {}
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_counters.csv"))):
+        with open(path) as f:
+            for row in csv.DictReader(f):
+                if row["workload"] == workload_key:
+                    out[row["kernel"]] = dict(dram_bytes=int(row["dram_read_bytes"]) + int(row["dram_write_bytes"]),
+                                              warp_instructions=int(row["warp_instructions"]),
+                                              lanes=float(row["active_lanes_per_instruction"]))
+                    out["_source"] = os.path.relpath(path, ROOT)
+    return out
+
+
 class ClockSampler:
     """nvidia-smi clocks/throttle-reason sampler running beside the timed region (B200_PROFILING.md recipe)."""
 
@@ -109,9 +127,10 @@ def algorithmic_bytes(n_events, n_layers, raw_bytes, n_clusters, n_tracks, n_tra
     clusters = 30 * n_clusters + 4 * (n_events * n_layers + 1) + 4 * (n_events + 1) + 4 * n_events
     tracks = 4 * (n_events + 1) + 4 * (n_tracks + 1) + 2 * n_track_hits + 16 * n_tracks
     return dict(raw=raw, clusters=clusters, tracks=tracks, total=raw + clusters + tracks,
-                # per-kernel shares: the cluster kernel reads raw and produces the clusters; the track kernel reads
-                # x, y, z, phi16 of every hit once (14 B) and produces the tracks
-                velo_cluster=raw + clusters, velo_track=14 * n_clusters + 4 * (n_events * n_layers + 1) + tracks)
+                # per-kernel shares: each compulsory byte is charged to the kernel that moves it.  The
+                # cluster kernel reads the raw banks; the track kernel writes the compacted clusters (it carries the
+                # compaction) and the tracks.  The slab between the two is overhead, not algorithmic traffic.
+                velo_cluster=raw, velo_track=clusters + tracks)
 
 
 def run_reference(args):
@@ -294,14 +313,22 @@ def run_ours(args):
     peak, peak_src = peaks()
     dom_bytes = ab.get(names[dom], 0)
     achieved = dom_bytes / (mean_ms[dom] * 1e-3) / 1e9
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "dram_traffic.json")
-    if os.path.exists(tpath):
-        with open(tpath) as f:
-            traffic = json.load(f).get(names[dom], {}).get(f"config{args.config}_{n_events}")
+    # DRAM traffic and instruction counts of the same launch configuration, from the committed ncu capture
+    counters = ncu_counters(f"config{args.config}_{n_events}")
+    traffic = counters.get(names[dom], {}).get("dram_bytes")
     roofline = dict(bound="hbm", kernel=names[dom], achieved=achieved, peak=peak, unit="GB/s", frac=achieved / peak,
                     traffic=traffic, peak_source=peak_src, algorithmic_bytes_per_launch=dom_bytes,
-                    kernel_ms=float(mean_ms[dom]), kernel_share_of_step=float(mean_ms[dom] / mean_ms.sum()))
+                    kernel_ms=float(mean_ms[dom]), kernel_share_of_step=float(mean_ms[dom] / mean_ms.sum()),
+                    traffic_source=counters.get("_source"))
+    # why the HBM fraction is low: the path is bound by instruction issue, not by memory
+    issue_peak = 148 * 4 * (clocks or {}).get("sm_mhz", 1965.0) * 1e6 if clocks and clocks.get("sm_mhz") else 148 * 4 * 1.965e9
+    roofline_issue = None
+    if names[dom] in counters and counters[names[dom]].get("warp_instructions"):
+        wi = counters[names[dom]]["warp_instructions"]
+        roofline_issue = dict(bound="alu", kernel=names[dom], achieved=wi / (mean_ms[dom] * 1e-3) / 1e9,
+                              peak=issue_peak / 1e9, unit="G warp-instr/s", frac=wi / (mean_ms[dom] * 1e-3) / issue_peak,
+                              warp_instructions_per_launch=wi, active_lanes_per_instruction=counters[names[dom]].get("lanes"),
+                              source=counters.get("_source"))
     path_gbs = ab["total"] / (ms_step * 1e-3) / 1e9
     roofline_path = dict(bound="hbm", achieved=path_gbs, peak=peak, unit="GB/s", frac=path_gbs / peak,
                          frac_of_8TBs_nominal=path_gbs / 8000.0, algorithmic_bytes_per_step=ab["total"],
@@ -341,7 +368,8 @@ def run_ours(args):
                  ms_per_step=e2e_ms),
         gpu_launches=launches,
         kernels={n: float(m) for n, m in zip(names, mean_ms)},
-        roofline=roofline, roofline_path=roofline_path, cpu_baseline=cpu_baseline, clocks=clocks,
+        roofline=roofline, roofline_path=roofline_path, roofline_issue=roofline_issue, cpu_baseline=cpu_baseline,
+        clocks=clocks,
     )
     print(json.dumps(line, default=float))
     if dist is not None:

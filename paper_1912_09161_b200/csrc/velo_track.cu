@@ -77,6 +77,7 @@ struct Smem {
   float ttx[C::kCapTracks], tty[C::kCapTracks];  // slopes of the last segment (older -> newest hit)
   uint32_t tstate[C::kCapTracks];                // newest << 16 | weak_ok << 15 | nhits << 8 | missed (0xFF: closed)
   uint16_t tseedB[C::kCapTracks];                // track_key: event-local index of the seed's middle hit
+  uint16_t fsel[C::kCapTracks];                  // hit of layer C chosen by the track in T1 (0xFFFF: none)
   uint16_t bucket[4][kBuckets + 2];
   uint32_t lo[kMaxLayers + 1];
   uint32_t src[kMaxLayers];  // first entry of every layer in the arrays X, Y, Z, PHI are read from
@@ -216,7 +217,7 @@ __device__ __forceinline__ void track_event(const TrackLaunch& a, uint32_t e, Sm
   const uint32_t lane = lane_id(), warp = tid >> 5;
   const uint32_t co = a.clusters.event_offsets[e];
   load_offsets<C>(a, e, sm, co);
-  if (tid == 0) { sm.flags = 0; sm.min_active[0] = 0; sm.min_active[1] = 0; }
+  if (tid == 0) { sm.flags = 0; sm.min_active[0] = 0; sm.min_active[1] = 0; sm.n_doublets = 0; }
   __syncthreads();
   if (C::kCopier && tid >= (uint32_t)C::kThreads) {
     // copier warp: layers in the order the search stages them (their slab lines are then in L2 for both readers)
@@ -260,10 +261,10 @@ __device__ __forceinline__ void track_event(const TrackLaunch& a, uint32_t e, Sm
 
     // ---- T1 forward: best hit of layer C per active track (nothing of C is used yet); claim with (bits(S), key)
     const uint32_t first = min(sm.min_active[i & 1], first_new);
-    if (tid == 0) { sm.min_active[(i - 1) & 1] = 0xFFFFFFFFu; sm.n_doublets = 0; }
+    if (tid == 0) sm.min_active[(i - 1) & 1] = 0xFFFFFFFFu;
 #pragma unroll 1
     for (uint32_t k = tid; k < max(nA, nC); k += C::kThreads) { sm.claimA[k] = kNoClaim; sm.claimC[k] = kNoClaim; }
-    uint16_t* fsel = reinterpret_cast<uint16_t*>(sm.doublets);  // hit of layer C chosen by every track (T1 -> T2)
+    uint16_t* fsel = sm.fsel;
 #pragma unroll 1
     for (uint32_t t = first + tid; t < n_tracks; t += C::kThreads) {
       fsel[t] = 0xFFFFu;
@@ -306,6 +307,26 @@ __device__ __forceinline__ void track_event(const TrackLaunch& a, uint32_t e, Sm
         atomicMin(&sm.best[ic_best], (best & 0xFFFFFFFF00000000ull) | sm.tseedB[t]);
       }
     }
+    // ---- T3/S1 (same phase as T1: it reads only the used flags of layers A and B, final since the last T4): every
+    //      unused b lists the unused hits of layer A inside its phi window as (b, a) doublets
+    const bool seeding = nA != 0 && nB != 0 && nC != 0;
+#pragma unroll 1
+    for (uint32_t kb = tid; kb < nB; kb += C::kThreads) {
+      const uint32_t wb = recB[kb].w;
+      if (!seeding || (wb & kUsedBit)) continue;
+      const int w = P.w_seed_phi16, phb = phi_of(wb);
+      uint32_t ia = lower_bound_phi(bucketA, recA, nA, wrap16(phb - w));
+#pragma unroll 1
+      for (uint32_t k = 0; k < nA; ++k, ++ia) {
+        if (ia >= nA) ia -= nA;
+        const uint32_t wa = recA[ia].w;
+        const int d = wrap16(phi_of(wa) - phb);
+        if (d > w || d < -w) break;
+        if (wa & kUsedBit) continue;
+        const uint32_t pos = atomicAdd(&sm.n_doublets, 1u);
+        if (pos < (uint32_t)C::kCapDoublets) sm.doublets[pos] = kb | (ia << 16);  // else: S2 enumerates again
+      }
+    }
     tsync<C>();  // B2
     // ---- T2 resolve: the minimal claim wins the hit (track keys are unique, so the low half of the claim names the
     //      winner); everyone else counts a miss
@@ -314,8 +335,11 @@ __device__ __forceinline__ void track_event(const TrackLaunch& a, uint32_t e, Sm
       const uint32_t st = sm.tstate[t];
       if ((st & 0xFFu) == 0xFFu) continue;
       const uint32_t fc = fsel[t];
+      // the winner puts the claim word back to "none" (losers then still fail the test: a key is never 0xFFFF), so
+      // best[] is clean again for the per-b argmin of T3 without a pass of its own
       const bool won = fc != 0xFFFFu && (uint16_t)sm.best[fc] == sm.tseedB[t];
       if (won) {
+        sm.best[fc] = kNoClaim;
         const uint32_t q = st >> 16, cg = C0 + fc;
         float xq, yq, zq;
         if (q < A1) {
@@ -349,42 +373,35 @@ __device__ __forceinline__ void track_event(const TrackLaunch& a, uint32_t e, Sm
     }
     tsync<C>();  // B3
 
-    // ---- T3/S1: every unused b lists the unused hits of layer A inside its phi window as (b, a) doublets
-    const bool seeding = nA != 0 && nB != 0 && nC != 0;
-#pragma unroll 1
-    for (uint32_t k = nB + tid; k < nC; k += C::kThreads) sm.best[k] = kNoClaim;  // forward claims beyond layer B's size
-#pragma unroll 1
-    for (uint32_t kb = tid; kb < nB; kb += C::kThreads) {
-      sm.best[kb] = kNoClaim;  // forward claims are done with; from here on: per-b argmin
-      const uint32_t wb = recB[kb].w;
-      if (!seeding || (wb & kUsedBit)) continue;
-      const int w = P.w_seed_phi16, phb = phi_of(wb);
-      uint32_t ia = lower_bound_phi(bucketA, recA, nA, wrap16(phb - w));
-#pragma unroll 1
-      for (uint32_t k = 0; k < nA; ++k, ++ia) {
-        if (ia >= nA) ia -= nA;
-        const uint32_t wa = recA[ia].w;
-        const int d = wrap16(phi_of(wa) - phb);
-        if (d > w || d < -w) break;
-        if (wa & kUsedBit) continue;
-        const uint32_t pos = atomicAdd(&sm.n_doublets, 1u);
-        if (pos < (uint32_t)C::kCapDoublets) sm.doublets[pos] = kb | (ia << 16);
-        else process_doublet(c, recA, recB, recC, bucketC, nC, kb, ia);  // list full: do it here (same result)
-      }
-    }
-    tsync<C>();  // B4
-    // ---- T3/S2: one thread per doublet
-    {
-      const uint32_t nd = min(sm.n_doublets, (uint32_t)C::kCapDoublets);
+    // ---- T3/S2: one thread per doublet; if the list overflowed, one thread per b walks its doublets itself
+    if (sm.n_doublets <= (uint32_t)C::kCapDoublets) {
+      const uint32_t nd = sm.n_doublets;
 #pragma unroll 1
       for (uint32_t d = tid; d < nd; d += C::kThreads) {
         const uint32_t v = sm.doublets[d];
         process_doublet(c, recA, recB, recC, bucketC, nC, v & 0xFFFFu, v >> 16);
       }
+    } else {
+#pragma unroll 1
+      for (uint32_t kb = tid; kb < nB; kb += C::kThreads) {
+        const uint32_t wb = recB[kb].w;
+        if (wb & kUsedBit) continue;
+        const int w = P.w_seed_phi16, phb = phi_of(wb);
+        uint32_t ia = lower_bound_phi(bucketA, recA, nA, wrap16(phb - w));
+#pragma unroll 1
+        for (uint32_t k = 0; k < nA; ++k, ++ia) {
+          if (ia >= nA) ia -= nA;
+          const uint32_t wa = recA[ia].w;
+          const int d = wrap16(phi_of(wa) - phb);
+          if (d > w || d < -w) break;
+          if (!(wa & kUsedBit)) process_doublet(c, recA, recB, recC, bucketC, nC, kb, ia);
+        }
+      }
     }
     tsync<C>();  // B5
 
     // ---- T4a: every b with a triplet claims its a and its c with (bits(S), b)
+    if (tid == 0) sm.n_doublets = 0;  // S2 is over; the next S1 starts after two more barriers
     const uint32_t roundsB = seeding ? (nB + C::kThreads - 1) / C::kThreads : 0;  // block-uniform
 #pragma unroll 1
     for (uint32_t kb = tid; kb < nB && seeding; kb += C::kThreads) {
