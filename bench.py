@@ -179,27 +179,14 @@ def run_ours(args):
 
         dist.init_process_group("nccl", device_id=device)
 
-    def barrier():
-        if dist is not None:
-            dist.barrier()
+    from paper_1912_09161_b200 import replicas
 
-    def max_over_ranks(v):
-        if dist is None:
-            return v
-        t = torch.tensor([v], dtype=torch.float64, device=device)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
-
-    def sum_over_ranks(v):
-        if dist is None:
-            return v
-        t = torch.tensor([v], dtype=torch.float64, device=device)
-        dist.all_reduce(t, op=dist.ReduceOp.SUM)
-        return float(t.item())
+    red = replicas.Reducer(device)
+    barrier, max_over_ranks, sum_over_ranks = red.barrier, red.max, red.sum
 
     # ---- workload: every rank reconstructs its own batch (batch_index = rank)
     t_gen = time.time()
-    batch = workload.generate(args.config, n_events=args.events, batch_index=rank)
+    batch = workload.generate(args.config, n_events=args.events, batch_index=replicas.batch_index_of(rank))
     t_gen = time.time() - t_gen
     geo = batch.geometry
     n_events, L = batch.n_events, geo.n_layers

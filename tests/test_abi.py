@@ -1,0 +1,66 @@
+"""The C-ABI library loads without a GPU and exports every function include/allen_velo.h declares (no compute calls)."""
+import ctypes
+import os
+import re
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_functions():
+    text = open(os.path.join(ROOT, "include", "allen_velo.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    names = re.findall(r"\b(allen_velo_[a-z_]+)\s*\(", text)
+    return sorted(set(names))
+
+
+def test_header_declares_the_three_calls_of_the_north_star():
+    names = declared_functions()
+    for n in ("allen_velo_create", "allen_velo_reconstruct", "allen_velo_destroy"):
+        assert n in names
+
+
+def test_library_exports_every_declared_symbol():
+    from paper_1912_09161_b200 import build
+
+    lib = ctypes.CDLL(build.build())
+    for name in declared_functions():
+        assert hasattr(lib, name), name
+
+
+def test_calls_that_need_no_device():
+    from paper_1912_09161_b200 import binding
+
+    lib = binding.load_library()
+    p = binding.allen_velo_default_params()
+    assert (p.w_seed_phi16, p.w_fwd_phi16, p.max_skipped) == (512, 512, 1)
+    assert (p.max_slope, p.s_seed, p.s_fwd, p.s_weak) == (ctypes.c_float(0.4).value, 2.0 ** -6, 2.0 ** -4, 2.0 ** -7)
+    names = [lib.allen_velo_kernel_name(i).decode() for i in range(lib.allen_velo_kernel_count())]
+    assert "velo_cluster" in names and "velo_track" in names
+    # null handle / null arguments are rejected, not dereferenced
+    assert lib.allen_velo_create(None, None) == binding.ERR_INVALID
+    assert lib.allen_velo_workspace_bytes(None, 10, 1000) == 0
+    assert lib.allen_velo_set_workspace(None, None, 0) == binding.ERR_INVALID
+    assert lib.allen_velo_reconstruct(None, None, None, 0, None, None, None) == binding.ERR_INVALID
+    lib.allen_velo_destroy(None)
+
+
+def test_binding_structs_match_the_header_layout():
+    """ctypes mirrors of the ABI structs: field order and sizes as the C compiler lays them out."""
+    from paper_1912_09161_b200 import binding
+
+    assert ctypes.sizeof(binding.allen_velo_params_t) == 28
+    assert ctypes.sizeof(binding.allen_velo_geometry_t) == 24 + 3 * 8 + 28 + 4  # padded to 8
+    assert ctypes.sizeof(binding.allen_velo_clusters_t) == 8 + 12 * 8
+    assert ctypes.sizeof(binding.allen_velo_tracks_t) == 8 + 7 * 8
+
+
+def test_product_path_refuses_to_run_without_cuda(geometry):
+    import pytest
+    import torch
+
+    from paper_1912_09161_b200 import binding
+
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    with pytest.raises(RuntimeError, match="no CPU fallback"):
+        binding.AllenVelo(geometry)
