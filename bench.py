@@ -198,6 +198,7 @@ def run_ours(args):
     oc, ot = binding.alloc_outputs(n_events, L, ccap, ccap // 3, ccap // 2, device, with_checksum=False)
     ws = torch.empty(velo.workspace_bytes(n_events, raw_bytes), dtype=torch.uint8, device=device)
     velo.set_workspace(ws)
+    velo.set_occupancy_hint(n_events, raw_bytes)
     h_raw = torch.from_numpy(batch.raw).pin_memory()
     h_off = torch.from_numpy(batch.event_offsets.view(np.int32)).pin_memory()
     d_raw = h_raw.to(device)

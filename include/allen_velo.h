@@ -112,6 +112,11 @@ size_t allen_velo_workspace_bytes(const allen_velo_t* handle, uint32_t n_events,
 /* Registers a caller-owned DEVICE buffer (256-byte aligned) as workspace for subsequent reconstruct() calls. */
 int allen_velo_set_workspace(allen_velo_t* handle, void* dev_ptr /* DEVICE */, size_t bytes);
 
+/* Optional: average number of SP words per (event, layer) of the batches to come (raw bytes / 4 / n_events / n_layers is
+ * close enough).  The results never depend on it; it selects the cluster-kernel instance whose shared-memory
+ * capacity suits the occupancy (above 192 words per layer: 512 entries per layer instead of 256).  0 = no hint. */
+int allen_velo_set_occupancy_hint(allen_velo_t* handle, uint32_t sp_words_per_layer);
+
 /* Enqueues the whole hot path for one batch on `cuda_stream` and returns WITHOUT synchronising.
  *   raw_banks      DEVICE, 16-byte aligned: events in raw format v1 (R1) back to back
  *   event_offsets  DEVICE [n_events+1]: byte offset of every event in raw_banks, multiples of 16

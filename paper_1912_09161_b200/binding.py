@@ -62,6 +62,8 @@ def load_library():
         L.allen_velo_workspace_bytes.restype = ctypes.c_size_t
         L.allen_velo_set_workspace.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t]
         L.allen_velo_set_workspace.restype = ctypes.c_int
+        L.allen_velo_set_occupancy_hint.argtypes = [ctypes.c_void_p, ctypes.c_uint32]
+        L.allen_velo_set_occupancy_hint.restype = ctypes.c_int
         L.allen_velo_reconstruct.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_uint32,
                                              ctypes.c_void_p, ctypes.POINTER(allen_velo_clusters_t),
                                              ctypes.POINTER(allen_velo_tracks_t)]
@@ -184,6 +186,12 @@ class AllenVelo:
     def workspace_bytes(self, n_events: int, raw_bytes: int) -> int:
         return int(self._lib.allen_velo_workspace_bytes(self._h, n_events, raw_bytes))
 
+    def set_occupancy_hint(self, n_events: int, raw_bytes: int) -> None:
+        """Tell the library the average SP words per (event, layer) of the batches to come (performance only)."""
+        per_layer = raw_bytes // 4 // max(1, n_events * self.n_layers)
+        if self._lib.allen_velo_set_occupancy_hint(self._h, per_layer) != OK:
+            raise RuntimeError("allen_velo_set_occupancy_hint failed")
+
     def set_workspace(self, tensor) -> None:
         """`tensor`: a torch uint8 CUDA tensor the caller keeps alive (kept referenced here too)."""
         rc = self._lib.allen_velo_set_workspace(self._h, tensor.data_ptr(), tensor.numel() * tensor.element_size())
@@ -254,6 +262,7 @@ def reconstruct_batch(velo: AllenVelo, raw: np.ndarray, event_offsets: np.ndarra
     oc, ot = alloc_outputs(n_events, velo.n_layers, ccap, tcap, hcap, device, with_checksum)
     ws = torch.empty(velo.workspace_bytes(n_events, raw_bytes), dtype=torch.uint8, device=device)
     velo.set_workspace(ws)
+    velo.set_occupancy_hint(n_events, raw_bytes)
     rc = velo.reconstruct(d_raw, d_off, n_events, None, oc, ot)
     if rc != OK:
         raise RuntimeError(f"allen_velo_reconstruct failed with {rc}: {velo.last_error()}")

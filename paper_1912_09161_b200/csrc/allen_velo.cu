@@ -19,6 +19,7 @@ struct allen_velo {
   uint32_t last_launches = 0;
   uint32_t n_mid_sms = 0;      // SM ids the mid-slot pool of the cluster kernel covers
   uint32_t n_sms = 0;
+  uint32_t sp_words_per_layer = 0;  // caller's hint (0: none)
   cudaStream_t side[2] = {nullptr, nullptr};  // the larger track-kernel instances run beside the first one
   cudaEvent_t fork_join[3] = {nullptr, nullptr, nullptr};
   std::string last_error;
@@ -174,6 +175,12 @@ size_t allen_velo_workspace_bytes(const allen_velo_t* h, uint32_t n_events, size
   return fixed_bytes(n_events, h->dev.n_layers, h->n_mid_sms) + entries * per_entry_bytes() + 16 * kAlign;
 }
 
+int allen_velo_set_occupancy_hint(allen_velo_t* h, uint32_t sp_words_per_layer) {
+  if (!h) return ALLEN_VELO_ERR_INVALID;
+  h->sp_words_per_layer = sp_words_per_layer;
+  return ALLEN_VELO_OK;
+}
+
 int allen_velo_set_workspace(allen_velo_t* h, void* dev_ptr, size_t bytes) {
   if (!h) return ALLEN_VELO_ERR_INVALID;
   if (dev_ptr && (reinterpret_cast<uintptr_t>(dev_ptr) % kAlign)) return fail(h, ALLEN_VELO_ERR_INVALID, "workspace misaligned");
@@ -273,7 +280,8 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   cl.n_mid_sms = h->n_mid_sms;
   cl.n_big_slots = n_big;
   cl.with_checksum = oc->checksum != nullptr;
-  if ((err = launch_cluster(cl, stream)) != cudaSuccess) return fail(h, ALLEN_VELO_ERR_CUDA, "cluster kernel", err);
+  const bool big_layers = h->sp_words_per_layer > 192;  // the larger shared-memory instance keeps such layers on chip
+  if ((err = launch_cluster(cl, big_layers, stream)) != cudaSuccess) return fail(h, ALLEN_VELO_ERR_CUDA, "cluster kernel", err);
   h->last_launches++;
   mark(1);
 

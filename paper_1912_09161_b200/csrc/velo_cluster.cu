@@ -35,7 +35,13 @@ namespace {
 
 constexpr int kWarps = 4;  // warps per CTA (independent work items)
 // per-warp shared memory
-constexpr uint32_t kCapSp = 256, kHashBits = 9, kCapEdges = 256, kCapCl = 256;
+// kCap SP words / clusters / edges per layer, 2 * kCap hash slots; two instances: 256 (nu ~ 6) and 512 (busier batches)
+template <uint32_t kCap>
+struct Caps {
+  static constexpr uint32_t kCapSp = kCap, kCapEdges = kCap, kCapCl = kCap;
+  static constexpr uint32_t kHashBits = kCap == 256 ? 9 : 10;
+  static_assert(kCap == 256 || kCap == 512, "hash bits");
+};
 // pool slots in global memory
 constexpr uint32_t kMidCl = 1024;
 constexpr uint32_t kBigSp = 8192, kBigHashBits = 14, kBigEdges = 7 * kBigSp, kBigCl = 2 * kBigSp;
@@ -411,8 +417,9 @@ __device__ __noinline__ void finish_layer_generic(const ClusterLaunch& a, const 
   finish_layer<kChecksum>(a, cs, ss, item, slab0, n_cl);
 }
 
-template <bool kChecksum>
+template <bool kChecksum, uint32_t kCap>
 struct WarpSmem {
+  static constexpr uint32_t kCapSp = kCap, kCapEdges = kCap, kCapCl = kCap, kHashBits = Caps<kCap>::kHashBits;
   uint32_t sp[kCapSp];
   uint32_t tab[1u << kHashBits];
   uint16_t lab[2 * kCapSp];
@@ -421,7 +428,7 @@ struct WarpSmem {
   uint32_t ccks[kChecksum ? kCapCl : 1];
   uint32_t n_edges;
 };
-static_assert(1024 + 6 * kCapCl <= 4 * kCapSp + 4 * (1u << kHashBits), "sort scratch aliases sp + tab");
+static_assert(1024 + 6 * 256 <= 4 * 256 + 4 * (1u << 9) && 1024 + 6 * 512 <= 4 * 512 + 4 * (1u << 10), "sort scratch aliases sp + tab");
 
 // Layout of the pool slots (bytes from the slot base).
 struct MidSlot {
@@ -451,10 +458,11 @@ __device__ __forceinline__ void stores_at(unsigned char* base, size_t stats, siz
   ss.tmp = t; ss.order = t + cap; ss.phis = t + 2 * cap;
 }
 
-template <bool kChecksum>
+template <bool kChecksum, uint32_t kCap>
 __global__ void __launch_bounds__(kWarps * 32) velo_cluster_kernel(const __grid_constant__ ClusterLaunch a) {
+  constexpr uint32_t kCapSp = kCap, kCapEdges = kCap, kCapCl = kCap, kHashBits = Caps<kCap>::kHashBits;
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  using WS = WarpSmem<kChecksum>;
+  using WS = WarpSmem<kChecksum, kCap>;
   WS& ws = reinterpret_cast<WS*>(smem_raw)[threadIdx.x >> 5];
   const DeviceGeometry& g = a.geo;
   const uint32_t lane = lane_id();
@@ -616,23 +624,25 @@ __global__ void __launch_bounds__(kWarps * 32) velo_cluster_kernel(const __grid_
 size_t cluster_mid_slot_bytes() { return MidSlot::kBytes; }
 size_t cluster_big_slot_bytes() { return BigSlot::kBytes; }
 
-cudaError_t launch_cluster(const ClusterLaunch& a, cudaStream_t stream) {
+template <bool kChecksum, uint32_t kCap>
+cudaError_t launch_cluster_instance(const ClusterLaunch& a, uint32_t grid, cudaStream_t stream) {
+  const size_t smem = sizeof(WarpSmem<kChecksum, kCap>) * kWarps;
+  cudaError_t err = cudaFuncSetAttribute(velo_cluster_kernel<kChecksum, kCap>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (err != cudaSuccess) return err;
+  velo_cluster_kernel<kChecksum, kCap><<<grid, kWarps * 32, smem, stream>>>(a);
+  return cudaGetLastError();
+}
+
+// `big_layers`: the batch averages more than 192 SP words per layer (the host knows the raw size): the instance with
+// 512 entries per layer in shared memory keeps such layers on chip at half the occupancy.
+cudaError_t launch_cluster(const ClusterLaunch& a, bool big_layers, cudaStream_t stream) {
   const uint32_t items = a.n_events * a.geo.n_layers;
   if (items == 0) return cudaSuccess;
   const uint32_t grid = (items + kWarps - 1) / kWarps;
-  cudaError_t err;
-  if (a.with_checksum) {
-    const size_t smem = sizeof(WarpSmem<true>) * kWarps;
-    err = cudaFuncSetAttribute(velo_cluster_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (err != cudaSuccess) return err;
-    velo_cluster_kernel<true><<<grid, kWarps * 32, smem, stream>>>(a);
-  } else {
-    const size_t smem = sizeof(WarpSmem<false>) * kWarps;
-    err = cudaFuncSetAttribute(velo_cluster_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (err != cudaSuccess) return err;
-    velo_cluster_kernel<false><<<grid, kWarps * 32, smem, stream>>>(a);
-  }
-  return cudaGetLastError();
+  if (a.with_checksum)
+    return big_layers ? launch_cluster_instance<true, 512>(a, grid, stream) : launch_cluster_instance<true, 256>(a, grid, stream);
+  return big_layers ? launch_cluster_instance<false, 512>(a, grid, stream) : launch_cluster_instance<false, 256>(a, grid, stream);
 }
 
 }  // namespace velo

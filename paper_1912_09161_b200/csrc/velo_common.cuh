@@ -118,7 +118,7 @@ struct ClusterLaunch {
   uint32_t n_mid_sms, n_big_slots;
   bool with_checksum;
 };
-cudaError_t launch_cluster(const ClusterLaunch& a, cudaStream_t stream);
+cudaError_t launch_cluster(const ClusterLaunch& a, bool big_layers, cudaStream_t stream);
 size_t cluster_mid_slot_bytes();
 size_t cluster_big_slot_bytes();
 

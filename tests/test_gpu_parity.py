@@ -197,3 +197,21 @@ def test_parity_on_a_larger_batch(velo, oracle_of):
     """2000 nu=6 events: several waves of CTAs per SM, events of every size class in one batch."""
     batch, ref = oracle_of(2, 2000)
     check_parity(velo, batch, ref)
+
+
+@pytest.mark.parametrize("config,n_events,hint", [(3, 48, 0), (1, 64, 1000), (2, 200, 1000)])
+def test_results_do_not_depend_on_the_occupancy_hint(velo, oracle_of, config, n_events, hint):
+    """Both cluster-kernel instances (256 / 512 entries per layer in shared memory) and the pool paths behind them."""
+    from paper_1912_09161_b200 import binding
+    from tests.helpers import compare_clusters
+
+    batch, ref = oracle_of(config, n_events)
+    orig = velo.set_occupancy_hint
+    velo.set_occupancy_hint = lambda n, b: orig(1, 4 * hint * velo.n_layers)  # reconstruct_batch sets its own otherwise
+    try:
+        clusters, tracks = binding.reconstruct_batch(velo, batch.raw, batch.event_offsets)
+    finally:
+        velo.set_occupancy_hint = orig
+    c, t = as_oracle_types(clusters, tracks)
+    assert not compare_clusters(c, ref.clusters)
+    assert np.array_equal(t.hits, ref.tracks.hits)
