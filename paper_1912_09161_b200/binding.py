@@ -287,3 +287,112 @@ def reconstruct_batch(velo: AllenVelo, raw: np.ndarray, event_offsets: np.ndarra
     for name in ("x0", "y0", "tx", "ty"):
         tracks[name] = host(getattr(ot, name), np.float32)[:min(nt, tcap)]
     return clusters, tracks
+
+
+class StreamedVelo:
+    """Host-to-host reconstruction of a large batch in chunks on several CUDA streams (the paper's host loop
+    gives every thread its own stream and ~1000-event batches so that copies and kernels of different batches overlap).
+
+    Every stream owns a handle, device input/output buffers, a workspace and pinned host buffers for the track output.
+    `reconstruct` cuts the batch into chunks of `chunk_events`, and for each chunk enqueues on its stream: H2D of the
+    raw banks and offsets, allen_velo_reconstruct, D2H of the offsets; once those arrive (the host waits for THIS stream
+    only, the others keep working) the D2H of exactly the tracks found.  All arithmetic runs in the CUDA kernels; this
+    class only moves bytes and calls the C ABI.
+    """
+
+    def __init__(self, geometry, chunk_events: int, max_chunk_raw_bytes: int, n_streams: int = 2, device="cuda:0",
+                 params: dict | None = None):
+        import torch
+
+        self.device, self.chunk_events, self.n_layers = torch.device(device), int(chunk_events), geometry.n_layers
+        self.max_raw = (int(max_chunk_raw_bytes) + 15) // 16 * 16
+        ccap = self.max_raw // 4 + 4096          # clusters <= SP words (x2 only for adversarial input: flagged, not UB)
+        tcap, hcap = ccap // 3 + 16, ccap
+        self.slots = []
+        for _ in range(n_streams):
+            v = AllenVelo(geometry, params)
+            oc, ot = alloc_outputs(self.chunk_events, self.n_layers, ccap, tcap, hcap, self.device, with_checksum=False)
+            ws = torch.empty(v.workspace_bytes(self.chunk_events, self.max_raw), dtype=torch.uint8, device=self.device)
+            v.set_workspace(ws)
+            v.set_occupancy_hint(self.chunk_events, self.max_raw)
+            pin = lambda n, dt: torch.empty(max(int(n), 1), dtype=dt).pin_memory()
+            self.slots.append(dict(
+                velo=v, oc=oc, ot=ot, stream=torch.cuda.Stream(device=self.device),
+                d_raw=torch.empty(self.max_raw, dtype=torch.uint8, device=self.device),
+                d_off=torch.empty(self.chunk_events + 1, dtype=torch.int32, device=self.device),
+                h_off=pin(self.chunk_events + 1, torch.int32), h_te=pin(self.chunk_events + 1, torch.int32),
+                h_st=pin(self.chunk_events, torch.int32), h_ho=pin(tcap + 1, torch.int32),
+                h_hits=pin(hcap, torch.int16), h_fit=[pin(tcap, torch.float32) for _ in range(4)],
+                pending=None))
+        self.h2d_bytes = self.d2h_bytes = 0
+
+    def _finish(self, s):
+        """Second half of a chunk: sizes have arrived -> fetch exactly the tracks found."""
+        import torch
+
+        p = s["pending"]
+        if p is None:
+            return None
+        s["stream"].synchronize()
+        n = p["n_events"]
+        nt = int(s["h_te"][n])
+        with torch.cuda.stream(s["stream"]):
+            s["h_ho"][:nt + 1].copy_(s["ot"].hit_offsets[:nt + 1], non_blocking=True)
+        s["stream"].synchronize()
+        nh = int(s["h_ho"][nt])
+        with torch.cuda.stream(s["stream"]):
+            for hb, db in zip(s["h_fit"], (s["ot"].x0, s["ot"].y0, s["ot"].tx, s["ot"].ty)):
+                hb[:nt].copy_(db[:nt], non_blocking=True)
+            s["h_hits"][:nh].copy_(s["ot"].hits[:nh], non_blocking=True)
+        self.d2h_bytes += 4 * (n + 1) + 4 * n + 4 * (nt + 1) + 16 * nt + 2 * nh
+        s["pending"] = None
+        return dict(first_event=p["first"], n_events=n, n_tracks=nt, n_hits=nh)
+
+    def reconstruct(self, h_raw, h_event_offsets, on_chunk=None):
+        """h_raw: pinned uint8 tensor (raw format v1, events back to back); h_event_offsets: int64/int32 numpy array
+        [n_events+1].  Calls on_chunk(info, slot) when a chunk's tracks are on their way to the slot's pinned buffers
+        (valid after slot['stream'].synchronize()).  Returns the list of chunk infos."""
+        import torch
+
+        off = np.asarray(h_event_offsets).astype(np.int64)
+        n_events = len(off) - 1
+        self.h2d_bytes = self.d2h_bytes = 0
+        infos = []
+        for k, first in enumerate(range(0, n_events, self.chunk_events)):
+            s = self.slots[k % len(self.slots)]
+            done = self._finish(s)  # the slot's previous chunk (the other slots keep running meanwhile)
+            if done is not None:
+                infos.append(done)
+                if on_chunk:
+                    on_chunk(done, s)
+            last = min(first + self.chunk_events, n_events)
+            n = last - first
+            b0, b1 = int(off[first]), int(off[last])
+            if b1 - b0 > self.max_raw:
+                raise ValueError("chunk larger than max_chunk_raw_bytes")
+            s["stream"].synchronize()  # the slot's host staging buffers are free again
+            s["h_off"][:n + 1] = torch.from_numpy((off[first:last + 1] - b0).astype(np.int32))
+            with torch.cuda.stream(s["stream"]):
+                s["d_raw"][:b1 - b0].copy_(h_raw[b0:b1], non_blocking=True)
+                s["d_off"][:n + 1].copy_(s["h_off"][:n + 1], non_blocking=True)
+                rc = s["velo"].reconstruct(s["d_raw"], s["d_off"], n, s["stream"], s["oc"], s["ot"])
+                if rc != OK:
+                    raise RuntimeError(f"allen_velo_reconstruct failed with {rc}: {s['velo'].last_error()}")
+                s["h_te"][:n + 1].copy_(s["ot"].event_offsets[:n + 1], non_blocking=True)
+                s["h_st"][:n].copy_(s["oc"].status[:n], non_blocking=True)
+            self.h2d_bytes += (b1 - b0) + 4 * (n + 1)
+            s["pending"] = dict(first=first, n_events=n)
+        for s in self.slots:
+            done = self._finish(s)
+            if done is not None:
+                infos.append(done)
+                if on_chunk:
+                    on_chunk(done, s)
+        for s in self.slots:
+            s["stream"].synchronize()
+        return sorted(infos, key=lambda i: i["first_event"])
+
+    def destroy(self):
+        for s in self.slots:
+            s["velo"].destroy()
+        self.slots = []

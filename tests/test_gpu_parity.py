@@ -215,3 +215,40 @@ def test_results_do_not_depend_on_the_occupancy_hint(velo, oracle_of, config, n_
     c, t = as_oracle_types(clusters, tracks)
     assert not compare_clusters(c, ref.clusters)
     assert np.array_equal(t.hits, ref.tracks.hits)
+
+
+def test_streamed_host_to_host_reconstruction(geometry, oracle_of):
+    """binding.StreamedVelo: chunks on several streams give the oracle's tracks, chunk by chunk, in host memory."""
+    import torch
+
+    from paper_1912_09161_b200 import binding
+
+    batch, ref = oracle_of(2, 200)
+    h_raw = torch.from_numpy(batch.raw).pin_memory()
+    got = {}
+
+    def on_chunk(info, slot):
+        slot["stream"].synchronize()
+        nt, nh, n = info["n_tracks"], info["n_hits"], info["n_events"]
+        got[info["first_event"]] = dict(
+            te=slot["h_te"][:n + 1].numpy().view(np.uint32).copy(), ho=slot["h_ho"][:nt + 1].numpy().view(np.uint32).copy(),
+            hits=slot["h_hits"][:nh].numpy().view(np.uint16).copy(), tx=slot["h_fit"][2][:nt].numpy().copy(),
+            status=slot["h_st"][:n].numpy().copy())
+
+    sv = binding.StreamedVelo(geometry, 64, int(batch.raw.size), n_streams=3)
+    try:
+        infos = sv.reconstruct(h_raw, batch.event_offsets.astype(np.int64), on_chunk=on_chunk)
+    finally:
+        sv.destroy()
+    assert [i["first_event"] for i in infos] == [0, 64, 128, 192]
+    rt = ref.tracks
+    for first, g in got.items():
+        n = len(g["te"]) - 1
+        t0, t1 = int(rt.event_offsets[first]), int(rt.event_offsets[first + n])
+        assert np.array_equal(g["te"], rt.event_offsets[first:first + n + 1] - t0)
+        h0, h1 = int(rt.hit_offsets[t0]), int(rt.hit_offsets[t1])
+        assert np.array_equal(g["ho"], rt.hit_offsets[t0:t1 + 1] - h0)
+        assert np.array_equal(g["hits"], rt.hits[h0:h1])
+        assert np.allclose(g["tx"], rt.tx[t0:t1], rtol=1e-5, atol=1e-8)
+        assert not g["status"].any()
+    assert sum(i["n_tracks"] for i in infos) == int(rt.event_offsets[-1])
