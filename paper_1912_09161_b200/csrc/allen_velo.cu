@@ -60,7 +60,7 @@ uint32_t big_slots(uint32_t items) { return 16 + items / 4096; }
 size_t fixed_bytes(uint32_t n_events, uint32_t n_layers, uint32_t n_mid_sms) {
   const uint32_t items = n_events * n_layers;
   size_t b = 0;
-  b += align_up((size_t)items * 4) * 2;                           // counts, slab_base
+  b += align_up((size_t)items * 4) * 2 + align_up((size_t)items * 18 * 4);  // counts, slab_base, layer descriptors
   b += align_up(scan_state_words(items) * 8);                     // scan state (clusters)
   b += align_up(8 + (size_t)n_mid_sms * 4);                       // big-pool counter, mid masks
   b += align_up((size_t)n_mid_sms * 32 * cluster_mid_slot_bytes());
@@ -221,6 +221,7 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   Carve cv{static_cast<unsigned char*>(h->ws)};
   uint32_t* counts = cv.take<uint32_t>(items);
   uint32_t* slab_base = cv.take<uint32_t>(items);
+  uint32_t* desc = cv.take<uint32_t>((size_t)items * 18);
   unsigned long long* scan_state = cv.take<unsigned long long>(scan_state_words(items));
   // one word for the big-pool counter, then the mid masks: zeroed by one memset
   const size_t state_bytes = 8 + (size_t)h->n_mid_sms * 4;
@@ -272,6 +273,7 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   cl.slab = slab;
   cl.counts = counts;
   cl.slab_base = slab_base;
+  cl.desc = desc;
   cl.status = oc->status;
   cl.big_ctr = reinterpret_cast<uint32_t*>(state);
   cl.mid_mask = reinterpret_cast<uint32_t*>(state + 1);
@@ -282,7 +284,7 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   cl.with_checksum = oc->checksum != nullptr;
   const bool big_layers = h->sp_words_per_layer > 192;  // the larger shared-memory instance keeps such layers on chip
   if ((err = launch_cluster(cl, big_layers, stream)) != cudaSuccess) return fail(h, ALLEN_VELO_ERR_CUDA, "cluster kernel", err);
-  h->last_launches++;
+  h->last_launches += 2;  // prepare + cluster
   mark(1);
 
   if ((err = launch_scan_u32(counts, oc->layer_offsets, items, scan_state, oc->event_offsets, L, stream)) != cudaSuccess)

@@ -34,6 +34,7 @@ namespace velo {
 namespace {
 
 constexpr int kWarps = 4;  // warps per CTA (independent work items)
+constexpr uint32_t kDescWords = 18;  // per (event, layer) descriptor written by velo_prepare_kernel
 // per-warp shared memory
 // kCap SP words / clusters / edges per layer, 2 * kCap hash slots; two instances: 256 (nu ~ 6) and 512 (busier batches)
 template <uint32_t kCap>
@@ -334,10 +335,7 @@ __device__ __forceinline__ void finish_layer(const ClusterLaunch& a, const Clust
                                              uint32_t item, uint32_t slab0, uint32_t n_cl) {
   const DeviceGeometry& g = a.geo;
   const uint32_t lane = lane_id();
-  if (lane == 0) {
-    a.counts[item] = n_cl;
-    a.slab_base[item] = slab0;
-  }
+  if (lane == 0) a.counts[item] = n_cl;  // slab_base[item] = slab0 was written by velo_prepare_kernel
   if (n_cl == 0) return;
 #pragma unroll 1
   for (uint32_t s = lane; s < 256; s += 32) ss.cnt256[s] = 0;
@@ -479,52 +477,25 @@ __global__ void __launch_bounds__(kWarps * 32) velo_cluster_kernel(const __grid_
   ss.order = ss.tmp + kCapCl;
   ss.phis = ss.order + kCapCl;
 
-  // ---------------- A1: header, bank table (raw format v1, R1) ----------------
-  const uint32_t byte0 = __ldg(a.event_offsets + e), byte1 = __ldg(a.event_offsets + e + 1);
-  const uint32_t* ev = a.raw + (byte0 >> 2);
-  bool bad = byte1 < byte0 || (byte1 - byte0) < 16 || ((byte1 - byte0) & 15u) || (byte0 & 15u);
-  uint32_t n_sp_total = 0;
-  if (!bad) {
-    const uint32_t n_words = (byte1 - byte0) >> 2;
-    bad = __ldg(ev) != kMagic || __ldg(ev + 1) != g.n_sensors;
-    n_sp_total = __ldg(ev + 2);
-    const unsigned long long need = 4ull + g.table_words + (((unsigned long long)n_sp_total + 3ull) & ~3ull);
-    bad = bad || need != n_words;
-  }
-  const uint32_t* tbl = ev + 4;
-  uint32_t before = 0;  // SP words of this event in layers below `layer` (slab placement)
-  if (!bad) {
-#pragma unroll 1
-    for (uint32_t j = lane; j < g.n_sensors; j += 32) {
-      const uint32_t o0 = __ldg(tbl + j), o1 = __ldg(tbl + j + 1);
-      bad = bad || o0 > o1 || (j == 0 && o0 != 0) || (j + 1 == g.n_sensors && o1 != n_sp_total);
-      if (__ldg(g.sensor_layer + j) < layer) before += o1 - o0;
-    }
-  }
-  bad = __any_sync(kFull, bad);
-  if (bad) {
-    if (lane == 0 && layer == 0) atomicOr(a.status + e, ALLEN_VELO_STATUS_BAD_HEADER);
+  // ---------------- A1: the layer's bank ranges, validated and laid out by velo_prepare_kernel ----------------
+  const uint32_t* d = a.desc + (size_t)item * kDescWords;
+  const uint32_t dv = lane < kDescWords ? __ldg(d + lane) : 0u;
+  const uint32_t my_off = dv;                                        // lanes 0..7: first SP word (index into raw)
+  const uint32_t my_cnt = __shfl_sync(kFull, dv, (lane & 7u) + 8u);  // lanes 0..7: SP words of sensor k
+  const uint32_t slab0 = __shfl_sync(kFull, dv, 16);
+  if (__shfl_sync(kFull, dv, 17) & 1u) {  // malformed event (BAD_HEADER set by the prepare kernel): no clusters
     finish_layer<kChecksum>(a, cs, ss, item, 0, 0);
     return;
   }
-  before = __reduce_add_sync(kFull, before);
-  const uint32_t* spw = tbl + g.table_words;
-  // two slab entries per SP word (a super-pixel holds at most two clusters), placed by the raw position of the layer
-  const uint32_t slab0 = 2u * ((byte0 >> 2) + 4u + g.table_words + before);
-
-  // sensors of this layer: lane k < K holds sensor k's bank range
+  const uint32_t* spw = a.raw;
   const uint32_t K = __ldg(g.layer_n_sensors + layer);
-  uint32_t my_sensor = 0, my_off = 0, my_cnt = 0;
-  if (lane < K) {
-    my_sensor = __ldg(g.layer_sensors + layer * kMaxSensorsPerLayer + lane);
-    my_off = __ldg(tbl + my_sensor);
-    my_cnt = __ldg(tbl + my_sensor + 1) - my_off;
-  }
-  const uint32_t n_sp_layer = __reduce_add_sync(kFull, my_cnt);
-  const uint32_t max_cnt = __reduce_max_sync(kFull, my_cnt);
+  const uint32_t my_sensor = lane < K ? __ldg(g.layer_sensors + layer * kMaxSensorsPerLayer + lane) : 0u;
+  const uint32_t cnt_k = lane < K ? my_cnt : 0u;
+  const uint32_t n_sp_layer = __reduce_add_sync(kFull, cnt_k);
+  const uint32_t max_cnt = __reduce_max_sync(kFull, cnt_k);
   if ((unsigned long long)slab0 + 2ull * n_sp_layer > a.slab.capacity) {  // workspace smaller than workspace_bytes()
     if (lane == 0) atomicOr(a.status + e, ALLEN_VELO_STATUS_STAGE_OVERFLOW);
-    finish_layer<kChecksum>(a, cs, ss, item, slab0, 0);
+    finish_layer<kChecksum>(a, cs, ss, item, 0, 0);
     return;
   }
 
@@ -536,7 +507,7 @@ __global__ void __launch_bounds__(kWarps * 32) velo_cluster_kernel(const __grid_
   bool bad_sp = false, overflow = false;
   int mode = n_sp_layer <= kCapSp ? 0 : (max_cnt <= kCapSp && n_sp_layer <= kMidCl) ? 1 : 2;
   if (mode == 0) {
-    if (ccl_pass<kChecksum>(fast, cs, g, spw, my_sensor, my_off, my_cnt, 0, K, n_cl, bad_sp, &ws.n_edges)) {
+    if (ccl_pass<kChecksum>(fast, cs, g, spw, my_sensor, my_off, cnt_k, 0, K, n_cl, bad_sp, &ws.n_edges)) {
       if (__any_sync(kFull, bad_sp) && lane == 0) atomicOr(a.status + e, ALLEN_VELO_STATUS_BAD_SP);
       finish_layer<kChecksum>(a, cs, ss, item, slab0, n_cl);
       return;
@@ -576,12 +547,12 @@ __global__ void __launch_bounds__(kWarps * 32) velo_cluster_kernel(const __grid_
         uint32_t k1 = k0, sum = 0;
 #pragma unroll 1
         while (k1 < K) {
-          const uint32_t cnt = __shfl_sync(kFull, my_cnt, k1);
+          const uint32_t cnt = __shfl_sync(kFull, cnt_k, k1);
           if (sum + cnt > kCapSp) break;
           sum += cnt;
           ++k1;
         }
-        ok = ccl_pass_generic<kChecksum>(fast, cs, g, spw, my_sensor, my_off, my_cnt, k0, k1, n_cl, bad_sp, &ws.n_edges);
+        ok = ccl_pass_generic<kChecksum>(fast, cs, g, spw, my_sensor, my_off, cnt_k, k0, k1, n_cl, bad_sp, &ws.n_edges);
         k0 = k1;
       }
       if (!ok) mode = 2;
@@ -604,7 +575,7 @@ __global__ void __launch_bounds__(kWarps * 32) velo_cluster_kernel(const __grid_
       stores_at(base, BigSlot::kStats, BigSlot::kCnt, BigSlot::kSort, kBigCl, cs, ss);
       n_cl = 0;
       bad_sp = false;
-      overflow = !ccl_pass_generic<kChecksum>(big, cs, g, spw, my_sensor, my_off, my_cnt, 0, K, n_cl, bad_sp,
+      overflow = !ccl_pass_generic<kChecksum>(big, cs, g, spw, my_sensor, my_off, cnt_k, 0, K, n_cl, bad_sp,
                                               reinterpret_cast<uint32_t*>(base + BigSlot::kCtr));
     }
   }
@@ -617,6 +588,74 @@ __global__ void __launch_bounds__(kWarps * 32) velo_cluster_kernel(const __grid_
   finish_layer_generic<kChecksum>(a, cs, ss, item, slab0, n_cl);
   __syncwarp();
   if (held != 0xFFFFFFFFu && lane == 0) atomicAnd(a.mid_mask + (held >> 5), ~(1u << (held & 31u)));
+}
+
+
+// One warp per event: validate header and bank table once (R1), and lay out for every layer of the event what its
+// cluster warp needs: desc[item] = { first SP word of each of its sensors (index into raw) [8], SP words of each [8],
+// slab base, flags (bit 0: malformed event) }.  26 warps per event used to redo this validation each.
+__global__ void __launch_bounds__(128) velo_prepare_kernel(const __grid_constant__ ClusterLaunch a) {
+  const DeviceGeometry& g = a.geo;
+  const uint32_t lane = lane_id(), L = g.n_layers;
+  const uint32_t e = blockIdx.x * 4 + (threadIdx.x >> 5);
+  if (e >= a.n_events) return;
+  const uint32_t byte0 = __ldg(a.event_offsets + e), byte1 = __ldg(a.event_offsets + e + 1);
+  const uint32_t* ev = a.raw + (byte0 >> 2);
+  bool bad = byte1 < byte0 || (byte1 - byte0) < 16 || ((byte1 - byte0) & 15u) || (byte0 & 15u);
+  uint32_t n_sp_total = 0;
+  if (!bad) {
+    const uint32_t n_words = (byte1 - byte0) >> 2;
+    bad = __ldg(ev) != kMagic || __ldg(ev + 1) != g.n_sensors;
+    n_sp_total = __ldg(ev + 2);
+    const unsigned long long need = 4ull + g.table_words + (((unsigned long long)n_sp_total + 3ull) & ~3ull);
+    bad = bad || need != n_words;
+  }
+  const uint32_t* tbl = ev + 4;
+  if (!bad) {
+#pragma unroll 1
+    for (uint32_t j = lane; j < g.n_sensors; j += 32) {
+      const uint32_t o0 = __ldg(tbl + j), o1 = __ldg(tbl + j + 1);
+      bad = bad || o0 > o1 || (j == 0 && o0 != 0) || (j + 1 == g.n_sensors && o1 != n_sp_total);
+    }
+  }
+  bad = __any_sync(kFull, bad);
+  if (bad && lane == 0) atomicOr(a.status + e, ALLEN_VELO_STATUS_BAD_HEADER);
+  const uint32_t words0 = (byte0 >> 2) + 4u + g.table_words;  // first SP word of the event in raw
+  uint32_t carry = 0;                                          // SP words of the layers handled in earlier rounds
+#pragma unroll 1
+  for (uint32_t l0 = 0; l0 < L; l0 += 32) {
+    const uint32_t l = l0 + lane;
+    uint32_t off[kMaxSensorsPerLayer], cnt[kMaxSensorsPerLayer], total = 0;
+    const uint32_t K = (l < L && !bad) ? __ldg(g.layer_n_sensors + l) : 0u;
+#pragma unroll
+    for (int k = 0; k < kMaxSensorsPerLayer; ++k) {
+      off[k] = 0; cnt[k] = 0;
+      if ((uint32_t)k < K) {
+        const uint32_t sns = __ldg(g.layer_sensors + l * kMaxSensorsPerLayer + k);
+        const uint32_t o0 = __ldg(tbl + sns), o1 = __ldg(tbl + sns + 1);
+        off[k] = words0 + o0; cnt[k] = o1 - o0; total += o1 - o0;
+      }
+    }
+    uint32_t incl = total;
+#pragma unroll
+    for (int dd = 1; dd < 32; dd <<= 1) {
+      const uint32_t t = __shfl_up_sync(kFull, incl, dd);
+      if (lane >= (uint32_t)dd) incl += t;
+    }
+    const uint32_t before = carry + incl - total;  // SP words of this event in the layers below l
+    carry += __shfl_sync(kFull, incl, 31);
+    if (l < L) {
+      const uint32_t item = e * L + l;
+      // two slab entries per SP word (a super-pixel holds at most two clusters), placed by the raw position
+      const uint32_t slab0 = bad ? 0u : 2u * (words0 + before);
+      uint32_t* d = a.desc + (size_t)item * kDescWords;
+#pragma unroll
+      for (int k = 0; k < kMaxSensorsPerLayer; ++k) { d[k] = off[k]; d[8 + k] = cnt[k]; }
+      d[16] = slab0;
+      d[17] = bad ? 1u : 0u;
+      a.slab_base[item] = slab0;
+    }
+  }
 }
 
 }  // namespace
@@ -639,6 +678,9 @@ cudaError_t launch_cluster_instance(const ClusterLaunch& a, uint32_t grid, cudaS
 cudaError_t launch_cluster(const ClusterLaunch& a, bool big_layers, cudaStream_t stream) {
   const uint32_t items = a.n_events * a.geo.n_layers;
   if (items == 0) return cudaSuccess;
+  velo_prepare_kernel<<<(a.n_events + 3) / 4, 128, 0, stream>>>(a);
+  cudaError_t perr = cudaGetLastError();
+  if (perr != cudaSuccess) return perr;
   const uint32_t grid = (items + kWarps - 1) / kWarps;
   if (a.with_checksum)
     return big_layers ? launch_cluster_instance<true, 512>(a, grid, stream) : launch_cluster_instance<true, 256>(a, grid, stream);

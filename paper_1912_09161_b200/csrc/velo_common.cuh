@@ -110,6 +110,7 @@ struct ClusterLaunch {
   ClusterSlab slab;
   uint32_t* counts;           // [n_events*n_layers] clusters per (event, layer)
   uint32_t* slab_base;        // [n_events*n_layers] first slab entry of the (event, layer) region
+  uint32_t* desc;             // [n_events*n_layers][18] bank ranges of the layer (velo_prepare_kernel)
   uint32_t* status;           // [n_events], zeroed before
   uint32_t* big_ctr;          // slots handed out of the big pool, zeroed before
   uint32_t* mid_mask;         // [n_mid_sms] busy bits of the mid slots of every SM, zeroed before
