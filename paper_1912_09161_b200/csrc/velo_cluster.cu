@@ -39,7 +39,6 @@ constexpr uint32_t kDescWords = 18;  // per (event, layer) descriptor written by
 // kCap SP words / clusters / edges per layer, 2 * kCap hash slots; two instances: 256 (nu ~ 6) and 512 (busier batches)
 template <uint32_t kCap>
 struct Caps {
-  static constexpr uint32_t kCapSp = kCap, kCapEdges = kCap, kCapCl = kCap;
   static constexpr uint32_t kHashBits = kCap == 256 ? 9 : 10;
   static_assert(kCap == 256 || kCap == 512, "hash bits");
 };

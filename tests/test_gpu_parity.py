@@ -252,3 +252,73 @@ def test_streamed_host_to_host_reconstruction(geometry, oracle_of):
         assert np.allclose(g["tx"], rt.tx[t0:t1], rtol=1e-5, atol=1e-8)
         assert not g["status"].any()
     assert sum(i["n_tracks"] for i in infos) == int(rt.event_offsets[-1])
+
+
+def test_full_size_batch_in_the_bench_configuration(geometry):
+    """BASELINE.json configs[2] at full size (10 000 events, nu = 6), buffers sized as bench.py sizes them, no checksum
+    array: properties that hold at any size for the whole batch, and element-wise parity with the oracle on a sample of
+    events spread over the batch (events are independent: the oracle run on the selected events alone gives
+    their per-event results)."""
+    import oracle
+    import torch
+
+    from paper_1912_09161_b200 import binding, workload
+
+    batch = workload.generate(2, n_events=10000)
+    n_events, L = batch.n_events, geometry.n_layers
+    raw_bytes, n_sp = int(batch.raw.size), batch.n_sp_words()
+    velo = binding.AllenVelo(geometry)
+    ccap = int(1.15 * n_sp) + 4096
+    oc, ot = binding.alloc_outputs(n_events, L, ccap, ccap // 3, ccap // 2, "cuda:0", with_checksum=False)
+    ws = torch.empty(velo.workspace_bytes(n_events, raw_bytes), dtype=torch.uint8, device="cuda:0")
+    velo.set_workspace(ws)
+    velo.set_occupancy_hint(n_events, raw_bytes)
+    d_raw = torch.from_numpy(batch.raw).to("cuda:0")
+    d_off = torch.from_numpy(batch.event_offsets.view(np.int32)).to("cuda:0")
+    for _ in range(2):  # the second call reuses workspace and outputs, as the timed steps do
+        assert velo.reconstruct(d_raw, d_off, n_events, None, oc, ot) == 0, velo.last_error()
+    torch.cuda.synchronize()
+    u32 = lambda t: t.cpu().numpy().view(np.uint32)
+    ce, lo, te = u32(oc.event_offsets), u32(oc.layer_offsets), u32(ot.event_offsets)
+    assert not u32(oc.status)[:n_events].any()
+    nc, nt = int(ce[n_events]), int(te[n_events])
+    ho = u32(ot.hit_offsets)[:nt + 1]
+    hits = ot.hits.cpu().numpy().view(np.uint16)[:int(ho[-1])]
+    key, phi = u32(oc.key)[:nc], oc.phi16.cpu().numpy()[:nc]
+    # -- whole batch: offsets consistent and monotone, clusters sorted by (phi16, key) inside every layer
+    assert ce[0] == 0 and lo[0] == 0 and np.all(np.diff(lo.astype(np.int64)) >= 0) and np.all(np.diff(ho.astype(np.int64)) >= 3)
+    assert np.array_equal(lo[::L][:n_events + 1], ce) and lo[-1] == nc
+    layer_of = np.repeat(np.arange(n_events * L), np.diff(lo))
+    same = layer_of[1:] == layer_of[:-1]
+    k64 = ((phi.astype(np.int64) + 32768) << 32) | key
+    assert np.all(k64[1:][same] > k64[:-1][same])
+    # -- whole batch: every hit index inside its event, every hit in at most one track
+    ev_of_track = np.repeat(np.arange(n_events), np.diff(te))
+    ev_of_hit = np.repeat(ev_of_track, np.diff(ho))
+    assert np.all(hits < (ce[1:] - ce[:-1])[ev_of_hit])
+    glob = ce[ev_of_hit].astype(np.int64) + hits
+    assert len(np.unique(glob)) == len(glob)
+    # -- sampled events against the oracle, element by element
+    sample = np.unique(np.concatenate([np.arange(0, n_events, 157), [n_events - 1],
+                                       np.argsort(np.diff(ce.astype(np.int64)))[-8:]]))  # incl. the 8 busiest events
+    sub = batch.select(sample)
+    ref = oracle.reconstruct(geometry, sub.raw, sub.event_offsets, n_threads=8)
+    x, y, z = (t.cpu().numpy()[:nc] for t in (oc.x, oc.y, oc.z))
+    npx, sc, sr = u32(oc.n_pixels)[:nc], u32(oc.sum_col)[:nc], u32(oc.sum_row)[:nc]
+    fit = [t.cpu().numpy()[:nt] for t in (ot.x0, ot.y0, ot.tx, ot.ty)]
+    rc, rt = ref.clusters, ref.tracks
+    for j, e in enumerate(sample):
+        a0, a1, b0, b1 = int(ce[e]), int(ce[e + 1]), int(rc.event_offsets[j]), int(rc.event_offsets[j + 1])
+        assert a1 - a0 == b1 - b0, e
+        assert np.array_equal(lo[e * L:(e + 1) * L + 1] - a0, rc.layer_offsets[j * L:(j + 1) * L + 1] - b0), e
+        for got, want in ((key, rc.key), (npx, rc.n_pixels), (sc, rc.sum_col), (sr, rc.sum_row), (phi, rc.phi16)):
+            assert np.array_equal(got[a0:a1], want[b0:b1]), e
+        for got, want in ((x, rc.x), (y, rc.y), (z, rc.z)):
+            assert np.array_equal(got[a0:a1].view(np.uint32), want[b0:b1].view(np.uint32)), e
+        t0, t1, r0, r1 = int(te[e]), int(te[e + 1]), int(rt.event_offsets[j]), int(rt.event_offsets[j + 1])
+        assert t1 - t0 == r1 - r0, e
+        assert np.array_equal(ho[t0:t1 + 1] - ho[t0], rt.hit_offsets[r0:r1 + 1] - rt.hit_offsets[r0]), e
+        assert np.array_equal(hits[ho[t0]:ho[t1]], rt.hits[rt.hit_offsets[r0]:rt.hit_offsets[r1]]), e
+        for got, want in zip(fit, (rt.x0, rt.y0, rt.tx, rt.ty)):
+            assert np.allclose(got[t0:t1], want[r0:r1], rtol=1e-5, atol=1e-5), e
+    velo.destroy()
