@@ -68,7 +68,8 @@ size_t fixed_bytes(uint32_t n_events, uint32_t n_layers, uint32_t n_mid_sms) {
   b += align_up((size_t)n_events * 8) + align_up(((size_t)n_events + 1) * 8);  // track counts, offsets
   b += align_up(scan_state_words(n_events) * 8);                  // scan state (tracks)
   b += align_up(n_events);                                        // class of every event
-  b += align_up((size_t)n_events * 4) * 4 + align_up(8 * 4);      // event lists of the larger instances, counters
+  b += align_up((size_t)n_events * 4) * 4 + align_up(12 * 4);     // event lists of the larger instances, counters
+  b += align_up((size_t)n_events * 16);                           // size-binned event order of the first instance
   return b + 16 * kAlign;
 }
 
@@ -235,7 +236,8 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   uint8_t* trk_level = cv.take<uint8_t>(n_events);
   uint32_t* trk_lists[4];
   for (uint32_t*& p : trk_lists) p = cv.take<uint32_t>(n_events);
-  uint32_t* trk_counters = cv.take<uint32_t>(8);
+  uint32_t* trk_counters = cv.take<uint32_t>(12);
+  uint32_t* trk_order = cv.take<uint32_t>((size_t)n_events * 4);
   size_t entries = (h->ws_bytes - cv.used - 16 * kAlign) / per_entry_bytes();
   if (entries > 0x7FFFFFF0u) entries = 0x7FFFFFF0u;
   ClusterSlab slab{};
@@ -308,6 +310,7 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   tl.ev_list[0] = trk_lists[0]; tl.ev_list[1] = trk_lists[1];
   tl.redo_list[0] = trk_lists[2]; tl.redo_list[1] = trk_lists[3];
   tl.counters = trk_counters;
+  tl.order = trk_order;
   uint32_t n_track_launches = 0;
   if ((err = launch_track(tl, stream, h->side, h->fork_join, h->n_sms, &n_track_launches)) != cudaSuccess) return fail(h, ALLEN_VELO_ERR_CUDA, "track kernel", err);
   h->last_launches += n_track_launches;

@@ -148,7 +148,8 @@ struct TrackLaunch {
   uint8_t* level;                  // [n_events] class of the event: searching instance 0..2, 254 copy only, 255 nothing
   uint32_t* ev_list[2];            // [n_events] each: events of level 1 / 2
   uint32_t* redo_list[2];          // [n_events] each: events level 0 / 1 ran out of track slots on (second pass)
-  uint32_t* counters;              // [8] list sizes and cursors, zeroed by the launcher
+  uint32_t* order;                 // [4][n_events] events of the first instance by size bin
+  uint32_t* counters;              // [12] list sizes and cursors, zeroed by the launcher
 };
 cudaError_t launch_track(const TrackLaunch& a, cudaStream_t stream, cudaStream_t* side, cudaEvent_t* ev,
                          uint32_t n_sms, uint32_t* n_launches);

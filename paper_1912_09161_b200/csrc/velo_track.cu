@@ -586,7 +586,9 @@ __global__ void __launch_bounds__(128) compact_tracks_kernel(const CompactTracks
 }
 
 // One thread per event: class of the event (which instance searches it, or copy only / nothing) and the event lists
-// of the two larger instances.  counters: [0], [1] events of level 1, 2; [2], [3] second-pass events; [4..7] cursors.
+// of the two larger instances.  counters: [0], [1] events of level 1, 2; [2], [3] second-pass events; [4..7] cursors;
+// [8..11] events of the first instance (and copy-only events) in four size bins: it takes them largest first, so that
+// the last CTAs of the grid are short ones.
 __global__ void __launch_bounds__(256) classify_events_kernel(const __grid_constant__ TrackLaunch a) {
   const uint32_t e = blockIdx.x * blockDim.x + threadIdx.x;
   if (e >= a.n_events) return;
@@ -622,6 +624,11 @@ __global__ void __launch_bounds__(256) classify_events_kernel(const __grid_const
     }
     if (cls == 1 || cls == 2) a.ev_list[cls - 1][atomicAdd(a.counters + (cls - 1), 1u)] = e;
   }
+  if (cls == 0 || cls == kClsCopy) {
+    const uint32_t avg = a.clusters.event_offsets[a.n_events] / a.n_events + 1u;
+    const uint32_t bin = cls == kClsCopy ? 3u : 20u * n_cl >= 30u * avg ? 0u : 20u * n_cl >= 23u * avg ? 1u : 20u * n_cl >= 17u * avg ? 2u : 3u;
+    a.order[(size_t)bin * a.n_events + atomicAdd(a.counters + 8 + bin, 1u)] = e;
+  }
   a.level[e] = cls;
   if (cls >= kClsCopy) a.counts[e] = 0;
 }
@@ -631,7 +638,15 @@ template <class C>
 __global__ void __launch_bounds__(C::kBlock) velo_track_kernel(const __grid_constant__ TrackLaunch a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   Smem<C>& sm = *reinterpret_cast<Smem<C>*>(smem_raw);
-  const uint32_t e = blockIdx.x;
+  uint32_t j = blockIdx.x, bin = 0;  // events in four size bins, largest first
+#pragma unroll 1
+  for (; bin < 4; ++bin) {
+    const uint32_t n = a.counters[8 + bin];
+    if (j < n) break;
+    j -= n;
+  }
+  if (bin == 4) return;
+  const uint32_t e = a.order[(size_t)bin * a.n_events + j];
   const uint8_t cls = a.level[e];
   if (cls == kClsCopy) {
     const uint32_t co = a.clusters.event_offsets[e], L = a.geo.n_layers;
@@ -687,7 +702,7 @@ cudaError_t launch_track(const TrackLaunch& a, cudaStream_t stream, cudaStream_t
                          uint32_t n_sms, uint32_t* n_launches) {
   *n_launches = 0;
   if (a.n_events == 0) return cudaSuccess;
-  cudaError_t err = cudaMemsetAsync(a.counters, 0, 8 * sizeof(uint32_t), stream);
+  cudaError_t err = cudaMemsetAsync(a.counters, 0, 12 * sizeof(uint32_t), stream);
   if (err != cudaSuccess) return err;
   classify_events_kernel<<<(a.n_events + 255) / 256, 256, 0, stream>>>(a);
   if ((err = cudaGetLastError()) != cudaSuccess) return err;
