@@ -61,6 +61,7 @@ def lib():
         L.oracle_scatter.restype = ctypes.c_float
         L.oracle_scatter.argtypes = [ctypes.c_void_p] * 3
         L.oracle_fit.argtypes = [ctypes.c_uint32] + [ctypes.c_void_p] * 4
+        L.oracle_kalman.argtypes = [ctypes.c_uint32] + [ctypes.c_void_p] * 5 + [ctypes.c_double, ctypes.c_void_p]
         L.oracle_run.restype = ctypes.c_void_p
         L.oracle_run.argtypes = [ctypes.POINTER(_Geometry), ctypes.c_void_p, ctypes.c_void_p, ctypes.c_uint32,
                                  ctypes.c_uint32]
@@ -214,3 +215,24 @@ def fit(x, y, z) -> np.ndarray:
     out = np.zeros(4, np.float32)
     lib().oracle_fit(len(x), _p(x), _p(y), _p(z), _p(out))
     return out
+
+
+def kalman(hit_offsets, abs_hits, x, y, z, pitch: float) -> np.ndarray:
+    """O7 (R9): simple Kalman fit of every track; hits are indices into x, y, z, in order of addition.
+    Returns [n_tracks, 12] float64: x, y, tx, ty, z, chi2, C00x, C01x, C11x, C00y, C01y, C11y at the last hit."""
+    ho = np.ascontiguousarray(hit_offsets, np.uint32)
+    hits = np.ascontiguousarray(abs_hits, np.uint32)
+    x, y, z = (np.ascontiguousarray(a, np.float32) for a in (x, y, z))
+    out = np.zeros((len(ho) - 1, 12), np.float64)
+    lib().oracle_kalman(len(ho) - 1, _p(ho), _p(hits), _p(x), _p(y), _p(z), float(pitch), _p(out))
+    return out
+
+
+def kalman_of(result: "Result", pitch: float) -> np.ndarray:
+    """O7 for every track of an oracle.Result (event-local hit indices resolved to absolute cluster indices)."""
+    t, c = result.tracks, result.clusters
+    n_per_event = np.diff(t.event_offsets.astype(np.int64))
+    ev_of_track = np.repeat(np.arange(len(n_per_event)), n_per_event)
+    ev_of_hit = np.repeat(ev_of_track, np.diff(t.hit_offsets.astype(np.int64)))
+    abs_hits = c.event_offsets[ev_of_hit].astype(np.int64) + t.hits
+    return kalman(t.hit_offsets, abs_hits, c.x, c.y, c.z, pitch)

@@ -15,6 +15,8 @@
 //   O5 search by triplet P:181-183 "seeds of three hits from consecutive layers ... extending these to the other
 //                        layers" (D:R5 step-by-step reading T1..T5)
 //   O6 straight-line fit P:149 "tracks in the Velo detector form straight lines" -> unweighted LSQ (D:R6)
+//   O7 simple Kalman fit P:185 "simple Kalman filter ... x- and y-components are independent ... constant average
+//                        transverse momentum of 400 MeV ... noise contribution from multiple scattering" (D:R9)
 //
 // Build: g++ -O2 -std=c++17 -ffp-contract=off (no fast-math) -shared -fPIC -pthread.
 #include <algorithm>
@@ -454,6 +456,50 @@ void fit_line(const std::vector<Hit>& hits, Track& T) {
   T.y0 = (float)(ym - ty * zm);
 }
 
+// ------------------------------------------------------------------------------------------------
+// O7: simple Kalman filter over the hits of a track in the order they were added (downstream -> upstream), x and y
+// independent, state (pos, slope) per projection (D:R9 step by step).  fp64 from the fp32 hit coordinates.
+//   measurement variance  var_m = pitch^2 / 12
+//   scattering per plane  theta0^2 = (13.6 MeV / p)^2 * X,  p = pT / sin(theta),  pT = 400 MeV,  X = 0.02;
+//                         sin^2(theta) = (tx^2 + ty^2) / (1 + tx^2 + ty^2) with the slopes of the first two hits;
+//                         q_x = theta0^2 (1 + tx^2)(1 + tx^2 + ty^2), q_y likewise with ty
+//   start at hit 0:       pos = measured, slope = 0, C = diag(var_m, 1)
+//   for hit k = 1..n-1:   C11 += q; propagate by dz = z_k - z_{k-1}; update with the measured position
+// out12 = x, y, tx, ty, z (of the last hit), chi2 (x + y), C00x, C01x, C11x, C00y, C01y, C11y.
+// ------------------------------------------------------------------------------------------------
+void kalman_track(uint32_t n, const float* x, const float* y, const float* z, double pitch, double* out12) {
+  const double var_m = pitch * pitch / 12.0;
+  const double tx0 = ((double)x[1] - x[0]) / ((double)z[1] - z[0]);
+  const double ty0 = ((double)y[1] - y[0]) / ((double)z[1] - z[0]);
+  const double t2 = tx0 * tx0 + ty0 * ty0;
+  const double theta02 = (13.6 / 400.0) * (13.6 / 400.0) * 0.02 * t2 / (1.0 + t2);
+  const double q[2] = {theta02 * (1.0 + tx0 * tx0) * (1.0 + t2), theta02 * (1.0 + ty0 * ty0) * (1.0 + t2)};
+  const float* m[2] = {x, y};
+  double chi2 = 0;
+  for (int pr = 0; pr < 2; ++pr) {
+    double pos = m[pr][0], slope = 0, c00 = var_m, c01 = 0, c11 = 1.0;
+    for (uint32_t k = 1; k < n; ++k) {
+      const double dz = (double)z[k] - z[k - 1];
+      c11 += q[pr];                                // scattering in the plane just left
+      pos += slope * dz;                           // straight-line propagation
+      c00 += 2.0 * dz * c01 + dz * dz * c11;
+      c01 += dz * c11;
+      const double r = m[pr][k] - pos, S = c00 + var_m;
+      const double k0 = c00 / S, k1 = c01 / S;     // gain
+      pos += k0 * r;
+      slope += k1 * r;
+      c11 -= k1 * c01;
+      c01 -= k0 * c01;
+      c00 -= k0 * c00;
+      chi2 += r * r / S;
+    }
+    out12[pr] = pos; out12[2 + pr] = slope;
+    out12[6 + 3 * pr] = c00; out12[7 + 3 * pr] = c01; out12[8 + 3 * pr] = c11;
+  }
+  out12[4] = z[n - 1];
+  out12[5] = chi2;
+}
+
 void reconstruct_event(const Geometry& g, const uint8_t* raw, size_t bytes, EventResult& out, Scratch& sc) {
   cluster_event(g, raw, bytes, out, sc);
   if (out.status & (STATUS_BAD_HEADER | STATUS_TOO_MANY_CLUSTERS)) return;
@@ -489,6 +535,21 @@ void oracle_fit(uint32_t n, const float* x, const float* y, const float* z, floa
   for (uint32_t i = 0; i < n; ++i) { hits[i] = {x[i], y[i], z[i], 0}; T.hits.push_back(i); }
   fit_line(hits, T);
   out4[0] = T.x0; out4[1] = T.y0; out4[2] = T.tx; out4[3] = T.ty;
+}
+
+// O7 for a batch of tracks: track t has hits abs_hits[hit_offsets[t] .. hit_offsets[t+1]) (indices into x, y, z).
+void oracle_kalman(uint32_t n_tracks, const uint32_t* hit_offsets, const uint32_t* abs_hits, const float* x,
+                   const float* y, const float* z, double pitch, double* out12) {
+  std::vector<float> hx, hy, hz;
+  for (uint32_t t = 0; t < n_tracks; ++t) {
+    const uint32_t n = hit_offsets[t + 1] - hit_offsets[t];
+    hx.resize(n); hy.resize(n); hz.resize(n);
+    for (uint32_t k = 0; k < n; ++k) {
+      const uint32_t h = abs_hits[hit_offsets[t] + k];
+      hx[k] = x[h]; hy[k] = y[h]; hz[k] = z[h];
+    }
+    kalman_track(n, hx.data(), hy.data(), hz.data(), pitch, out12 + 12 * (size_t)t);
+  }
 }
 
 void* oracle_run(const Geometry* g, const uint8_t* raw, const uint32_t* event_offsets, uint32_t n_events,
