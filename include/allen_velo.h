@@ -95,6 +95,9 @@ typedef struct {
   float* y0;
   float* tx;
   float* ty;
+  float* kalman;           /* DEVICE [capacity_tracks][12] or NULL: simple Kalman fit (R9) at the track's last hit
+                              (the most upstream one): x, y, tx, ty, z, chi2, then the covariances C00, C01, C11 of
+                              (position, slope) for x and for y */
 } allen_velo_tracks_t;
 
 typedef struct allen_velo allen_velo_t;

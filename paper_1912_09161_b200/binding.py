@@ -40,7 +40,7 @@ class allen_velo_clusters_t(ctypes.Structure):
 
 class allen_velo_tracks_t(ctypes.Structure):
     _fields_ = [("capacity_tracks", ctypes.c_uint32), ("capacity_hits", ctypes.c_uint32)] + [
-        (n, ctypes.c_void_p) for n in ("event_offsets", "hit_offsets", "hits", "x0", "y0", "tx", "ty")]
+        (n, ctypes.c_void_p) for n in ("event_offsets", "hit_offsets", "hits", "x0", "y0", "tx", "ty", "kalman")]
 
 
 _lib = None
@@ -130,17 +130,19 @@ class TrackBuffers:
     y0: "torch.Tensor"
     tx: "torch.Tensor"
     ty: "torch.Tensor"
+    kalman: "torch.Tensor | None" = None
 
     def struct(self) -> allen_velo_tracks_t:
         s = allen_velo_tracks_t()
         s.capacity_tracks, s.capacity_hits = self.capacity_tracks, self.capacity_hits
         for name in ("event_offsets", "hit_offsets", "hits", "x0", "y0", "tx", "ty"):
             setattr(s, name, getattr(self, name).data_ptr())
+        s.kalman = self.kalman.data_ptr() if self.kalman is not None else None
         return s
 
 
 def alloc_outputs(n_events: int, n_layers: int, cluster_capacity: int, track_capacity: int, hit_capacity: int,
-                  device, with_checksum: bool = True):
+                  device, with_checksum: bool = True, with_kalman: bool = False):
     """Allocate output tensors with torch (device memory only; int32 storage stands for u32, int16 for u16)."""
     import torch
 
@@ -153,7 +155,7 @@ def alloc_outputs(n_events: int, n_layers: int, cluster_capacity: int, track_cap
                        z(cluster_capacity, i32) if with_checksum else None, z(n_events, i32))
     t = TrackBuffers(track_capacity, hit_capacity, z(n_events + 1, i32), z(track_capacity + 1, i32),
                      z(hit_capacity, i16), z(track_capacity, f32), z(track_capacity, f32), z(track_capacity, f32),
-                     z(track_capacity, f32))
+                     z(track_capacity, f32), z(12 * track_capacity, f32) if with_kalman else None)
     return c, t
 
 
@@ -244,7 +246,7 @@ class AllenVelo:
 
 def reconstruct_batch(velo: AllenVelo, raw: np.ndarray, event_offsets: np.ndarray, device="cuda:0",
                       with_checksum: bool = True, cluster_capacity: int | None = None,
-                      track_capacity: int | None = None, hit_capacity: int | None = None):
+                      track_capacity: int | None = None, hit_capacity: int | None = None, with_kalman: bool = False):
     """Convenience for tests/smoke: copy a host batch to the device, run the path once, return host copies.
 
     Host<->device copies and the final synchronise happen here, outside the C ABI.  Returns (clusters, tracks)
@@ -259,7 +261,7 @@ def reconstruct_batch(velo: AllenVelo, raw: np.ndarray, event_offsets: np.ndarra
     ccap = cluster_capacity if cluster_capacity is not None else raw_bytes // 2 + 16  # <= 2 clusters per SP word
     tcap = track_capacity if track_capacity is not None else ccap // 3 + 16
     hcap = hit_capacity if hit_capacity is not None else ccap
-    oc, ot = alloc_outputs(n_events, velo.n_layers, ccap, tcap, hcap, device, with_checksum)
+    oc, ot = alloc_outputs(n_events, velo.n_layers, ccap, tcap, hcap, device, with_checksum, with_kalman)
     ws = torch.empty(velo.workspace_bytes(n_events, raw_bytes), dtype=torch.uint8, device=device)
     velo.set_workspace(ws)
     velo.set_occupancy_hint(n_events, raw_bytes)
@@ -286,6 +288,8 @@ def reconstruct_batch(velo: AllenVelo, raw: np.ndarray, event_offsets: np.ndarra
     tracks = dict(event_offsets=te, hit_offsets=ho, hits=host(ot.hits, u16)[:min(nh, hcap)], n=nt)
     for name in ("x0", "y0", "tx", "ty"):
         tracks[name] = host(getattr(ot, name), np.float32)[:min(nt, tcap)]
+    if with_kalman:
+        tracks["kalman"] = host(ot.kalman, np.float32).reshape(-1, 12)[:min(nt, tcap)]
     return clusters, tracks
 
 

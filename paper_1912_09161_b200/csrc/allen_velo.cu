@@ -323,6 +323,7 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
 
   CompactTracksLaunch ct{};
   ct.n_events = n_events;
+  ct.pitch = h->dev.pitch;
   ct.clusters = *oc;
   ct.hits_slab = hits_slab;
   ct.trk_hitoff = trk_hitoff;

@@ -156,6 +156,7 @@ cudaError_t launch_track(const TrackLaunch& a, cudaStream_t stream, cudaStream_t
 
 struct CompactTracksLaunch {
   uint32_t n_events;
+  float pitch;  // pixel pitch, mm (measurement error of the Kalman fit)
   allen_velo_clusters_t clusters;
   const uint16_t* hits_slab;
   const uint32_t* trk_hitoff;

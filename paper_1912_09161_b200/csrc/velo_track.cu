@@ -582,6 +582,59 @@ __global__ void __launch_bounds__(128) compact_tracks_kernel(const CompactTracks
   }
 #pragma unroll 1
   for (uint32_t k = threadIdx.x; k < nH; k += blockDim.x) a.out.hits[H0 + k] = a.hits_slab[co + k];
+  // ---- simple Kalman fit (R9), one thread per track, x and y independent: start at the first hit
+  //      with (measured position, slope 0), C = diag(var_m, 1); per further hit add the scattering of a 400 MeV pT
+  //      track to C11, propagate, update.  (1 - K0) = var_m / S keeps the covariance update free of cancellation.
+  if (a.out.kalman) {
+    const float* X = a.clusters.x + co;
+    const float* Y = a.clusters.y + co;
+    const float* Z = a.clusters.z + co;
+    const float var_m = a.pitch * a.pitch * (1.0f / 12.0f);
+#pragma unroll 1
+    for (uint32_t t = threadIdx.x; t < nT; t += blockDim.x) {
+      const uint32_t h0 = a.trk_hitoff[trk0 + t], h1 = t + 1 < nT ? a.trk_hitoff[trk0 + t + 1] : nH;
+      const uint16_t* hits = a.hits_slab + co + h0;
+      uint32_t h = hits[0], hn = hits[1];
+      float zp = Z[h];
+      const float dz01 = Z[hn] - zp, tx0 = (X[hn] - X[h]) / dz01, ty0 = (Y[hn] - Y[h]) / dz01;
+      const float t2 = tx0 * tx0 + ty0 * ty0;
+      const float theta02 = (13.6f / 400.0f) * (13.6f / 400.0f) * 0.02f * t2 / (1.0f + t2);
+      const float qx = theta02 * (1.0f + tx0 * tx0) * (1.0f + t2), qy = theta02 * (1.0f + ty0 * ty0) * (1.0f + t2);
+      // Hit 1 in closed form: with the diffuse slope prior (C11 = 1) the generic update subtracts two nearly equal
+      // numbers; for C = [[v + dz^2 P, dz P], [dz P, P]], P = 1 + q, S = 2 v + dz^2 P the posterior is
+      // C00 = (v + dz^2 P) v / S, C01 = dz P v / S, C11 = 2 v P / S, gains K0 = (v + dz^2 P) / S, K1 = dz P / S.
+      float px, sx, ax, bx, cx, py, sy, ay, by, cy, chi2;
+      {
+        const float Px = 1.0f + qx, Py = 1.0f + qy, d2 = dz01 * dz01;
+        const float ix = 1.0f / (2.0f * var_m + d2 * Px), iy = 1.0f / (2.0f * var_m + d2 * Py);
+        const float rx = X[hn] - X[h], ry = Y[hn] - Y[h];
+        px = X[h] + (var_m + d2 * Px) * ix * rx; sx = dz01 * Px * ix * rx;
+        py = Y[h] + (var_m + d2 * Py) * iy * ry; sy = dz01 * Py * iy * ry;
+        ax = (var_m + d2 * Px) * var_m * ix; bx = dz01 * Px * var_m * ix; cx = 2.0f * var_m * Px * ix;
+        ay = (var_m + d2 * Py) * var_m * iy; by = dz01 * Py * var_m * iy; cy = 2.0f * var_m * Py * iy;
+        chi2 = rx * rx * ix + ry * ry * iy;
+        zp = Z[hn];
+      }
+#pragma unroll 1
+      for (uint32_t k = 2; k < h1 - h0; ++k) {
+        h = hits[k];
+        const float z = Z[h], dz = z - zp;
+        zp = z;
+        cx += qx; px += sx * dz; ax += 2.0f * dz * bx + dz * dz * cx; bx += dz * cx;
+        cy += qy; py += sy * dz; ay += 2.0f * dz * by + dz * dz * cy; by += dz * cy;
+        const float rx = X[h] - px, ry = Y[h] - py;
+        const float ix = 1.0f / (ax + var_m), iy = 1.0f / (ay + var_m);
+        px += ax * ix * rx; sx += bx * ix * rx; cx -= bx * bx * ix;
+        py += ay * iy * ry; sy += by * iy * ry; cy -= by * by * iy;
+        bx *= var_m * ix; ax *= var_m * ix;
+        by *= var_m * iy; ay *= var_m * iy;
+        chi2 += rx * rx * ix + ry * ry * iy;
+      }
+      float* o = a.out.kalman + 12 * (size_t)(T0 + t);
+      o[0] = px; o[1] = py; o[2] = sx; o[3] = sy; o[4] = zp; o[5] = chi2;
+      o[6] = ax; o[7] = bx; o[8] = cx; o[9] = ay; o[10] = by; o[11] = cy;
+    }
+  }
   if (threadIdx.x == 0 && e + 1 == a.n_events) a.out.hit_offsets[T0 + nT] = H0 + nH;
 }
 

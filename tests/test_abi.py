@@ -51,7 +51,7 @@ def test_binding_structs_match_the_header_layout():
     assert ctypes.sizeof(binding.allen_velo_params_t) == 28
     assert ctypes.sizeof(binding.allen_velo_geometry_t) == 24 + 3 * 8 + 28 + 4  # padded to 8
     assert ctypes.sizeof(binding.allen_velo_clusters_t) == 8 + 12 * 8
-    assert ctypes.sizeof(binding.allen_velo_tracks_t) == 8 + 7 * 8
+    assert ctypes.sizeof(binding.allen_velo_tracks_t) == 8 + 8 * 8
 
 
 def test_product_path_refuses_to_run_without_cuda(geometry):

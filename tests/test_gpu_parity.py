@@ -322,3 +322,29 @@ def test_full_size_batch_in_the_bench_configuration(geometry):
         for got, want in zip(fit, (rt.x0, rt.y0, rt.tx, rt.ty)):
             assert np.allclose(got[t0:t1], want[r0:r1], rtol=1e-5, atol=1e-5), e
     velo.destroy()
+
+
+@pytest.mark.parametrize("config,n_events", [(0, None), (2, 200), (3, 48)])
+def test_kalman_fit_against_the_oracle(velo, geometry, oracle_of, config, n_events):
+    """Optional output of the track stage: simple Kalman fit (R9), fp32 on the GPU against the fp64
+    oracle.  Tolerances (R9): positions 1e-5 (1 mm + |value|), slopes 1e-5 |slope| + 1e-7, covariances 2e-4
+    relative (fp32 recursion over <= 26 hits); chi2 2e-3 relative + 1e-3: its residuals (~0.01 mm) are differences of
+    fp32 coordinates of up to ~50 mm (ulp 4e-6 mm), so every term carries ~1e-3 relative error."""
+    import oracle
+    from paper_1912_09161_b200 import binding
+
+    batch, ref = oracle_of(config, n_events)
+    clusters, tracks = binding.reconstruct_batch(velo, batch.raw, batch.event_offsets, with_kalman=True)
+    assert np.array_equal(tracks["hits"], ref.tracks.hits)
+    want = oracle.kalman_of(ref, geometry.pitch_mm)
+    got = tracks["kalman"].astype(np.float64)
+    assert got.shape == want.shape and len(want) > 0
+    dev = dict(pos=np.abs(got[:, 0:2] - want[:, 0:2]).max(), slope=(np.abs(got[:, 2:4] - want[:, 2:4]) / (np.abs(want[:, 2:4]) + 1e-3)).max(),
+               chi2=(np.abs(got[:, 5] - want[:, 5]) / (want[:, 5] + 1e-3)).max(),
+               cov=(np.abs(got[:, 6:] - want[:, 6:]) / np.abs(want[:, 6:])).max())
+    print("max deviations", dev)
+    assert np.all(np.abs(got[:, 0:2] - want[:, 0:2]) <= 1e-5 * (1 + np.abs(want[:, 0:2])))
+    assert np.all(np.abs(got[:, 2:4] - want[:, 2:4]) <= 1e-5 * np.abs(want[:, 2:4]) + 1e-7)
+    assert np.array_equal(got[:, 4], want[:, 4])
+    assert np.all(np.abs(got[:, 5] - want[:, 5]) <= 2e-3 * want[:, 5] + 1e-3)
+    assert np.all(np.abs(got[:, 6:] - want[:, 6:]) <= 2e-4 * np.abs(want[:, 6:]))
