@@ -5,9 +5,9 @@
 //
 // One CTA per event ("a single event is assigned to one block, while intra-event parallelism is mapped to the threads
 // within one block").  The L-2 layer iterations are sequential.  Design for sm_100a:
-//  * the three layers of an iteration (plus the one being prefetched) live in shared memory as 16-byte hit records
-//    (x, y, z, phi16 | used << 16) in a ring of four slots: one LDS.128 per candidate; the next layer is brought in
-//    with cp.async one iteration ahead, so its DRAM latency hides behind the current iteration;
+//  * the three layers of an iteration live in shared memory as 16-byte hit records (x, y, z, phi16 | used << 16) in a
+//    ring of three slots: one LDS.128 per candidate; the next layer is brought in with cp.async into the slot of the
+//    layer that leaves, as soon as the seeding is done with it, so its DRAM latency hides behind T4;
 //  * phi look-up uses a 128-bucket start table per layer, built while the layer is staged (no binary search);
 //  * seeding is flattened: S1 lists (b, a) doublets inside the phi window, S2 gives every doublet one thread that
 //    scans b's window on layer C; the per-b argmin is a 64-bit shared-memory atomicMin on (bits(S), a, c);
@@ -70,7 +70,7 @@ constexpr uint8_t kClsCopy = 254;  // clusters are moved to the output, no track
 
 template <class C>
 struct Smem {
-  Hit rec[4][C::kCap];
+  Hit rec[3][C::kCap];
   unsigned long long best[C::kCap];  // T3: per-b argmin key; T1/T2: forward claims on layer C (aliased by phase)
   unsigned long long claimA[C::kCap], claimC[C::kCap];
   uint32_t doublets[C::kCapDoublets];  // b_local | a_local << 16
@@ -78,7 +78,7 @@ struct Smem {
   uint32_t tstate[C::kCapTracks];                // newest << 16 | weak_ok << 15 | nhits << 8 | missed (0xFF: closed)
   uint16_t tseedB[C::kCapTracks];                // track_key: event-local index of the seed's middle hit
   uint16_t fsel[C::kCapTracks];                  // hit of layer C chosen by the track in T1 (0xFFFF: none)
-  uint16_t bucket[4][kBuckets + 2];
+  uint16_t bucket[3][kBuckets + 2];
   uint32_t lo[kMaxLayers + 1];
   uint32_t src[kMaxLayers];  // first entry of every layer in the arrays X, Y, Z, PHI are read from
   uint32_t warp_tot[C::kRoundsB > C::kRoundsT ? C::kRoundsB : C::kRoundsT][C::kWarps];
@@ -118,14 +118,14 @@ struct Ctx {
   allen_velo_params_t P;
 };
 
-// Bring layer `l` into ring slot l & 3: x, y, z by cp.async (4-byte copies into the 16-byte records), the phi word and
+// Bring layer `l` into ring slot l % 3: x, y, z by cp.async (4-byte copies into the 16-byte records), the phi word and
 // the bucket table by this thread.  Completion: __pipeline_wait_prior(0) + __syncthreads() by the caller.
 template <class C>
 __device__ __forceinline__ void stage_layer(const Ctx<C>& c, uint32_t l) {
   Smem<C>& sm = c.sm;
   const uint32_t base = sm.src[l], n = sm.lo[l + 1] - sm.lo[l];
-  Hit* rec = sm.rec[l & 3];
-  uint16_t* bucket = sm.bucket[l & 3];
+  Hit* rec = sm.rec[l % 3];
+  uint16_t* bucket = sm.bucket[l % 3];
   if (n == 0) {
 #pragma unroll 1
     for (uint32_t b = threadIdx.x; b <= (uint32_t)kBuckets; b += C::kThreads) bucket[b] = 0;
@@ -249,15 +249,14 @@ __device__ __forceinline__ void track_event(const TrackLaunch& a, uint32_t e, Sm
   for (int i = (int)L - 1; i >= 2; --i) {
     const uint32_t A0 = sm.lo[i], A1 = sm.lo[i + 1], B0 = sm.lo[i - 1], C0 = sm.lo[i - 2];
     const uint32_t nA = A1 - A0, nB = A0 - B0, nC = B0 - C0;
-    Hit* recA = sm.rec[i & 3];
-    Hit* recB = sm.rec[(i - 1) & 3];
-    Hit* recC = sm.rec[(i - 2) & 3];
-    const uint16_t* bucketA = sm.bucket[i & 3];
-    const uint16_t* bucketC = sm.bucket[(i - 2) & 3];
+    Hit* recA = sm.rec[i % 3];
+    Hit* recB = sm.rec[(i - 1) % 3];
+    Hit* recC = sm.rec[(i - 2) % 3];
+    const uint16_t* bucketA = sm.bucket[i % 3];
+    const uint16_t* bucketC = sm.bucket[(i - 2) % 3];
 
     __pipeline_wait_prior(0);
     tsync<C>();  // B1: layer C staged; tracks created by the previous T4 visible; claims re-initialised
-    if (i >= 3) stage_layer(c, (uint32_t)i - 3);  // prefetch: needed at the top of the next iteration
 
     // ---- T1 forward: best hit of layer C per active track (nothing of C is used yet); claim with (bits(S), key)
     const uint32_t first = min(sm.min_active[i & 1], first_new);
@@ -402,6 +401,9 @@ __device__ __forceinline__ void track_event(const TrackLaunch& a, uint32_t e, Sm
 
     // ---- T4a: every b with a triplet claims its a and its c with (bits(S), b)
     if (tid == 0) sm.n_doublets = 0;  // S2 is over; the next S1 starts after two more barriers
+    // layer A is done with (T4 reads only B and C): its ring slot takes the next layer, needed at the top of the
+    // next iteration; the copy runs behind T4
+    if (i >= 3) stage_layer(c, (uint32_t)i - 3);
     const uint32_t roundsB = seeding ? (nB + C::kThreads - 1) / C::kThreads : 0;  // block-uniform
 #pragma unroll 1
     for (uint32_t kb = tid; kb < nB && seeding; kb += C::kThreads) {
