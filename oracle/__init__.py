@@ -62,6 +62,7 @@ def lib():
         L.oracle_scatter.argtypes = [ctypes.c_void_p] * 3
         L.oracle_fit.argtypes = [ctypes.c_uint32] + [ctypes.c_void_p] * 4
         L.oracle_kalman.argtypes = [ctypes.c_uint32] + [ctypes.c_void_p] * 5 + [ctypes.c_double, ctypes.c_void_p]
+        L.oracle_pvs.argtypes = [ctypes.c_uint32] + [ctypes.c_void_p] * 9 + [ctypes.c_int]
         L.oracle_run.restype = ctypes.c_void_p
         L.oracle_run.argtypes = [ctypes.POINTER(_Geometry), ctypes.c_void_p, ctypes.c_void_p, ctypes.c_uint32,
                                  ctypes.c_uint32]
@@ -236,3 +237,24 @@ def kalman_of(result: "Result", pitch: float) -> np.ndarray:
     ev_of_hit = np.repeat(ev_of_track, np.diff(t.hit_offsets.astype(np.int64)))
     abs_hits = c.event_offsets[ev_of_hit].astype(np.int64) + t.hits
     return kalman(t.hit_offsets, abs_hits, c.x, c.y, c.z, pitch)
+
+
+PV_MAX = 32
+
+
+def find_pvs(track_offsets, x0, y0, tx, ty, kal, iterations: int = 8):
+    """O8 (R10): primary vertices per event from the straight-line fit (seeding histogram) and the Kalman
+    states (weighted fit).  Returns (vertices [n_events, 32, 8] float64, counts [n_events], candidates [n_events])."""
+    to = np.ascontiguousarray(track_offsets, np.uint32)
+    x0, y0, tx, ty = (np.ascontiguousarray(a, np.float32) for a in (x0, y0, tx, ty))
+    kal = np.ascontiguousarray(kal, np.float64)
+    n = len(to) - 1
+    out = np.zeros((n, PV_MAX, 8), np.float64)
+    counts, cands = np.zeros(n, np.uint32), np.zeros(n, np.uint32)
+    lib().oracle_pvs(n, _p(to), _p(x0), _p(y0), _p(tx), _p(ty), _p(kal), _p(out), _p(counts), _p(cands), iterations)
+    return out, counts, cands
+
+
+def pvs_of(result: "Result", pitch: float):
+    t = result.tracks
+    return find_pvs(t.event_offsets, t.x0, t.y0, t.tx, t.ty, kalman_of(result, pitch))

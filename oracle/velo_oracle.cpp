@@ -17,6 +17,9 @@
 //   O6 straight-line fit P:149 "tracks in the Velo detector form straight lines" -> unweighted LSQ (D:R6)
 //   O7 simple Kalman fit P:185 "simple Kalman filter ... x- and y-components are independent ... constant average
 //                        transverse momentum of 400 MeV ... noise contribution from multiple scattering" (D:R9)
+//   O8 PV finding        P:187 "histogram of the point of closest approach of tracks to the beamline, where a cluster
+//                        indicates a PV candidate ... every track is assigned to every vertex based on a weight, so
+//                        that all candidates can be fitted in parallel" (D:R10)
 //
 // Build: g++ -O2 -std=c++17 -ffp-contract=off (no fast-math) -shared -fPIC -pthread.
 #include <algorithm>
@@ -500,6 +503,98 @@ void kalman_track(uint32_t n, const float* x, const float* y, const float* z, do
   out12[5] = chi2;
 }
 
+// ------------------------------------------------------------------------------------------------
+// O8: primary vertices of one event (D:R10 step by step).
+//   1. z of closest approach to the beam line (x = y = 0) from the straight-line fit (O6, fp32, normative ops):
+//      t2 = tx*tx + ty*ty (fma), zp = -(x0*tx + y0*ty) / t2; tracks with t2 < 1e-8 or zp outside [-300, 300) are left out
+//   2. histogram h of zp in 600 bins of 1 mm; s[b] = h[b-1] + h[b] + h[b+1]; bin b is a candidate iff s[b] >= 4 and
+//      (s[b], h[b]) > (s[b-1], h[b-1]) and (s[b], h[b]) >= (s[b+1], h[b+1]) in lexicographic order;
+//      z_seed = -300 + b + 0.5 + (h[b+1] - h[b-1]) / s[b]
+//   3. every candidate is fitted with ALL tracks, 8 iterations from (0, 0, z_seed): track position and variance at the
+//      vertex z from its Kalman state (O7); chi2_t = dx^2/var_x + dy^2/var_y; Tukey weight w = (1 - chi2_t/12)^2 below
+//      12, else 0; one exact weighted least-squares step for (vx, vy, vz) per iteration
+//   4. accepted iff sum w >= 3 after the last iteration; a vertex is dropped if another accepted one lies within 1 mm
+//      in z and has a larger sum w (equal: the earlier candidate wins)
+// kal: [n][12] from O7; out rows: x, y, z, sum_w, n_tracks (w > 0), chi2 (sum w chi2_t), z_seed, 0.  fp64 except step 1.
+// ------------------------------------------------------------------------------------------------
+constexpr int kPvBins = 600;
+constexpr int kPvMax = 32;
+
+uint32_t find_pvs(uint32_t n, const float* x0, const float* y0, const float* tx, const float* ty, const double* kal,
+                  double* out /* [kPvMax][8] */, uint32_t* n_candidates, int n_iter = 8) {
+  int h[kPvBins + 2] = {0};  // h[b + 1] = bin b; guard bins at both ends
+  for (uint32_t i = 0; i < n; ++i) {
+    const float t2 = std::fmaf(tx[i], tx[i], ty[i] * ty[i]);
+    if (!(t2 >= 1e-8f)) continue;
+    const float zp = -std::fmaf(x0[i], tx[i], y0[i] * ty[i]) / t2;
+    const float u = zp + 300.0f;
+    if (!(u >= 0.0f) || !(u < (float)kPvBins)) continue;
+    h[(int)std::floor(u) + 1] += 1;
+  }
+  struct Cand { double z_seed, v[3], sw, chi2; int nw; bool ok; };
+  std::vector<Cand> cands;
+  for (int b = 0; b < kPvBins; ++b) {
+    const int hm = h[b], hc = h[b + 1], hp = h[b + 2];
+    const int s = hm + hc + hp;
+    const int sl = (b > 0 ? h[b - 1] : 0) + hm + hc, sr = hc + hp + (b + 3 < kPvBins + 2 ? h[b + 3] : 0);
+    // local maximum of (s, h) in lexicographic order: strictly above the left neighbour, not below the right one
+    const bool above_left = s > sl || (s == sl && hc > hm), not_below_right = s > sr || (s == sr && hc >= hp);
+    if (s >= 4 && above_left && not_below_right) {
+      Cand c{};
+      c.z_seed = -300.0 + b + 0.5 + (double)(hp - hm) / s;
+      cands.push_back(c);
+    }
+  }
+  *n_candidates = (uint32_t)cands.size();
+  for (Cand& c : cands) {
+    double vx = 0, vy = 0, vz = c.z_seed;
+    c.ok = true;
+    for (int it = 0; it < n_iter && c.ok; ++it) {
+      double a00 = 0, a11 = 0, a02 = 0, a12 = 0, a22 = 0, b0 = 0, b1 = 0, b2 = 0, sw = 0, chi2 = 0;
+      int nw = 0;
+      for (uint32_t i = 0; i < n; ++i) {
+        const double* k = kal + 12 * (size_t)i;
+        const double d = vz - k[4];
+        const double dx = k[0] + k[2] * d - vx, dy = k[1] + k[3] * d - vy;
+        const double var_x = k[6] + 2 * d * k[7] + d * d * k[8], var_y = k[9] + 2 * d * k[10] + d * d * k[11];
+        const double c2 = dx * dx / var_x + dy * dy / var_y;
+        if (!(c2 < 12.0)) continue;
+        const double w = (1 - c2 / 12.0) * (1 - c2 / 12.0);
+        const double wx = w / var_x, wy = w / var_y;
+        a00 += wx; a11 += wy; a02 -= wx * k[2]; a12 -= wy * k[3]; a22 += wx * k[2] * k[2] + wy * k[3] * k[3];
+        b0 += wx * dx; b1 += wy * dy; b2 -= wx * k[2] * dx + wy * k[3] * dy;
+        sw += w; chi2 += w * c2; nw += 1;
+      }
+      c.sw = sw; c.chi2 = chi2; c.nw = nw;
+      if (it == n_iter - 1) break;  // the sums of the last pass describe the final position
+      // solve [[a00, 0, a02], [0, a11, a12], [a02, a12, a22]] delta = b by eliminating the first two unknowns
+      if (!(a00 > 0) || !(a11 > 0)) { c.ok = false; break; }
+      const double den = a22 - a02 * a02 / a00 - a12 * a12 / a11;
+      if (!(den > 0)) { c.ok = false; break; }
+      const double dz = (b2 - a02 * b0 / a00 - a12 * b1 / a11) / den;
+      vx += (b0 - a02 * dz) / a00;
+      vy += (b1 - a12 * dz) / a11;
+      vz += dz;
+    }
+    c.v[0] = vx; c.v[1] = vy; c.v[2] = vz;
+    c.ok = c.ok && c.sw >= 3.0;
+  }
+  uint32_t n_out = 0;
+  for (size_t i = 0; i < cands.size(); ++i) {
+    if (!cands[i].ok) continue;
+    bool dropped = false;
+    for (size_t j = 0; j < cands.size() && !dropped; ++j)
+      if (j != i && cands[j].ok && std::fabs(cands[j].v[2] - cands[i].v[2]) < 1.0 &&
+          (cands[j].sw > cands[i].sw || (cands[j].sw == cands[i].sw && j < i)))
+        dropped = true;
+    if (dropped || n_out >= (uint32_t)kPvMax) continue;
+    double* o = out + 8 * (size_t)n_out++;
+    o[0] = cands[i].v[0]; o[1] = cands[i].v[1]; o[2] = cands[i].v[2]; o[3] = cands[i].sw;
+    o[4] = cands[i].nw; o[5] = cands[i].chi2; o[6] = cands[i].z_seed; o[7] = 0;
+  }
+  return n_out;
+}
+
 void reconstruct_event(const Geometry& g, const uint8_t* raw, size_t bytes, EventResult& out, Scratch& sc) {
   cluster_event(g, raw, bytes, out, sc);
   if (out.status & (STATUS_BAD_HEADER | STATUS_TOO_MANY_CLUSTERS)) return;
@@ -549,6 +644,18 @@ void oracle_kalman(uint32_t n_tracks, const uint32_t* hit_offsets, const uint32_
       hx[k] = x[h]; hy[k] = y[h]; hz[k] = z[h];
     }
     kalman_track(n, hx.data(), hy.data(), hz.data(), pitch, out12 + 12 * (size_t)t);
+  }
+}
+
+// O8 for a batch: tracks of event e are [track_offsets[e], track_offsets[e+1]); out [n_events][32][8], counts [n_events],
+// candidates [n_events] (histogram peaks before the fit).
+void oracle_pvs(uint32_t n_events, const uint32_t* track_offsets, const float* x0, const float* y0, const float* tx,
+                const float* ty, const double* kal, double* out, uint32_t* counts, uint32_t* candidates,
+                int n_iter /* 8 in the method; other values only for the pins */) {
+  for (uint32_t e = 0; e < n_events; ++e) {
+    const uint32_t t0 = track_offsets[e], n = track_offsets[e + 1] - t0;
+    counts[e] = find_pvs(n, x0 + t0, y0 + t0, tx + t0, ty + t0, kal + 12 * (size_t)t0, out + (size_t)e * kPvMax * 8,
+                         candidates + e, n_iter);
   }
 }
 
