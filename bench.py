@@ -196,7 +196,11 @@ def run_ours(args):
     velo = binding.AllenVelo(geo)
     ccap = int(1.15 * n_sp) + 4096
     oc, ot = binding.alloc_outputs(n_events, L, ccap, ccap // 3, ccap // 2, device, with_checksum=False,
-                                   with_kalman=args.with_kalman)
+                                   with_kalman=args.with_kalman or args.with_vertices)
+    if args.with_vertices:
+        d_nv = torch.zeros(n_events, dtype=torch.int32, device=device)
+        d_pv = torch.zeros((n_events, 32, 8), dtype=torch.float32, device=device)
+        velo.set_vertex_output(d_nv, d_pv)
     ws = torch.empty(velo.workspace_bytes(n_events, raw_bytes), dtype=torch.uint8, device=device)
     velo.set_workspace(ws)
     velo.set_occupancy_hint(n_events, raw_bytes)
@@ -370,7 +374,7 @@ def run_ours(args):
         ms_per_step=ms_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32", data="synthetic",
         config=dict(workload=f"config{args.config}: {n_events} events/GPU at nu={'12' if args.config == 3 else '6'} "
                              f"(BASELINE.json configs[{args.config}])",
-                    events_per_gpu=n_events, parallelism=f"replicas x{world} (events independent, no collective)", kalman_fit=bool(args.with_kalman),
+                    events_per_gpu=n_events, parallelism=f"replicas x{world} (events independent, no collective)", kalman_fit=bool(args.with_kalman or args.with_vertices), vertices=bool(args.with_vertices),
                     l2_policy="inputs+outputs per step (%.0f MB) larger than the 126 MB L2" % (ab["total"] / 1e6),
                     input_sha=batch.sha(), sp_words_per_event=n_sp / n_events, clusters_per_event=n_clusters / n_events,
                     tracks_per_event=n_tracks / n_events, hits_per_track=n_track_hits / max(1, n_tracks),
@@ -404,6 +408,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--with-kalman", action="store_true",
                     help="also produce the simple Kalman fit (SURVEY 8(f1), beyond the headline path; +48 B per track)")
+    ap.add_argument("--with-vertices", action="store_true",
+                    help="also find primary vertices (SURVEY 8(f2), beyond the headline path; implies --with-kalman)")
     ap.add_argument("--e2e-chunk", type=int, default=1250, help="events per chunk of the streamed end-to-end run")
     ap.add_argument("--e2e-streams", type=int, default=4)
     args = ap.parse_args()

@@ -100,6 +100,14 @@ typedef struct {
                               (position, slope) for x and for y */
 } allen_velo_tracks_t;
 
+/* Primary vertices (R10; optional, beyond the headline path): a fixed number of slots per event. */
+typedef struct {
+  uint32_t max_per_event; /* slots per event in `vertices`; at most 32 are ever filled */
+  uint32_t* n_vertices;   /* DEVICE [n_events] */
+  float* vertices;        /* DEVICE [n_events][max_per_event][8]: x, y, z, sum of track weights, tracks with weight > 0,
+                             chi2 (sum w chi2_t), z of the histogram seed, 0 */
+} allen_velo_vertices_t;
+
 typedef struct allen_velo allen_velo_t;
 
 /* Fills *params with the default cuts of R5. */
@@ -119,6 +127,11 @@ int allen_velo_set_workspace(allen_velo_t* handle, void* dev_ptr /* DEVICE */, s
  * close enough).  The results never depend on it; it selects the cluster-kernel instance whose shared-memory
  * capacity suits the occupancy (above 192 words per layer: 512 entries per layer instead of 256).  0 = no hint. */
 int allen_velo_set_occupancy_hint(allen_velo_t* handle, uint32_t sp_words_per_layer);
+
+/* Optional: from now on reconstruct() also finds primary vertices and writes them to `out` (a HOST struct of DEVICE
+ * pointers, copied; NULL switches it off again).  Needs out_tracks->kalman in the reconstruct() calls (the vertex fit
+ * uses the Kalman states); reconstruct() returns ALLEN_VELO_ERR_INVALID otherwise. */
+int allen_velo_set_vertex_output(allen_velo_t* handle, const allen_velo_vertices_t* out);
 
 /* Enqueues the whole hot path for one batch on `cuda_stream` and returns WITHOUT synchronising.
  *   raw_banks      DEVICE, 16-byte aligned: events in raw format v1 (R1) back to back

@@ -514,7 +514,7 @@ void kalman_track(uint32_t n, const float* x, const float* y, const float* z, do
 //      vertex z from its Kalman state (O7); chi2_t = dx^2/var_x + dy^2/var_y; Tukey weight w = (1 - chi2_t/12)^2 below
 //      12, else 0; one exact weighted least-squares step for (vx, vy, vz) per iteration
 //   4. accepted iff sum w >= 3 after the last iteration; a vertex is dropped if another accepted one lies within 1 mm
-//      in z and has a larger sum w (equal: the earlier candidate wins)
+//      in z and has a sum w more than 0.1 % larger (within 0.1 %: the earlier candidate wins)
 // kal: [n][12] from O7; out rows: x, y, z, sum_w, n_tracks (w > 0), chi2 (sum w chi2_t), z_seed, 0.  fp64 except step 1.
 // ------------------------------------------------------------------------------------------------
 constexpr int kPvBins = 600;
@@ -584,9 +584,11 @@ uint32_t find_pvs(uint32_t n, const float* x0, const float* y0, const float* tx,
     if (!cands[i].ok) continue;
     bool dropped = false;
     for (size_t j = 0; j < cands.size() && !dropped; ++j)
-      if (j != i && cands[j].ok && std::fabs(cands[j].v[2] - cands[i].v[2]) < 1.0 &&
-          (cands[j].sw > cands[i].sw || (cands[j].sw == cands[i].sw && j < i)))
-        dropped = true;
+      if (j != i && cands[j].ok && std::fabs(cands[j].v[2] - cands[i].v[2]) < 1.0) {
+        // candidates that converged to the same vertex have the same sum w up to rounding: within 0.1 % is a tie
+        const bool j_larger = cands[j].sw > cands[i].sw * 1.001, i_larger = cands[i].sw > cands[j].sw * 1.001;
+        if (j_larger || (!i_larger && j < i)) dropped = true;
+      }
     if (dropped || n_out >= (uint32_t)kPvMax) continue;
     double* o = out + 8 * (size_t)n_out++;
     o[0] = cands[i].v[0]; o[1] = cands[i].v[1]; o[2] = cands[i].v[2]; o[3] = cands[i].sw;

@@ -43,6 +43,10 @@ class allen_velo_tracks_t(ctypes.Structure):
         (n, ctypes.c_void_p) for n in ("event_offsets", "hit_offsets", "hits", "x0", "y0", "tx", "ty", "kalman")]
 
 
+class allen_velo_vertices_t(ctypes.Structure):
+    _fields_ = [("max_per_event", ctypes.c_uint32), ("n_vertices", ctypes.c_void_p), ("vertices", ctypes.c_void_p)]
+
+
 _lib = None
 
 
@@ -64,6 +68,8 @@ def load_library():
         L.allen_velo_set_workspace.restype = ctypes.c_int
         L.allen_velo_set_occupancy_hint.argtypes = [ctypes.c_void_p, ctypes.c_uint32]
         L.allen_velo_set_occupancy_hint.restype = ctypes.c_int
+        L.allen_velo_set_vertex_output.argtypes = [ctypes.c_void_p, ctypes.POINTER(allen_velo_vertices_t)]
+        L.allen_velo_set_vertex_output.restype = ctypes.c_int
         L.allen_velo_reconstruct.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_uint32,
                                              ctypes.c_void_p, ctypes.POINTER(allen_velo_clusters_t),
                                              ctypes.POINTER(allen_velo_tracks_t)]
@@ -194,6 +200,19 @@ class AllenVelo:
         if self._lib.allen_velo_set_occupancy_hint(self._h, per_layer) != OK:
             raise RuntimeError("allen_velo_set_occupancy_hint failed")
 
+    def set_vertex_output(self, n_vertices=None, vertices=None) -> None:
+        """Primary vertices (optional): `n_vertices` int32 [n_events], `vertices` float32 [n_events, slots, 8] CUDA
+        tensors the caller keeps alive; None switches the output off."""
+        if vertices is None:
+            rc = self._lib.allen_velo_set_vertex_output(self._h, None)
+            self._pv = None
+        else:
+            s = allen_velo_vertices_t(int(vertices.shape[1]), n_vertices.data_ptr(), vertices.data_ptr())
+            rc = self._lib.allen_velo_set_vertex_output(self._h, ctypes.byref(s))
+            self._pv = (n_vertices, vertices)
+        if rc != OK:
+            raise RuntimeError(f"allen_velo_set_vertex_output failed with {rc}: {self.last_error()}")
+
     def set_workspace(self, tensor) -> None:
         """`tensor`: a torch uint8 CUDA tensor the caller keeps alive (kept referenced here too)."""
         rc = self._lib.allen_velo_set_workspace(self._h, tensor.data_ptr(), tensor.numel() * tensor.element_size())
@@ -246,7 +265,8 @@ class AllenVelo:
 
 def reconstruct_batch(velo: AllenVelo, raw: np.ndarray, event_offsets: np.ndarray, device="cuda:0",
                       with_checksum: bool = True, cluster_capacity: int | None = None,
-                      track_capacity: int | None = None, hit_capacity: int | None = None, with_kalman: bool = False):
+                      track_capacity: int | None = None, hit_capacity: int | None = None, with_kalman: bool = False,
+                      with_vertices: bool = False):
     """Convenience for tests/smoke: copy a host batch to the device, run the path once, return host copies.
 
     Host<->device copies and the final synchronise happen here, outside the C ABI.  Returns (clusters, tracks)
@@ -265,7 +285,15 @@ def reconstruct_batch(velo: AllenVelo, raw: np.ndarray, event_offsets: np.ndarra
     ws = torch.empty(velo.workspace_bytes(n_events, raw_bytes), dtype=torch.uint8, device=device)
     velo.set_workspace(ws)
     velo.set_occupancy_hint(n_events, raw_bytes)
-    rc = velo.reconstruct(d_raw, d_off, n_events, None, oc, ot)
+    if with_vertices:
+        d_nv = torch.zeros(max(n_events, 1), dtype=torch.int32, device=device)
+        d_pv = torch.zeros((max(n_events, 1), 32, 8), dtype=torch.float32, device=device)
+        velo.set_vertex_output(d_nv, d_pv)
+    try:
+        rc = velo.reconstruct(d_raw, d_off, n_events, None, oc, ot)
+    finally:
+        if with_vertices:
+            velo.set_vertex_output(None, None)
     if rc != OK:
         raise RuntimeError(f"allen_velo_reconstruct failed with {rc}: {velo.last_error()}")
     torch.cuda.synchronize()
@@ -290,6 +318,9 @@ def reconstruct_batch(velo: AllenVelo, raw: np.ndarray, event_offsets: np.ndarra
         tracks[name] = host(getattr(ot, name), np.float32)[:min(nt, tcap)]
     if with_kalman:
         tracks["kalman"] = host(ot.kalman, np.float32).reshape(-1, 12)[:min(nt, tcap)]
+    if with_vertices:
+        tracks["n_vertices"] = d_nv.cpu().numpy().view(np.uint32)[:n_events]
+        tracks["vertices"] = d_pv.cpu().numpy()[:n_events]
     return clusters, tracks
 
 

@@ -20,6 +20,7 @@ struct allen_velo {
   uint32_t n_mid_sms = 0;      // SM ids the mid-slot pool of the cluster kernel covers
   uint32_t n_sms = 0;
   uint32_t sp_words_per_layer = 0;  // caller's hint (0: none)
+  allen_velo_vertices_t vertices{};  // optional primary-vertex output (vertices == nullptr: off)
   cudaStream_t side[2] = {nullptr, nullptr};  // the larger track-kernel instances run beside the first one
   cudaEvent_t fork_join[3] = {nullptr, nullptr, nullptr};
   std::string last_error;
@@ -182,6 +183,14 @@ int allen_velo_set_occupancy_hint(allen_velo_t* h, uint32_t sp_words_per_layer) 
   return ALLEN_VELO_OK;
 }
 
+int allen_velo_set_vertex_output(allen_velo_t* h, const allen_velo_vertices_t* out) {
+  if (!h) return ALLEN_VELO_ERR_INVALID;
+  if (!out) { h->vertices = allen_velo_vertices_t{}; return ALLEN_VELO_OK; }
+  if (!out->n_vertices || !out->vertices || out->max_per_event == 0) return fail(h, ALLEN_VELO_ERR_INVALID, "null vertex output");
+  h->vertices = *out;
+  return ALLEN_VELO_OK;
+}
+
 int allen_velo_set_workspace(allen_velo_t* h, void* dev_ptr, size_t bytes) {
   if (!h) return ALLEN_VELO_ERR_INVALID;
   if (dev_ptr && (reinterpret_cast<uintptr_t>(dev_ptr) % kAlign)) return fail(h, ALLEN_VELO_ERR_INVALID, "workspace misaligned");
@@ -202,6 +211,7 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
     return fail(h, ALLEN_VELO_ERR_INVALID, "null cluster array");
   if (ot->capacity_tracks && (!ot->x0 || !ot->y0 || !ot->tx || !ot->ty)) return fail(h, ALLEN_VELO_ERR_INVALID, "null track array");
   if (ot->capacity_hits && !ot->hits) return fail(h, ALLEN_VELO_ERR_INVALID, "null hits array");
+  if (h->vertices.vertices && !ot->kalman) return fail(h, ALLEN_VELO_ERR_INVALID, "vertex output needs tracks.kalman");
   const uint32_t L = h->dev.n_layers;
   if ((uint64_t)n_events * L >= (1ull << 31)) return fail(h, ALLEN_VELO_ERR_INVALID, "too many events");
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
@@ -333,6 +343,15 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   if ((err = launch_compact_tracks(ct, stream)) != cudaSuccess) return fail(h, ALLEN_VELO_ERR_CUDA, "track compaction", err);
   h->last_launches++;
   mark(5);
+  if (h->vertices.vertices) {  // beyond the timed segments of the headline path
+    PvLaunch pv{};
+    pv.n_events = n_events;
+    pv.tracks = *ot;
+    pv.out = h->vertices;
+    pv.status = oc->status;
+    if ((err = launch_pv(pv, stream)) != cudaSuccess) return fail(h, ALLEN_VELO_ERR_CUDA, "vertex kernel", err);
+    h->last_launches++;
+  }
   return ALLEN_VELO_OK;
 }
 

@@ -166,4 +166,13 @@ struct CompactTracksLaunch {
 };
 cudaError_t launch_compact_tracks(const CompactTracksLaunch& a, cudaStream_t stream);
 
+// Primary-vertex finding, one warp per event, after the tracks are compacted (velo_pv.cu).
+struct PvLaunch {
+  uint32_t n_events;
+  allen_velo_tracks_t tracks;  // compacted tracks incl. the Kalman states
+  allen_velo_vertices_t out;
+  uint32_t* status;            // [n_events]
+};
+cudaError_t launch_pv(const PvLaunch& a, cudaStream_t stream);
+
 }  // namespace velo
