@@ -389,3 +389,36 @@ def test_primary_vertices_against_the_oracle(velo, geometry, oracle_of, config, 
             assert abs(a[4] - b[4]) <= 1, (e, a, b)   # a track exactly at the Tukey cut-off may flip
     print("vertices", n_total, "near-cut disagreements", n_near_cut, "fit bit-identical", same_fit, "worst", worst)
     assert n_total > 0 and n_near_cut <= max(1, n_total // 1000)
+
+
+def test_layer_beyond_the_largest_staging_capacity_is_flagged_not_wrong(velo, geometry):
+    """Documented limit: more than 1024 hits in one layer -> the event is flagged STAGE_OVERFLOW and
+    gets no tracks; its clusters are still complete and exact, and the other events of the batch are untouched."""
+    import oracle
+    from paper_1912_09161_b200 import binding, workload
+    from tests.helpers import compare_clusters
+
+    rng = np.random.default_rng(11)
+    busy = set()
+    while len(busy) < 1300:   # isolated pixels (every third column / row) on the four sensors of layer 6
+        busy.add((24 + int(rng.integers(4)), 3 * int(rng.integers(256)), 3 * int(rng.integers(85))))
+    normal = workload.generate(1, n_events=3)
+    ev = []
+    for e in range(3):   # re-pack three generated events through pack_events, with the busy layer added to the second
+        m = normal.pixels["event"] == e
+        px = sorted(set(zip(normal.pixels["sensor"][m].tolist(), normal.pixels["col"][m].tolist(), normal.pixels["row"][m].tolist())))
+        ev.append(px + (sorted(busy) if e == 1 else []))
+    raw, off = workload.pack_events(geometry, ev, shuffle_seed=5)
+    ref = oracle.reconstruct(geometry, raw, off)
+    clusters, tracks = binding.reconstruct_batch(velo, raw, off)
+    assert clusters["status"].tolist() == [0, binding.STATUS_STAGE_OVERFLOW, 0]
+    clusters["status"] = ref.clusters.status   # compare everything but the flag
+    c, t = as_oracle_types(clusters, tracks)
+    assert not compare_clusters(c, ref.clusters)
+    rt = ref.tracks
+    assert int(np.diff(rt.event_offsets)[1]) > 0   # the oracle, without the limit, does find tracks there
+    assert np.diff(tracks["event_offsets"]).tolist() == [int(np.diff(rt.event_offsets)[0]), 0, int(np.diff(rt.event_offsets)[2])]
+    # events 0 and 2: identical hit lists
+    h0 = rt.hits[:rt.hit_offsets[rt.event_offsets[1]]]
+    h2 = rt.hits[rt.hit_offsets[rt.event_offsets[2]]:]
+    assert np.array_equal(tracks["hits"], np.concatenate([h0, h2]))
