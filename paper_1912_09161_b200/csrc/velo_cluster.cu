@@ -61,6 +61,8 @@ struct ClusterStore {  // cluster records of the whole layer
 struct SortStore {
   uint32_t* cnt256;             // [256]
   uint16_t *tmp, *order, *phis; // [cap] each; phis = phi16 + 32768
+  float* uv;                    // [2][cap] local coordinates kept between ranking and writing, or nullptr (recompute)
+  uint32_t cap;
 };
 
 __device__ __forceinline__ uint32_t hash_slot(uint32_t key, uint32_t bits) { return (key * 0x9E3779B1u) >> (32 - bits); }
@@ -137,6 +139,12 @@ __device__ __forceinline__ bool ccl_pass(const Pass& p, const ClusterStore& cs, 
   }
   const uint32_t my_start = incl - in_group;                 // first staged index of sensor `lane`
   const uint32_t n = __shfl_sync(kFull, incl, (k1 - 1) & 31);  // staged words of the group
+  uint32_t start_of[kMaxSensorsPerLayer];  // first staged index of every sensor of the group; "never" outside it
+#pragma unroll
+  for (int kk = 0; kk < kMaxSensorsPerLayer; ++kk) {
+    const uint32_t st = __shfl_sync(kFull, my_start, kk);
+    start_of[kk] = ((uint32_t)kk > k0 && (uint32_t)kk < k1) ? st : 0xFFFFFFFFu;
+  }
 #pragma unroll 1
   for (uint32_t i0 = 0; i0 < n; i0 += 128) {
     uint32_t w[4], ks[4];
@@ -144,8 +152,8 @@ __device__ __forceinline__ bool ccl_pass(const Pass& p, const ClusterStore& cs, 
     for (int u = 0; u < 4; ++u) {
       const uint32_t i = i0 + 32 * u + lane;
       uint32_t k = k0;
-#pragma unroll 1
-      for (uint32_t kk = k0 + 1; kk < k1; ++kk) k += i >= __shfl_sync(kFull, my_start, kk);
+#pragma unroll
+      for (int kk = 1; kk < kMaxSensorsPerLayer; ++kk) k += i >= start_of[kk];
       const uint32_t src = __shfl_sync(kFull, my_off, k) + (i - __shfl_sync(kFull, my_start, k));
       ks[u] = k;
       w[u] = i < n ? __ldg(spw + src) : 0u;
@@ -162,8 +170,11 @@ __device__ __forceinline__ bool ccl_pass(const Pass& p, const ClusterStore& cs, 
       }
     }
   }
+  {
+    uint4* tab4 = reinterpret_cast<uint4*>(p.tab);  // 16-byte aligned in every storage
 #pragma unroll 1
-  for (uint32_t s = lane; s < (1u << bits); s += 32) p.tab[s] = 0;
+    for (uint32_t s = lane; s < (1u << bits) / 4; s += 32) tab4[s] = make_uint4(0, 0, 0, 0);
+  }
   if (lane == 0) *n_edges_ctr = 0;
   __syncwarp();
 
@@ -341,8 +352,10 @@ __device__ __forceinline__ void finish_layer(const ClusterLaunch& a, const Clust
   __syncwarp();
 #pragma unroll 1
   for (uint32_t c = lane; c < n_cl; c += 32) {
-    float x, y, z;
-    cluster_position(cs.n[c], cs.col[c], cs.row[c], g.pitch, g.ltg + 9 * (cs.key[c] >> 18), x, y, z);
+    float u, v, x, y, z;
+    cluster_local(cs.n[c], cs.col[c], cs.row[c], g.pitch, u, v);
+    local_to_global(u, v, g.ltg + 9 * (cs.key[c] >> 18), x, y, z);
+    if (ss.uv) { ss.uv[c] = u; ss.uv[ss.cap + c] = v; }
     const uint16_t p = (uint16_t)((uint16_t)phi16_of(x, y) ^ 0x8000u);
     ss.phis[c] = p;
     atomicAdd(&ss.cnt256[p >> 8], 1u);
@@ -385,8 +398,10 @@ __device__ __forceinline__ void finish_layer(const ClusterLaunch& a, const Clust
   for (uint32_t j = lane; j < n_cl; j += 32) {
     const uint32_t c = ss.order[j];
     const uint32_t key = cs.key[c], n = cs.n[c], sc = cs.col[c], sr = cs.row[c];
-    float x, y, z;
-    cluster_position(n, sc, sr, g.pitch, g.ltg + 9 * (key >> 18), x, y, z);
+    float u, v, x, y, z;
+    if (ss.uv) { u = ss.uv[c]; v = ss.uv[ss.cap + c]; }
+    else cluster_local(n, sc, sr, g.pitch, u, v);
+    local_to_global(u, v, g.ltg + 9 * (key >> 18), x, y, z);
     const uint32_t o = slab0 + j;
     a.slab.key[o] = key;
     a.slab.n_pixels[o] = n;
@@ -415,7 +430,7 @@ __device__ __noinline__ void finish_layer_generic(const ClusterLaunch& a, const 
 }
 
 template <bool kChecksum, uint32_t kCap>
-struct WarpSmem {
+struct alignas(16) WarpSmem {
   static constexpr uint32_t kCapSp = kCap, kCapEdges = kCap, kCapCl = kCap, kHashBits = Caps<kCap>::kHashBits;
   uint32_t sp[kCapSp];
   uint32_t tab[1u << kHashBits];
@@ -453,6 +468,7 @@ __device__ __forceinline__ void stores_at(unsigned char* base, size_t stats, siz
   ss.cnt256 = reinterpret_cast<uint32_t*>(base + cnt);
   uint16_t* t = reinterpret_cast<uint16_t*>(base + sort);
   ss.tmp = t; ss.order = t + cap; ss.phis = t + 2 * cap;
+  ss.uv = nullptr; ss.cap = cap;
 }
 
 template <bool kChecksum, uint32_t kCap>
@@ -475,6 +491,8 @@ __global__ void __launch_bounds__(kWarps * 32) velo_cluster_kernel(const __grid_
   ss.tmp = reinterpret_cast<uint16_t*>(ws.tab);
   ss.order = ss.tmp + kCapCl;
   ss.phis = ss.order + kCapCl;
+  ss.uv = reinterpret_cast<float*>(ws.lab);  // lab + edges: 2 * kCapCl floats, dead once the cluster records exist
+  ss.cap = kCapCl;
 
   // ---------------- A1: the layer's bank ranges, validated and laid out by velo_prepare_kernel ----------------
   const uint32_t* d = a.desc + (size_t)item * kDescWords;

@@ -51,15 +51,26 @@ __device__ __forceinline__ uint32_t mix32(uint32_t v) {
 }
 
 // Normative fp32 position of a cluster (R3): every operation a single IEEE RN op, fma fused, no contraction.
-__device__ __forceinline__ void cluster_position(uint32_t n, uint32_t sum_col, uint32_t sum_row, float pitch,
-                                                 const float* __restrict__ M, float& x, float& y, float& z) {
+// Two halves: local coordinates (u, v) from the integer sums, then the sensor's local-to-global transform.
+__device__ __forceinline__ void cluster_local(uint32_t n, uint32_t sum_col, uint32_t sum_row, float pitch, float& u,
+                                              float& v) {
   const float fn = __uint2float_rn(n);
   const float fc = __fadd_rn(__fdiv_rn(__uint2float_rn(sum_col), fn), 0.5f);
   const float fr = __fadd_rn(__fdiv_rn(__uint2float_rn(sum_row), fn), 0.5f);
-  const float u = __fmul_rn(fc, pitch), v = __fmul_rn(fr, pitch);
+  u = __fmul_rn(fc, pitch);
+  v = __fmul_rn(fr, pitch);
+}
+__device__ __forceinline__ void local_to_global(float u, float v, const float* __restrict__ M, float& x, float& y,
+                                                float& z) {
   x = __fmaf_rn(u, __ldg(M + 0), __fmaf_rn(v, __ldg(M + 1), __ldg(M + 2)));
   y = __fmaf_rn(u, __ldg(M + 3), __fmaf_rn(v, __ldg(M + 4), __ldg(M + 5)));
   z = __fmaf_rn(u, __ldg(M + 6), __fmaf_rn(v, __ldg(M + 7), __ldg(M + 8)));
+}
+__device__ __forceinline__ void cluster_position(uint32_t n, uint32_t sum_col, uint32_t sum_row, float pitch,
+                                                 const float* __restrict__ M, float& x, float& y, float& z) {
+  float u, v;
+  cluster_local(n, sum_col, sum_row, pitch, u, v);
+  local_to_global(u, v, M, x, y, z);
 }
 
 // Normative phi16 (R3): Abramowitz & Stegun 4.4.49 polynomial, Horner with fma, round-half-even, wrap.
