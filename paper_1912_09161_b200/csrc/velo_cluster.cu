@@ -471,17 +471,14 @@ __device__ __forceinline__ void stores_at(unsigned char* base, size_t stats, siz
   ss.uv = nullptr; ss.cap = cap;
 }
 
-template <bool kChecksum, uint32_t kCap>
-__global__ void __launch_bounds__(kWarps * 32) velo_cluster_kernel(const __grid_constant__ ClusterLaunch a) {
+// Everything for one (event, layer) item, by one warp.  kDefer: layers that do not fit this instance's shared memory
+// are put on a list for the instance with 512 entries (launched next) instead of taking the pool paths here.
+template <bool kChecksum, uint32_t kCap, bool kDefer>
+__device__ __forceinline__ void cluster_item(const ClusterLaunch& a, WarpSmem<kChecksum, kCap>& ws, uint32_t item) {
   constexpr uint32_t kCapSp = kCap, kCapEdges = kCap, kCapCl = kCap, kHashBits = Caps<kCap>::kHashBits;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  using WS = WarpSmem<kChecksum, kCap>;
-  WS& ws = reinterpret_cast<WS*>(smem_raw)[threadIdx.x >> 5];
   const DeviceGeometry& g = a.geo;
   const uint32_t lane = lane_id();
   const uint32_t L = g.n_layers;
-  const uint32_t item = blockIdx.x * kWarps + (threadIdx.x >> 5);
-  if (item >= a.n_events * L) return;
   const uint32_t e = item / L, layer = item % L;
 
   ClusterStore cs;
@@ -523,6 +520,10 @@ __global__ void __launch_bounds__(kWarps * 32) velo_cluster_kernel(const __grid_
   uint32_t n_cl = 0;
   bool bad_sp = false, overflow = false;
   int mode = n_sp_layer <= kCapSp ? 0 : (max_cnt <= kCapSp && n_sp_layer <= kMidCl) ? 1 : 2;
+  if (kDefer && mode != 0) {
+    if (lane == 0) a.defer_list[atomicAdd(a.defer_count, 1u)] = item;
+    return;
+  }
   if (mode == 0) {
     if (ccl_pass<kChecksum>(fast, cs, g, spw, my_sensor, my_off, cnt_k, 0, K, n_cl, bad_sp, &ws.n_edges)) {
       if (__any_sync(kFull, bad_sp) && lane == 0) atomicOr(a.status + e, ALLEN_VELO_STATUS_BAD_SP);
@@ -608,6 +609,34 @@ __global__ void __launch_bounds__(kWarps * 32) velo_cluster_kernel(const __grid_
 }
 
 
+// One warp per item of the batch, in grid order.
+template <bool kChecksum, uint32_t kCap, bool kDefer>
+__global__ void __launch_bounds__(kWarps * 32) velo_cluster_kernel(const __grid_constant__ ClusterLaunch a) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  using WS = WarpSmem<kChecksum, kCap>;
+  const uint32_t item = blockIdx.x * kWarps + (threadIdx.x >> 5);
+  if (item >= a.n_events * a.geo.n_layers) return;
+  cluster_item<kChecksum, kCap, kDefer>(a, reinterpret_cast<WS*>(smem_raw)[threadIdx.x >> 5], item);
+}
+
+// Resident warps take the deferred items from the list (a few per cent of the layers at most).
+template <bool kChecksum, uint32_t kCap>
+__global__ void __launch_bounds__(kWarps * 32) velo_cluster_list_kernel(const __grid_constant__ ClusterLaunch a) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  using WS = WarpSmem<kChecksum, kCap>;
+  WS& ws = reinterpret_cast<WS*>(smem_raw)[threadIdx.x >> 5];
+  const uint32_t n = *a.defer_count;
+#pragma unroll 1
+  for (;;) {
+    uint32_t idx = 0;
+    if (lane_id() == 0) idx = atomicAdd(a.defer_count + 1, 1u);
+    idx = __shfl_sync(kFull, idx, 0);
+    if (idx >= n) return;
+    cluster_item<kChecksum, kCap, false>(a, ws, a.defer_list[idx]);
+    __syncwarp();
+  }
+}
+
 // One warp per event: validate header and bank table once (R1), and lay out for every layer of the event what its
 // cluster warp needs: desc[item] = { first SP word of each of its sensors (index into raw) [8], SP words of each [8],
 // slab base, flags (bit 0: malformed event) }.  26 warps per event used to redo this validation each.
@@ -680,28 +709,53 @@ __global__ void __launch_bounds__(128) velo_prepare_kernel(const __grid_constant
 size_t cluster_mid_slot_bytes() { return MidSlot::kBytes; }
 size_t cluster_big_slot_bytes() { return BigSlot::kBytes; }
 
-template <bool kChecksum, uint32_t kCap>
+template <bool kChecksum, uint32_t kCap, bool kDefer>
 cudaError_t launch_cluster_instance(const ClusterLaunch& a, uint32_t grid, cudaStream_t stream) {
   const size_t smem = sizeof(WarpSmem<kChecksum, kCap>) * kWarps;
-  cudaError_t err = cudaFuncSetAttribute(velo_cluster_kernel<kChecksum, kCap>,
+  cudaError_t err = cudaFuncSetAttribute(velo_cluster_kernel<kChecksum, kCap, kDefer>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (err != cudaSuccess) return err;
-  velo_cluster_kernel<kChecksum, kCap><<<grid, kWarps * 32, smem, stream>>>(a);
+  velo_cluster_kernel<kChecksum, kCap, kDefer><<<grid, kWarps * 32, smem, stream>>>(a);
   return cudaGetLastError();
 }
 
-// `big_layers`: the batch averages more than 192 SP words per layer (the host knows the raw size): the instance with
-// 512 entries per layer in shared memory keeps such layers on chip at half the occupancy.
-cudaError_t launch_cluster(const ClusterLaunch& a, bool big_layers, cudaStream_t stream) {
+template <bool kChecksum>
+cudaError_t launch_cluster_list(const ClusterLaunch& a, uint32_t grid, cudaStream_t stream) {
+  const size_t smem = sizeof(WarpSmem<kChecksum, 512>) * kWarps;
+  cudaError_t err = cudaFuncSetAttribute(velo_cluster_list_kernel<kChecksum, 512>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (err != cudaSuccess) return err;
+  velo_cluster_list_kernel<kChecksum, 512><<<grid, kWarps * 32, smem, stream>>>(a);
+  return cudaGetLastError();
+}
+
+// prepare -> cluster kernel over all (event, layer) items [-> the 512-entry instance over the items the 256-entry one
+// deferred].  `big_layers`: the batch averages more than 192 SP words per layer (caller's hint): the instance with
+// 512 entries per layer in shared memory is used for everything, at half the occupancy.
+cudaError_t launch_cluster(const ClusterLaunch& a, bool big_layers, uint32_t n_sms, uint32_t* n_launches,
+                           cudaStream_t stream) {
+  *n_launches = 0;
   const uint32_t items = a.n_events * a.geo.n_layers;
   if (items == 0) return cudaSuccess;
   velo_prepare_kernel<<<(a.n_events + 3) / 4, 128, 0, stream>>>(a);
-  cudaError_t perr = cudaGetLastError();
-  if (perr != cudaSuccess) return perr;
+  cudaError_t err = cudaGetLastError();
+  if (err != cudaSuccess) return err;
+  ++*n_launches;
   const uint32_t grid = (items + kWarps - 1) / kWarps;
-  if (a.with_checksum)
-    return big_layers ? launch_cluster_instance<true, 512>(a, grid, stream) : launch_cluster_instance<true, 256>(a, grid, stream);
-  return big_layers ? launch_cluster_instance<false, 512>(a, grid, stream) : launch_cluster_instance<false, 256>(a, grid, stream);
+  if (big_layers) {
+    err = a.with_checksum ? launch_cluster_instance<true, 512, false>(a, grid, stream)
+                          : launch_cluster_instance<false, 512, false>(a, grid, stream);
+    ++*n_launches;
+    return err;
+  }
+  err = a.with_checksum ? launch_cluster_instance<true, 256, true>(a, grid, stream)
+                        : launch_cluster_instance<false, 256, true>(a, grid, stream);
+  if (err != cudaSuccess) return err;
+  ++*n_launches;
+  const uint32_t list_grid = min(grid, 3 * n_sms);
+  err = a.with_checksum ? launch_cluster_list<true>(a, list_grid, stream) : launch_cluster_list<false>(a, list_grid, stream);
+  ++*n_launches;
+  return err;
 }
 
 }  // namespace velo

@@ -123,6 +123,8 @@ struct ClusterLaunch {
   uint32_t* slab_base;        // [n_events*n_layers] first slab entry of the (event, layer) region
   uint32_t* desc;             // [n_events*n_layers][18] bank ranges of the layer (velo_prepare_kernel)
   uint32_t* status;           // [n_events], zeroed before
+  uint32_t* defer_list;       // [n_events*n_layers] items left to the 512-entry instance
+  uint32_t* defer_count;      // [2] list size, cursor; zeroed before
   uint32_t* big_ctr;          // slots handed out of the big pool, zeroed before
   uint32_t* mid_mask;         // [n_mid_sms] busy bits of the mid slots of every SM, zeroed before
   unsigned char* mid_pool;    // [32 * n_mid_sms] slots
@@ -130,7 +132,8 @@ struct ClusterLaunch {
   uint32_t n_mid_sms, n_big_slots;
   bool with_checksum;
 };
-cudaError_t launch_cluster(const ClusterLaunch& a, bool big_layers, cudaStream_t stream);
+cudaError_t launch_cluster(const ClusterLaunch& a, bool big_layers, uint32_t n_sms, uint32_t* n_launches,
+                           cudaStream_t stream);
 size_t cluster_mid_slot_bytes();
 size_t cluster_big_slot_bytes();
 
