@@ -63,8 +63,8 @@ size_t fixed_bytes(uint32_t n_events, uint32_t n_layers, uint32_t n_mid_sms) {
   size_t b = 0;
   b += align_up((size_t)items * 4) * 2 + align_up((size_t)items * 18 * 4);  // counts, slab_base, layer descriptors
   b += align_up(scan_state_words(items) * 8);                     // scan state (clusters)
-  b += align_up(16 + (size_t)n_mid_sms * 4);                      // big-pool counter, deferred-item counters, mid masks
-  b += align_up((size_t)items * 4);                               // deferred items of the cluster kernel
+  b += align_up(24 + (size_t)n_mid_sms * 4);                      // big-pool counter, deferred-item counters, mid masks
+  b += align_up((size_t)items * 4) * 2;                           // deferred items of the cluster kernel (two lists)
   b += align_up((size_t)n_mid_sms * 32 * cluster_mid_slot_bytes());
   b += align_up((size_t)big_slots(items) * cluster_big_slot_bytes());
   b += align_up((size_t)n_events * 8) + align_up(((size_t)n_events + 1) * 8);  // track counts, offsets
@@ -236,9 +236,10 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   uint32_t* desc = cv.take<uint32_t>((size_t)items * 18);
   unsigned long long* scan_state = cv.take<unsigned long long>(scan_state_words(items));
   // big-pool counter, deferred-item count and cursor, then the mid masks: zeroed by one memset
-  const size_t state_bytes = 16 + (size_t)h->n_mid_sms * 4;
+  const size_t state_bytes = 24 + (size_t)h->n_mid_sms * 4;
   unsigned long long* state = reinterpret_cast<unsigned long long*>(cv.take<unsigned char>(state_bytes));
   uint32_t* defer_list = cv.take<uint32_t>(items);
+  uint32_t* defer_list2 = cv.take<uint32_t>(items);
   const uint32_t n_big = big_slots(items);
   unsigned char* mid_pool = cv.take<unsigned char>((size_t)h->n_mid_sms * 32 * cluster_mid_slot_bytes());
   unsigned char* big_pool = cv.take<unsigned char>((size_t)n_big * cluster_big_slot_bytes());
@@ -291,8 +292,9 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   cl.status = oc->status;
   cl.big_ctr = reinterpret_cast<uint32_t*>(state);
   cl.defer_count = reinterpret_cast<uint32_t*>(state) + 2;
-  cl.defer_list = defer_list;
-  cl.mid_mask = reinterpret_cast<uint32_t*>(state + 2);
+  cl.defer_list[0] = defer_list;
+  cl.defer_list[1] = defer_list2;
+  cl.mid_mask = reinterpret_cast<uint32_t*>(state + 3);
   cl.mid_pool = mid_pool;
   cl.big_pool = big_pool;
   cl.n_mid_sms = h->n_mid_sms;

@@ -39,8 +39,9 @@ constexpr uint32_t kDescWords = 18;  // per (event, layer) descriptor written by
 // kCap SP words / clusters / edges per layer, 2 * kCap hash slots; two instances: 256 (nu ~ 6) and 512 (busier batches)
 template <uint32_t kCap>
 struct Caps {
-  static constexpr uint32_t kHashBits = kCap == 256 ? 9 : 10;
-  static_assert(kCap == 256 || kCap == 512, "hash bits");
+  static constexpr uint32_t kHashBits = kCap == 128 ? 8 : kCap == 256 ? 9 : 10;
+  static constexpr uint32_t kLevel = kCap == 128 ? 0 : 1;  // deferral list an instance with kDefer appends to
+  static_assert(kCap == 128 || kCap == 256 || kCap == 512, "hash bits");
 };
 // pool slots in global memory
 constexpr uint32_t kMidCl = 1024;
@@ -440,7 +441,10 @@ struct alignas(16) WarpSmem {
   uint32_t ccks[kChecksum ? kCapCl : 1];
   uint32_t n_edges;
 };
-static_assert(1024 + 6 * 256 <= 4 * 256 + 4 * (1u << 9) && 1024 + 6 * 512 <= 4 * 512 + 4 * (1u << 10), "sort scratch aliases sp + tab");
+// sort scratch (1 kB of bucket counts, then tmp / order / phis) aliases sp + tab, for 128 entries also lab
+static_assert(1024 + 6 * 128 <= 4 * 128 + 4 * (1u << 8) + 4 * 128 && 1024 + 6 * 256 <= 4 * 256 + 4 * (1u << 9) &&
+                  1024 + 6 * 512 <= 4 * 512 + 4 * (1u << 10),
+              "sort scratch aliases sp + tab (+ lab)");
 
 // Layout of the pool slots (bytes from the slot base).
 struct MidSlot {
@@ -485,10 +489,11 @@ __device__ __forceinline__ void cluster_item(const ClusterLaunch& a, WarpSmem<kC
   cs.key = ws.ckey; cs.n = ws.cn; cs.col = ws.ccol; cs.row = ws.crow; cs.cks = ws.ccks; cs.cap = kCapCl;
   SortStore ss;
   ss.cnt256 = ws.sp;
-  ss.tmp = reinterpret_cast<uint16_t*>(ws.tab);
+  ss.tmp = reinterpret_cast<uint16_t*>(ws.sp + 256);  // sp, tab, lab, edges are contiguous
   ss.order = ss.tmp + kCapCl;
   ss.phis = ss.order + kCapCl;
-  ss.uv = reinterpret_cast<float*>(ws.lab);  // lab + edges: 2 * kCapCl floats, dead once the cluster records exist
+  // lab + edges: 2 * kCapCl floats, dead once the cluster records exist (128 entries: the sort scratch reaches into lab)
+  ss.uv = kCap == 128 ? nullptr : reinterpret_cast<float*>(ws.lab);
   ss.cap = kCapCl;
 
   // ---------------- A1: the layer's bank ranges, validated and laid out by velo_prepare_kernel ----------------
@@ -521,7 +526,7 @@ __device__ __forceinline__ void cluster_item(const ClusterLaunch& a, WarpSmem<kC
   bool bad_sp = false, overflow = false;
   int mode = n_sp_layer <= kCapSp ? 0 : (max_cnt <= kCapSp && n_sp_layer <= kMidCl) ? 1 : 2;
   if (kDefer && mode != 0) {
-    if (lane == 0) a.defer_list[atomicAdd(a.defer_count, 1u)] = item;
+    if (lane == 0) a.defer_list[Caps<kCap>::kLevel][atomicAdd(a.defer_count + 2 * Caps<kCap>::kLevel, 1u)] = item;
     return;
   }
   if (mode == 0) {
@@ -619,20 +624,20 @@ __global__ void __launch_bounds__(kWarps * 32) velo_cluster_kernel(const __grid_
   cluster_item<kChecksum, kCap, kDefer>(a, reinterpret_cast<WS*>(smem_raw)[threadIdx.x >> 5], item);
 }
 
-// Resident warps take the deferred items from the list (a few per cent of the layers at most).
-template <bool kChecksum, uint32_t kCap>
+// Resident warps take the deferred items of list `kFrom` (a few per cent of the layers at most for the last list).
+template <bool kChecksum, uint32_t kCap, bool kDefer, uint32_t kFrom>
 __global__ void __launch_bounds__(kWarps * 32) velo_cluster_list_kernel(const __grid_constant__ ClusterLaunch a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   using WS = WarpSmem<kChecksum, kCap>;
   WS& ws = reinterpret_cast<WS*>(smem_raw)[threadIdx.x >> 5];
-  const uint32_t n = *a.defer_count;
+  const uint32_t n = a.defer_count[2 * kFrom];
 #pragma unroll 1
   for (;;) {
     uint32_t idx = 0;
-    if (lane_id() == 0) idx = atomicAdd(a.defer_count + 1, 1u);
+    if (lane_id() == 0) idx = atomicAdd(a.defer_count + 2 * kFrom + 1, 1u);
     idx = __shfl_sync(kFull, idx, 0);
     if (idx >= n) return;
-    cluster_item<kChecksum, kCap, false>(a, ws, a.defer_list[idx]);
+    cluster_item<kChecksum, kCap, kDefer>(a, ws, a.defer_list[kFrom][idx]);
     __syncwarp();
   }
 }
@@ -719,19 +724,34 @@ cudaError_t launch_cluster_instance(const ClusterLaunch& a, uint32_t grid, cudaS
   return cudaGetLastError();
 }
 
-template <bool kChecksum>
+template <bool kChecksum, uint32_t kCap, bool kDefer, uint32_t kFrom>
 cudaError_t launch_cluster_list(const ClusterLaunch& a, uint32_t grid, cudaStream_t stream) {
-  const size_t smem = sizeof(WarpSmem<kChecksum, 512>) * kWarps;
-  cudaError_t err = cudaFuncSetAttribute(velo_cluster_list_kernel<kChecksum, 512>,
+  const size_t smem = sizeof(WarpSmem<kChecksum, kCap>) * kWarps;
+  cudaError_t err = cudaFuncSetAttribute(velo_cluster_list_kernel<kChecksum, kCap, kDefer, kFrom>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (err != cudaSuccess) return err;
-  velo_cluster_list_kernel<kChecksum, 512><<<grid, kWarps * 32, smem, stream>>>(a);
+  velo_cluster_list_kernel<kChecksum, kCap, kDefer, kFrom><<<grid, kWarps * 32, smem, stream>>>(a);
   return cudaGetLastError();
 }
 
-// prepare -> cluster kernel over all (event, layer) items [-> the 512-entry instance over the items the 256-entry one
-// deferred].  `big_layers`: the batch averages more than 192 SP words per layer (caller's hint): the instance with
-// 512 entries per layer in shared memory is used for everything, at half the occupancy.
+template <bool kChecksum>
+cudaError_t launch_cluster_chain(const ClusterLaunch& a, uint32_t grid, uint32_t n_sms, uint32_t* n_launches,
+                                 cudaStream_t stream) {
+  cudaError_t err = launch_cluster_instance<kChecksum, 128, true>(a, grid, stream);
+  if (err != cudaSuccess) return err;
+  ++*n_launches;
+  if ((err = launch_cluster_list<kChecksum, 256, true, 0>(a, min(grid, 6 * n_sms), stream)) != cudaSuccess) return err;
+  ++*n_launches;
+  if ((err = launch_cluster_list<kChecksum, 512, false, 1>(a, min(grid, 3 * n_sms), stream)) != cudaSuccess) return err;
+  ++*n_launches;
+  return cudaSuccess;
+}
+
+// prepare -> cluster kernel with 128 entries per layer over all (event, layer) items -> the 256-entry instance over
+// the layers that one deferred -> the 512-entry instance over the layers the second deferred.  Small layers run at
+// twice the occupancy of the 256-entry instance (4.6 instead of 9.2 kB of shared memory per warp).
+// `big_layers`: the batch averages more than 192 SP words per layer (caller's hint): the instance with 512 entries
+// is used for everything.
 cudaError_t launch_cluster(const ClusterLaunch& a, bool big_layers, uint32_t n_sms, uint32_t* n_launches,
                            cudaStream_t stream) {
   *n_launches = 0;
@@ -748,14 +768,8 @@ cudaError_t launch_cluster(const ClusterLaunch& a, bool big_layers, uint32_t n_s
     ++*n_launches;
     return err;
   }
-  err = a.with_checksum ? launch_cluster_instance<true, 256, true>(a, grid, stream)
-                        : launch_cluster_instance<false, 256, true>(a, grid, stream);
-  if (err != cudaSuccess) return err;
-  ++*n_launches;
-  const uint32_t list_grid = min(grid, 3 * n_sms);
-  err = a.with_checksum ? launch_cluster_list<true>(a, list_grid, stream) : launch_cluster_list<false>(a, list_grid, stream);
-  ++*n_launches;
-  return err;
+  return a.with_checksum ? launch_cluster_chain<true>(a, grid, n_sms, n_launches, stream)
+                         : launch_cluster_chain<false>(a, grid, n_sms, n_launches, stream);
 }
 
 }  // namespace velo

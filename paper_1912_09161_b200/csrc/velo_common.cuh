@@ -123,8 +123,8 @@ struct ClusterLaunch {
   uint32_t* slab_base;        // [n_events*n_layers] first slab entry of the (event, layer) region
   uint32_t* desc;             // [n_events*n_layers][18] bank ranges of the layer (velo_prepare_kernel)
   uint32_t* status;           // [n_events], zeroed before
-  uint32_t* defer_list;       // [n_events*n_layers] items left to the 512-entry instance
-  uint32_t* defer_count;      // [2] list size, cursor; zeroed before
+  uint32_t* defer_list[2];    // [n_events*n_layers] each: items left to the 256-entry / the 512-entry instance
+  uint32_t* defer_count;      // [2][2] list size, cursor; zeroed before
   uint32_t* big_ctr;          // slots handed out of the big pool, zeroed before
   uint32_t* mid_mask;         // [n_mid_sms] busy bits of the mid slots of every SM, zeroed before
   unsigned char* mid_pool;    // [32 * n_mid_sms] slots
