@@ -23,11 +23,14 @@
 // first: in-order publication made every warp wait for its slowest predecessor — 66 % of the issued instructions
 // were the spin — so compaction moved into the track kernel, which reads every hit anyway; profiles/README.md.)
 //
-// Capacities.  FAST: the layer's SP words fit the warp's shared memory (256).  MID: they do not, but every sensor
-// does: one pass per sensor group in shared memory, cluster records and sort scratch in a pool slot in global memory.
-// BIG: everything in a (larger) pool slot in global memory.  Same code, same results, decreasing speed; a layer is
-// flagged STAGE_OVERFLOW only if it exceeds 8192 SP words or the BIG pool (counter-allocated) is exhausted.  MID
-// slots belong to resident warps (per-SM bit masks), so they never run out and nobody waits for one.
+// Capacities.  The kernel is instantiated for 128, 256 and 512 SP words / clusters / edges per layer in shared memory
+// (4.6 / 9.2 / 18 kB per warp).  Every layer is clustered by the smallest instance that holds it (FAST): an instance
+// appends the layers that are too large for it to a list, and the next larger one takes that list with resident warps.
+// Beyond 512: MID — every sensor of the layer fits: one pass per sensor group in shared memory, cluster records and
+// sort scratch in a pool slot in global memory; BIG — everything in a (larger) pool slot in global memory.  Same code,
+// same results, decreasing speed; a layer is flagged STAGE_OVERFLOW only if it exceeds 8192 SP words or the BIG pool
+// (counter-allocated) is exhausted.  MID slots belong to resident warps (per-SM bit masks), so they never run out and
+// nobody waits for one.
 #include "velo_common.cuh"
 
 namespace velo {
@@ -750,8 +753,7 @@ cudaError_t launch_cluster_chain(const ClusterLaunch& a, uint32_t grid, uint32_t
 // prepare -> cluster kernel with 128 entries per layer over all (event, layer) items -> the 256-entry instance over
 // the layers that one deferred -> the 512-entry instance over the layers the second deferred.  Small layers run at
 // twice the occupancy of the 256-entry instance (4.6 instead of 9.2 kB of shared memory per warp).
-// `big_layers`: the batch averages more than 192 SP words per layer (caller's hint): the instance with 512 entries
-// is used for everything.
+// `big_layers`: the batch averages more than 192 SP words per layer (caller's hint): the chain starts at 256 entries.
 cudaError_t launch_cluster(const ClusterLaunch& a, bool big_layers, uint32_t n_sms, uint32_t* n_launches,
                            cudaStream_t stream) {
   *n_launches = 0;
@@ -762,9 +764,14 @@ cudaError_t launch_cluster(const ClusterLaunch& a, bool big_layers, uint32_t n_s
   if (err != cudaSuccess) return err;
   ++*n_launches;
   const uint32_t grid = (items + kWarps - 1) / kWarps;
-  if (big_layers) {
-    err = a.with_checksum ? launch_cluster_instance<true, 512, false>(a, grid, stream)
-                          : launch_cluster_instance<false, 512, false>(a, grid, stream);
+  if (big_layers) {  // 256 -> 512
+    err = a.with_checksum ? launch_cluster_instance<true, 256, true>(a, grid, stream)
+                          : launch_cluster_instance<false, 256, true>(a, grid, stream);
+    if (err != cudaSuccess) return err;
+    ++*n_launches;
+    const uint32_t lg = min(grid, 3 * n_sms);
+    err = a.with_checksum ? launch_cluster_list<true, 512, false, 1>(a, lg, stream)
+                          : launch_cluster_list<false, 512, false, 1>(a, lg, stream);
     ++*n_launches;
     return err;
   }
