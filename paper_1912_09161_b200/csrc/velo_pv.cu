@@ -46,6 +46,7 @@ __global__ void __launch_bounds__(kPvWarps * 32) velo_pv_kernel(const __grid_con
   for (uint32_t b = lane; b < kPvBins + 4; b += 32) sm.h[b] = 0;
   if (lane == 0) sm.n_cand = 0;
   __syncwarp();
+  uint32_t b_lo = kPvBins, b_hi = 0;  // occupied bin range: candidates can only be within one bin of it
 #pragma unroll 1
   for (uint32_t i = lane; i < n && fits; i += 32) {
     const float x0 = a.tracks.x0[t0 + i], y0 = a.tracks.y0[t0 + i], tx = a.tracks.tx[t0 + i], ty = a.tracks.ty[t0 + i];
@@ -54,16 +55,22 @@ __global__ void __launch_bounds__(kPvWarps * 32) velo_pv_kernel(const __grid_con
     const float zp = __fdiv_rn(-__fmaf_rn(x0, tx, __fmul_rn(y0, ty)), t2);
     const float u = __fadd_rn(zp, 300.0f);
     if (!(u >= 0.0f) || !(u < (float)kPvBins)) continue;
-    atomicAdd(&sm.h[(int)floorf(u) + 2], 1u);
+    const int bin = (int)floorf(u);
+    atomicAdd(&sm.h[bin + 2], 1u);
+    b_lo = min(b_lo, (uint32_t)bin);
+    b_hi = max(b_hi, (uint32_t)bin);
   }
+  b_lo = __reduce_min_sync(kFull, b_lo);
+  b_hi = __reduce_max_sync(kFull, b_hi);
   __syncwarp();
   // ---- candidates: local maxima of (s, h), s = three-bin sum >= 4; ascending bin order by ballot
+  const uint32_t scan_lo = b_lo > 0 ? b_lo - 1 : 0, scan_hi = min(b_hi + 2, (uint32_t)kPvBins);
 #pragma unroll 1
-  for (uint32_t b0 = 0; b0 < kPvBins; b0 += 32) {
+  for (uint32_t b0 = scan_lo; b0 < scan_hi && b_lo <= b_hi; b0 += 32) {
     const uint32_t b = b0 + lane;
     bool cand = false;
     float seed = 0.0f;
-    if (b < kPvBins) {
+    if (b < scan_hi) {
       const int hmm = sm.h[b], hm = sm.h[b + 1], hc = sm.h[b + 2], hp = sm.h[b + 3], hpp = sm.h[b + 4];
       const int s = hm + hc + hp, sl = hmm + hm + hc, sr = hc + hp + hpp;
       const bool above_left = s > sl || (s == sl && hc > hm), not_below_right = s > sr || (s == sr && hc >= hp);
@@ -102,6 +109,8 @@ __global__ void __launch_bounds__(kPvWarps * 32) velo_pv_kernel(const __grid_con
         const float d = vz - k1.x;
         const float dx = k0.x + k0.z * d - vx, dy = k0.y + k0.w * d - vy;
         const float var_x = k1.z + 2.0f * d * k1.w + d * d * k2.x, var_y = k2.y + 2.0f * d * k2.z + d * d * k2.w;
+        // most tracks belong to other vertices: reject them before the two divisions (same cut, cross-multiplied)
+        if (!(dx * dx * var_y + dy * dy * var_x < kChi2Max * var_x * var_y)) continue;
         const float ix = 1.0f / var_x, iy = 1.0f / var_y;
         const float c2 = dx * dx * ix + dy * dy * iy;
         if (!(c2 < kChi2Max)) continue;
