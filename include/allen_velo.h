@@ -89,7 +89,8 @@ typedef struct {
   uint32_t capacity_tracks;
   uint32_t capacity_hits;
   uint32_t* event_offsets; /* DEVICE [n_events+1]        first track of every event */
-  uint32_t* hit_offsets;   /* DEVICE [capacity_tracks+1] first entry of hits[] of every track */
+  uint32_t* hit_offsets;   /* DEVICE [capacity_tracks+1] first entry of hits[] of every track; the last element
+                              [capacity_tracks] also receives the total number of hits (= hit_offsets[n_tracks]) */
   uint16_t* hits;          /* DEVICE [capacity_hits] */
   float* x0;               /* DEVICE [capacity_tracks] straight-line fit x(z) = x0 + tx*z, y(z) = y0 + ty*z (R6) */
   float* y0;

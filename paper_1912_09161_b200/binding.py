@@ -356,7 +356,8 @@ class StreamedVelo:
                 d_raw=torch.empty(self.max_raw, dtype=torch.uint8, device=self.device),
                 d_off=torch.empty(self.chunk_events + 1, dtype=torch.int32, device=self.device),
                 h_off=pin(self.chunk_events + 1, torch.int32), h_te=pin(self.chunk_events + 1, torch.int32),
-                h_st=pin(self.chunk_events, torch.int32), h_ho=pin(tcap + 1, torch.int32),
+                h_st=pin(self.chunk_events, torch.int32), h_ho=pin(tcap + 1, torch.int32), h_tot=pin(1, torch.int32),
+                tcap=tcap,
                 h_hits=pin(hcap, torch.int16), h_fit=[pin(tcap, torch.float32) for _ in range(4)],
                 pending=None))
         self.h2d_bytes = self.d2h_bytes = 0
@@ -370,16 +371,13 @@ class StreamedVelo:
             return None
         s["stream"].synchronize()
         n = p["n_events"]
-        nt = int(s["h_te"][n])
+        nt, nh = int(s["h_te"][n]), int(s["h_tot"][0])  # both totals came with the offsets: one wait per chunk
         with torch.cuda.stream(s["stream"]):
             s["h_ho"][:nt + 1].copy_(s["ot"].hit_offsets[:nt + 1], non_blocking=True)
-        s["stream"].synchronize()
-        nh = int(s["h_ho"][nt])
-        with torch.cuda.stream(s["stream"]):
             for hb, db in zip(s["h_fit"], (s["ot"].x0, s["ot"].y0, s["ot"].tx, s["ot"].ty)):
                 hb[:nt].copy_(db[:nt], non_blocking=True)
             s["h_hits"][:nh].copy_(s["ot"].hits[:nh], non_blocking=True)
-        self.d2h_bytes += 4 * (n + 1) + 4 * n + 4 * (nt + 1) + 16 * nt + 2 * nh
+        self.d2h_bytes += 4 * (n + 1) + 4 * n + 4 + 4 * (nt + 1) + 16 * nt + 2 * nh
         s["pending"] = None
         return dict(first_event=p["first"], n_events=n, n_tracks=nt, n_hits=nh)
 
@@ -415,6 +413,7 @@ class StreamedVelo:
                     raise RuntimeError(f"allen_velo_reconstruct failed with {rc}: {s['velo'].last_error()}")
                 s["h_te"][:n + 1].copy_(s["ot"].event_offsets[:n + 1], non_blocking=True)
                 s["h_st"][:n].copy_(s["oc"].status[:n], non_blocking=True)
+                s["h_tot"].copy_(s["ot"].hit_offsets[s["tcap"]:s["tcap"] + 1], non_blocking=True)
             self.h2d_bytes += (b1 - b0) + 4 * (n + 1)
             s["pending"] = dict(first=first, n_events=n)
         for s in self.slots:

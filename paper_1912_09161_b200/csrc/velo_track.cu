@@ -637,7 +637,11 @@ __global__ void __launch_bounds__(128) compact_tracks_kernel(const CompactTracks
       o[6] = ax; o[7] = bx; o[8] = cx; o[9] = ay; o[10] = by; o[11] = cy;
     }
   }
-  if (threadIdx.x == 0 && e + 1 == a.n_events) a.out.hit_offsets[T0 + nT] = H0 + nH;
+  if (threadIdx.x == 0 && e + 1 == a.n_events) {
+    a.out.hit_offsets[T0 + nT] = H0 + nH;
+    // the total number of hits also at a fixed place (the last element), so that a host needs one read for both totals
+    if (T0 + nT < a.out.capacity_tracks) a.out.hit_offsets[a.out.capacity_tracks] = H0 + nH;
+  }
 }
 
 // One thread per event: class of the event (which instance searches it, or copy only / nothing) and the event lists
