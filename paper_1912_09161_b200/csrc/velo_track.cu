@@ -315,15 +315,30 @@ __device__ __forceinline__ void track_event(const TrackLaunch& a, uint32_t e, Sm
       if (!seeding || (wb & kUsedBit)) continue;
       const int w = P.w_seed_phi16, phb = phi_of(wb);
       uint32_t ia = lower_bound_phi(bucketA, recA, nA, wrap16(phb - w));
+      // the window is walked in runs of up to 32 hits: a bit mask of the unused ones, ONE reservation in the list per
+      // run, then the entries are written from the mask (no list atomic per doublet)
+      bool more = true;
 #pragma unroll 1
-      for (uint32_t k = 0; k < nA; ++k, ++ia) {
-        if (ia >= nA) ia -= nA;
-        const uint32_t wa = recA[ia].w;
-        const int d = wrap16(phi_of(wa) - phb);
-        if (d > w || d < -w) break;
-        if (wa & kUsedBit) continue;
-        const uint32_t pos = atomicAdd(&sm.n_doublets, 1u);
-        if (pos < (uint32_t)C::kCapDoublets) sm.doublets[pos] = kb | (ia << 16);  // else: S2 enumerates again
+      for (uint32_t k = 0; k < nA && more;) {
+        const uint32_t ia0 = ia;
+        uint32_t mask = 0, run = 0;
+#pragma unroll 1
+        for (; run < 32 && k < nA; ++run, ++k, ++ia) {
+          if (ia >= nA) ia -= nA;
+          const uint32_t wa = recA[ia].w;
+          const int d = wrap16(phi_of(wa) - phb);
+          if (d > w || d < -w) { more = false; break; }
+          if (!(wa & kUsedBit)) mask |= 1u << run;
+        }
+        if (mask) {
+          uint32_t pos = atomicAdd(&sm.n_doublets, (uint32_t)__popc(mask));
+#pragma unroll 1
+          for (; mask; mask &= mask - 1, ++pos) {
+            uint32_t a_idx = ia0 + (uint32_t)__ffs(mask) - 1u;
+            if (a_idx >= nA) a_idx -= nA;
+            if (pos < (uint32_t)C::kCapDoublets) sm.doublets[pos] = kb | (a_idx << 16);  // else: S2 enumerates again
+          }
+        }
       }
     }
     tsync<C>();  // B2
