@@ -344,6 +344,7 @@ __device__ __forceinline__ void track_event(const TrackLaunch& a, uint32_t e, Sm
     tsync<C>();  // B2
     // ---- T2 resolve: the minimal claim wins the hit (track keys are unique, so the low half of the claim names the
     //      winner); everyone else counts a miss
+    uint32_t my_min_active = 0xFFFFFFFFu;  // lowest track slot of this thread that stays active
 #pragma unroll 1
     for (uint32_t t = first + tid; t < n_tracks; t += C::kThreads) {
       const uint32_t st = sm.tstate[t];
@@ -374,17 +375,19 @@ __device__ __forceinline__ void track_event(const TrackLaunch& a, uint32_t e, Sm
         link[cg] = (uint16_t)q;
         const uint32_t nh = ((st >> 8) & 0x7Fu) + 1u;
         sm.tstate[t] = (cg << 16) | (st & 0x8000u) | (nh << 8);
-        atomicMin(&sm.min_active[(i - 1) & 1], t);
+        my_min_active = min(my_min_active, t);
       } else {
         const uint32_t m = (st & 0xFFu) + 1u;
         if (m > (uint32_t)P.max_skipped) {
           sm.tstate[t] = st | 0xFFu;
         } else {
           sm.tstate[t] = (st & 0xFFFFFF00u) | m;
-          atomicMin(&sm.min_active[(i - 1) & 1], t);
+          my_min_active = min(my_min_active, t);
         }
       }
     }
+    my_min_active = __reduce_min_sync(kFull, my_min_active);  // one shared-memory atomic per warp, not per track
+    if (lane == 0 && my_min_active != 0xFFFFFFFFu) atomicMin(&sm.min_active[(i - 1) & 1], my_min_active);
     tsync<C>();  // B3
 
     // ---- T3/S2: one thread per doublet; if the list overflowed, one thread per b walks its doublets itself
