@@ -2,7 +2,7 @@
 // point of closest approach of tracks to the beamline, where a cluster indicates a PV candidate ... every track is
 // assigned to every vertex based on a weight, so that all candidates can be fitted in parallel"; R10).
 //
-// One warp per event.  Seeding is integer work on fp32 values that are bit-identical to the oracle's (normative
+// One CTA of four warps per event; the warps share the histogram and take the candidates in turn.  Seeding is integer work on fp32 values that are bit-identical to the oracle's (normative
 // operations on the straight-line fit), so the candidates are exactly the oracle's; the weighted fits (all tracks to
 // every candidate, 8 passes of Tukey-weighted least squares on the Kalman states) run in fp32, lanes over tracks,
 // sums by warp shuffles.
@@ -22,7 +22,7 @@ struct PvSmem {
   float seed[kPvCand];
   float vx[kPvCand], vy[kPvCand], vz[kPvCand], sw[kPvCand], chi2[kPvCand];
   uint32_t nw[kPvCand];     // tracks with w > 0; 0xFFFFFFFF: fit failed
-  uint32_t n_cand;
+  uint32_t n_cand, b_lo, b_hi;
 };
 
 __device__ __forceinline__ float warp_sum(float v) {
@@ -32,23 +32,21 @@ __device__ __forceinline__ float warp_sum(float v) {
 }
 
 __global__ void __launch_bounds__(kPvWarps * 32) velo_pv_kernel(const __grid_constant__ PvLaunch a) {
-  __shared__ PvSmem smem[kPvWarps];
-  PvSmem& sm = smem[threadIdx.x >> 5];
-  const uint32_t lane = lane_id();
-  const uint32_t e = blockIdx.x * kPvWarps + (threadIdx.x >> 5);
-  if (e >= a.n_events) return;
+  __shared__ PvSmem sm;
+  const uint32_t lane = lane_id(), warp = threadIdx.x >> 5, tid = threadIdx.x;
+  const uint32_t e = blockIdx.x;
   const uint32_t t0 = a.tracks.event_offsets[e], n = a.tracks.event_offsets[e + 1] - t0;
   const bool fits = (unsigned long long)t0 + n <= a.tracks.capacity_tracks;  // else the tracks were not written
   float* out = a.out.vertices + (size_t)e * a.out.max_per_event * 8;
 
   // ---- 1, 2: histogram of the z of closest approach to the beam line (normative fp32 operations)
 #pragma unroll 1
-  for (uint32_t b = lane; b < kPvBins + 4; b += 32) sm.h[b] = 0;
-  if (lane == 0) sm.n_cand = 0;
-  __syncwarp();
+  for (uint32_t b = tid; b < kPvBins + 4; b += kPvWarps * 32) sm.h[b] = 0;
+  if (tid == 0) { sm.n_cand = 0; sm.b_lo = kPvBins; sm.b_hi = 0; }
+  __syncthreads();
   uint32_t b_lo = kPvBins, b_hi = 0;  // occupied bin range: candidates can only be within one bin of it
 #pragma unroll 1
-  for (uint32_t i = lane; i < n && fits; i += 32) {
+  for (uint32_t i = tid; i < n && fits; i += kPvWarps * 32) {
     const float x0 = a.tracks.x0[t0 + i], y0 = a.tracks.y0[t0 + i], tx = a.tracks.tx[t0 + i], ty = a.tracks.ty[t0 + i];
     const float t2 = __fmaf_rn(tx, tx, __fmul_rn(ty, ty));
     if (!(t2 >= 1e-8f)) continue;
@@ -62,11 +60,14 @@ __global__ void __launch_bounds__(kPvWarps * 32) velo_pv_kernel(const __grid_con
   }
   b_lo = __reduce_min_sync(kFull, b_lo);
   b_hi = __reduce_max_sync(kFull, b_hi);
-  __syncwarp();
+  if (lane == 0 && b_lo <= b_hi) { atomicMin(&sm.b_lo, b_lo); atomicMax(&sm.b_hi, b_hi); }
+  __syncthreads();
+  b_lo = sm.b_lo;
+  b_hi = sm.b_hi;
   // ---- candidates: local maxima of (s, h), s = three-bin sum >= 4; ascending bin order by ballot
   const uint32_t scan_lo = b_lo > 0 ? b_lo - 1 : 0, scan_hi = min(b_hi + 2, (uint32_t)kPvBins);
 #pragma unroll 1
-  for (uint32_t b0 = scan_lo; b0 < scan_hi && b_lo <= b_hi; b0 += 32) {
+  for (uint32_t b0 = scan_lo; b0 < scan_hi && b_lo <= b_hi && warp == 0; b0 += 32) {  // warp 0 lists the candidates
     const uint32_t b = b0 + lane;
     bool cand = false;
     float seed = 0.0f;
@@ -87,13 +88,14 @@ __global__ void __launch_bounds__(kPvWarps * 32) velo_pv_kernel(const __grid_con
     if (lane == 0) sm.n_cand = base + __popc(ballot);
     __syncwarp();
   }
+  __syncthreads();
   const uint32_t n_cand = min(sm.n_cand, (uint32_t)kPvCand);
-  if (sm.n_cand > (uint32_t)kPvCand && lane == 0) atomicOr(a.status + e, ALLEN_VELO_STATUS_STAGE_OVERFLOW);
+  if (sm.n_cand > (uint32_t)kPvCand && tid == 0) atomicOr(a.status + e, ALLEN_VELO_STATUS_STAGE_OVERFLOW);
 
   // ---- 3: every candidate is fitted with all tracks (lanes over tracks)
   const float* K = a.tracks.kalman + 12 * (size_t)t0;
 #pragma unroll 1
-  for (uint32_t c = 0; c < n_cand; ++c) {
+  for (uint32_t c = warp; c < n_cand; c += kPvWarps) {  // the warps take the candidates in turn
     float vx = 0.0f, vy = 0.0f, vz = sm.seed[c], sw = 0.0f, chi2 = 0.0f;
     uint32_t nw = 0;
     bool ok = true;
@@ -137,7 +139,8 @@ __global__ void __launch_bounds__(kPvWarps * 32) velo_pv_kernel(const __grid_con
       sm.nw[c] = (ok && sw >= 3.0f) ? nw : 0xFFFFFFFFu;
     }
   }
-  __syncwarp();
+  __syncthreads();
+  if (warp != 0) return;
   // ---- 4: drop duplicates (another accepted vertex within 1 mm in z with a sum w more than 0.1 % larger; within
   //         0.1 %, i.e. two candidates that converged to the same vertex: the earlier wins),
   //         write in candidate order
@@ -170,7 +173,7 @@ __global__ void __launch_bounds__(kPvWarps * 32) velo_pv_kernel(const __grid_con
 
 cudaError_t launch_pv(const PvLaunch& a, cudaStream_t stream) {
   if (a.n_events == 0) return cudaSuccess;
-  velo_pv_kernel<<<(a.n_events + kPvWarps - 1) / kPvWarps, kPvWarps * 32, 0, stream>>>(a);
+  velo_pv_kernel<<<a.n_events, kPvWarps * 32, 0, stream>>>(a);
   return cudaGetLastError();
 }
 

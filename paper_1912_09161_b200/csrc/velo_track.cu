@@ -13,8 +13,8 @@
 //    scans b's window on layer C; the per-b argmin is a 64-bit shared-memory atomicMin on (bits(S), a, c);
 //  * all conflict rules are order-independent minima on packed keys (bits(S) << 32 | index): no "first thread wins",
 //    so the result is exactly the oracle's whatever the thread schedule;
-//  * compaction of the clusters (A9) rides along: in the first instance a fifth warp copies the event's layers from
-//    the cluster kernel's slab to their final place while the four tracking warps (own named barrier) search;
+//  * compaction of the clusters (A9) rides along: an extra warp copies the event's layers from the cluster kernel's
+//    slab to their final place while the tracking warps (own named barrier) search;
 //  * the kernel is instantiated for three staging capacities (256 / 512 / 1024 hits per layer); every event is taken
 //    by the smallest instance it fits, and an instance that runs out of track slots hands the event to the next one.
 #include <cuda_pipeline.h>
