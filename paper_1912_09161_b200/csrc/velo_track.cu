@@ -58,10 +58,10 @@ struct Cfg {
 #define VELO_TRK_S_DOUBLETS 576
 #endif
 using CfgS = Cfg<VELO_TRK_S_THREADS, 256, VELO_TRK_S_TRACKS, VELO_TRK_S_DOUBLETS, 0, false, true>;
-using CfgM = Cfg<256, 512, 1024, 2304, 1, false, true>;
+using CfgM = Cfg<256, 512, 1024, 4096, 1, false, true>;
 using CfgL = Cfg<512, 1024, 2048, 2048, 2, true, true>;
 // second pass for events a smaller instance ran out of track slots on: their clusters are already in the output
-using CfgMr = Cfg<256, 512, 1024, 2304, 1, false, false>;
+using CfgMr = Cfg<256, 512, 1024, 4096, 1, false, false>;
 using CfgLr = Cfg<512, 1024, 2048, 2048, 2, true, false>;
 
 // class of an event (TrackLaunch::level), set by classify_events_kernel
