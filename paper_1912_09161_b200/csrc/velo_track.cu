@@ -82,6 +82,7 @@ struct Smem {
   uint32_t lo[kMaxLayers + 1];
   uint32_t src[kMaxLayers];  // first entry of every layer in the arrays X, Y, Z, PHI are read from
   uint32_t warp_tot[C::kRoundsB > C::kRoundsT ? C::kRoundsB : C::kRoundsT][C::kWarps];
+  uint32_t ovf[(C::kCap + 31) / 32];   // middle hits whose doublets did not all fit the list (S2 walks those itself)
   uint32_t n_doublets;
   uint32_t min_active[2];
   uint32_t flags;
@@ -218,6 +219,7 @@ __device__ __forceinline__ void track_event(const TrackLaunch& a, uint32_t e, Sm
   const uint32_t co = a.clusters.event_offsets[e];
   load_offsets<C>(a, e, sm, co);
   if (tid == 0) { sm.flags = 0; sm.min_active[0] = 0; sm.min_active[1] = 0; sm.n_doublets = 0; }
+  if (tid < (uint32_t)(C::kCap + 31) / 32) sm.ovf[tid] = 0;
   __syncthreads();
   if (C::kCopier && tid >= (uint32_t)C::kThreads) {
     // copier warp: layers in the order the search stages them (their slab lines are then in L2 for both readers)
@@ -332,11 +334,12 @@ __device__ __forceinline__ void track_event(const TrackLaunch& a, uint32_t e, Sm
         }
         if (mask) {
           uint32_t pos = atomicAdd(&sm.n_doublets, (uint32_t)__popc(mask));
+          if (pos + (uint32_t)__popc(mask) > (uint32_t)C::kCapDoublets) atomicOr(&sm.ovf[kb >> 5], 1u << (kb & 31u));
 #pragma unroll 1
           for (; mask; mask &= mask - 1, ++pos) {
             uint32_t a_idx = ia0 + (uint32_t)__ffs(mask) - 1u;
             if (a_idx >= nA) a_idx -= nA;
-            if (pos < (uint32_t)C::kCapDoublets) sm.doublets[pos] = kb | (a_idx << 16);  // else: S2 enumerates again
+            if (pos < (uint32_t)C::kCapDoublets) sm.doublets[pos] = kb | (a_idx << 16);  // else: S2 walks this b again
           }
         }
       }
@@ -390,28 +393,30 @@ __device__ __forceinline__ void track_event(const TrackLaunch& a, uint32_t e, Sm
     if (lane == 0 && my_min_active != 0xFFFFFFFFu) atomicMin(&sm.min_active[(i - 1) & 1], my_min_active);
     tsync<C>();  // B3
 
-    // ---- T3/S2: one thread per doublet; if the list overflowed, one thread per b walks its doublets itself
-    if (sm.n_doublets <= (uint32_t)C::kCapDoublets) {
-      const uint32_t nd = sm.n_doublets;
+    // ---- T3/S2: one thread per listed doublet; middle hits whose doublets did not all fit the list walk their phi
+    //      window themselves (a doublet evaluated twice gives the same key: the argmin does not care)
+    {
+      const uint32_t n_listed = sm.n_doublets, nd = min(n_listed, (uint32_t)C::kCapDoublets);
 #pragma unroll 1
       for (uint32_t d = tid; d < nd; d += C::kThreads) {
         const uint32_t v = sm.doublets[d];
         process_doublet(c, recA, recB, recC, bucketC, nC, v & 0xFFFFu, v >> 16);
       }
-    } else {
+      if (n_listed > (uint32_t)C::kCapDoublets) {  // block-uniform
 #pragma unroll 1
-      for (uint32_t kb = tid; kb < nB; kb += C::kThreads) {
-        const uint32_t wb = recB[kb].w;
-        if (wb & kUsedBit) continue;
-        const int w = P.w_seed_phi16, phb = phi_of(wb);
-        uint32_t ia = lower_bound_phi(bucketA, recA, nA, wrap16(phb - w));
+        for (uint32_t kb = tid; kb < nB; kb += C::kThreads) {
+          if (!(sm.ovf[kb >> 5] >> (kb & 31u) & 1u)) continue;
+          const uint32_t wb = recB[kb].w;
+          const int w = P.w_seed_phi16, phb = phi_of(wb);
+          uint32_t ia = lower_bound_phi(bucketA, recA, nA, wrap16(phb - w));
 #pragma unroll 1
-        for (uint32_t k = 0; k < nA; ++k, ++ia) {
-          if (ia >= nA) ia -= nA;
-          const uint32_t wa = recA[ia].w;
-          const int d = wrap16(phi_of(wa) - phb);
-          if (d > w || d < -w) break;
-          if (!(wa & kUsedBit)) process_doublet(c, recA, recB, recC, bucketC, nC, kb, ia);
+          for (uint32_t k = 0; k < nA; ++k, ++ia) {
+            if (ia >= nA) ia -= nA;
+            const uint32_t wa = recA[ia].w;
+            const int d = wrap16(phi_of(wa) - phb);
+            if (d > w || d < -w) break;
+            if (!(wa & kUsedBit)) process_doublet(c, recA, recB, recC, bucketC, nC, kb, ia);
+          }
         }
       }
     }
@@ -419,6 +424,7 @@ __device__ __forceinline__ void track_event(const TrackLaunch& a, uint32_t e, Sm
 
     // ---- T4a: every b with a triplet claims its a and its c with (bits(S), b)
     if (tid == 0) sm.n_doublets = 0;  // S2 is over; the next S1 starts after two more barriers
+    if (tid < (uint32_t)(C::kCap + 31) / 32) sm.ovf[tid] = 0;
     // layer A is done with (T4 reads only B and C): its ring slot takes the next layer, needed at the top of the
     // next iteration; the copy runs behind T4
     if (i >= 3) stage_layer(c, (uint32_t)i - 3);
