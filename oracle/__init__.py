@@ -63,6 +63,8 @@ def lib():
         L.oracle_fit.argtypes = [ctypes.c_uint32] + [ctypes.c_void_p] * 4
         L.oracle_kalman.argtypes = [ctypes.c_uint32] + [ctypes.c_void_p] * 5 + [ctypes.c_double, ctypes.c_void_p]
         L.oracle_pvs.argtypes = [ctypes.c_uint32] + [ctypes.c_void_p] * 9 + [ctypes.c_int]
+        L.oracle_pv_candidates.restype = ctypes.c_uint32
+        L.oracle_pv_candidates.argtypes = [ctypes.c_uint32] + [ctypes.c_void_p] * 8 + [ctypes.c_uint32]
         L.oracle_run.restype = ctypes.c_void_p
         L.oracle_run.argtypes = [ctypes.POINTER(_Geometry), ctypes.c_void_p, ctypes.c_void_p, ctypes.c_uint32,
                                  ctypes.c_uint32]
@@ -253,6 +255,17 @@ def find_pvs(track_offsets, x0, y0, tx, ty, kal, iterations: int = 8):
     counts, cands = np.zeros(n, np.uint32), np.zeros(n, np.uint32)
     lib().oracle_pvs(n, _p(to), _p(x0), _p(y0), _p(tx), _p(ty), _p(kal), _p(out), _p(counts), _p(cands), iterations)
     return out, counts, cands
+
+
+def pv_candidates(x0, y0, tx, ty, kal, cap: int = 300):
+    """O8 for ONE event with every candidate as it stands before the duplicate removal of step 4 (R10).
+    Returns (vertices [n, 8], candidates [m, 6]: z_seed, x, y, z, sum_w, ok)."""
+    x0, y0, tx, ty = (np.ascontiguousarray(a, np.float32) for a in (x0, y0, tx, ty))
+    kal = np.ascontiguousarray(kal, np.float64)
+    out, cand, m = np.zeros((PV_MAX, 8), np.float64), np.zeros((cap, 6), np.float64), ctypes.c_uint32(0)
+    n = lib().oracle_pv_candidates(len(x0), _p(x0), _p(y0), _p(tx), _p(ty), _p(kal), _p(out), ctypes.byref(m), _p(cand),
+                                   cap)
+    return out[:n], cand[:min(m.value, cap)]
 
 
 def pvs_of(result: "Result", pitch: float):

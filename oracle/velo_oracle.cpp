@@ -520,8 +520,11 @@ void kalman_track(uint32_t n, const float* x, const float* y, const float* z, do
 constexpr int kPvBins = 600;
 constexpr int kPvMax = 32;
 
+// cand_out (optional, pins only): every candidate as it stands after step 3, before the duplicate removal of step 4:
+// rows of z_seed, x, y, z, sum_w, ok (1 = fit converged and sum w >= 3), at most cand_cap rows.
 uint32_t find_pvs(uint32_t n, const float* x0, const float* y0, const float* tx, const float* ty, const double* kal,
-                  double* out /* [kPvMax][8] */, uint32_t* n_candidates, int n_iter = 8) {
+                  double* out /* [kPvMax][8] */, uint32_t* n_candidates, int n_iter = 8, double* cand_out = nullptr,
+                  uint32_t cand_cap = 0) {
   int h[kPvBins + 2] = {0};  // h[b + 1] = bin b; guard bins at both ends
   for (uint32_t i = 0; i < n; ++i) {
     const float t2 = std::fmaf(tx[i], tx[i], ty[i] * ty[i]);
@@ -578,6 +581,11 @@ uint32_t find_pvs(uint32_t n, const float* x0, const float* y0, const float* tx,
     }
     c.v[0] = vx; c.v[1] = vy; c.v[2] = vz;
     c.ok = c.ok && c.sw >= 3.0;
+  }
+  for (size_t i = 0; cand_out && i < cands.size() && i < cand_cap; ++i) {
+    double* o = cand_out + 6 * i;
+    o[0] = cands[i].z_seed; o[1] = cands[i].v[0]; o[2] = cands[i].v[1]; o[3] = cands[i].v[2]; o[4] = cands[i].sw;
+    o[5] = cands[i].ok ? 1.0 : 0.0;
   }
   uint32_t n_out = 0;
   for (size_t i = 0; i < cands.size(); ++i) {
@@ -659,6 +667,15 @@ void oracle_pvs(uint32_t n_events, const uint32_t* track_offsets, const float* x
     counts[e] = find_pvs(n, x0 + t0, y0 + t0, tx + t0, ty + t0, kal + 12 * (size_t)t0, out + (size_t)e * kPvMax * 8,
                          candidates + e, n_iter);
   }
+}
+
+// O8 for ONE event, also returning every candidate before step 4 (cand [cand_cap][6]: z_seed, x, y, z, sum_w, ok).
+// Returns the number of vertices; *n_candidates = histogram peaks.  Used by the pins of step 4 and by the parity test's
+// near-cut accounting.
+uint32_t oracle_pv_candidates(uint32_t n, const float* x0, const float* y0, const float* tx, const float* ty,
+                              const double* kal, double* out /* [32][8] */, uint32_t* n_candidates, double* cand,
+                              uint32_t cand_cap) {
+  return find_pvs(n, x0, y0, tx, ty, kal, out, n_candidates, 8, cand, cand_cap);
 }
 
 void* oracle_run(const Geometry* g, const uint8_t* raw, const uint32_t* event_offsets, uint32_t n_events,

@@ -112,12 +112,27 @@ def fit_close(got4, ref4, rel=1e-5):
         np.abs(gty - ty) <= slope_tol)
 
 
-def compare_tracks(got, ref, near_cut_per_event=None):
+def compare_tracks(got, ref, near_cut=None):
     """Compare Tracks as canonically sorted hit sets per event, then fit parameters of identical tracks.
 
-    Returns dict(n_ref, n_got, mismatched_tracks, near_cut_mismatched_tracks, hard_mismatched_tracks, bad_fits).
+    `near_cut`: the oracle.Result of the reference (its near-cut log, R7) or None.  A mismatching track counts as
+    "near-cut" only if the oracle logged a decision within 1e-4 of a cut that touches one of the hits on which the two
+    track sets of that event differ, or a hit of an EARLIER iteration of the same event (iterations run from the last
+    layer down, hit indices grow with the layer: a logged hit with an index above the lowest differing hit), from which
+    the difference can cascade; every other mismatch is a hard failure.
+
+    Returns dict(n_ref, n_got, mismatched_tracks, near_cut_mismatched_tracks, hard_mismatched_tracks, bad_fits,
+    near_cut_decisions).
     """
     n_events = len(ref.event_offsets) - 1
+    logged = [()] * n_events
+    n_decisions = 0
+    if near_cut is not None:
+        n_decisions = int(near_cut.near_cut_per_event.sum())
+        order = np.argsort(near_cut.near_cut_hit_event, kind="stable")
+        ev, idx = near_cut.near_cut_hit_event[order], near_cut.near_cut_hit_index[order]
+        first = np.searchsorted(ev, np.arange(n_events + 1))
+        logged = [idx[first[e]:first[e + 1]] for e in range(n_events)]
     mism = near = bad_fit = 0
     for e in range(n_events):
         def table(t):
@@ -131,14 +146,15 @@ def compare_tracks(got, ref, near_cut_per_event=None):
         diff = set(tg) ^ set(tr)
         if diff:
             mism += len(diff)
-            if near_cut_per_event is not None and near_cut_per_event[e] > 0:
+            differing = set(h for hs in diff for h in hs)
+            if len(logged[e]) and (differing & set(int(h) for h in logged[e]) or int(max(logged[e])) > min(differing)):
                 near += len(diff)
         for hs in set(tg) & set(tr):
             i, j = tg[hs], tr[hs]
             ok = fit_close((got.x0[i], got.y0[i], got.tx[i], got.ty[i]), (ref.x0[j], ref.y0[j], ref.tx[j], ref.ty[j]))
             bad_fit += int(not ok)
     return dict(n_ref=len(ref.x0), n_got=len(got.x0), mismatched_tracks=mism, near_cut_mismatched_tracks=near,
-                hard_mismatched_tracks=mism - near, bad_fits=bad_fit)
+                hard_mismatched_tracks=mism - near, bad_fits=bad_fit, near_cut_decisions=n_decisions)
 
 
 # ------------------------------------------------------------------------------------------------

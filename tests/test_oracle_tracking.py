@@ -211,3 +211,85 @@ def test_weak_three_hit_tracks_are_dropped_and_missed_layers_close_tracks():
     phi = np.array([oracle.phi16(a, b) for a, b in zip(x, y)], np.int16)
     assert oracle.search_hits(x, y, zs, phi, lo).tracks.hit_sets(0) == [(2, 3, 4)]
     assert oracle.search_hits(x, y, zs, phi, lo, dict(P, max_skipped=2)).tracks.hit_sets(0) == [(0, 1, 2, 3, 4)]
+
+
+# ------------------------------------------------------------------------------------------------
+# Near-cut accounting (R7; BASELINE.json: "decisions falling within 1e-4 of a window cut ... are counted and
+# reported").  Hand cases: one a (layer 2), one b (layer 1), one or two c (layer 0); the expected counts follow from
+# R7's three rules: a value within relative 1e-4 of its cut, |dphi| in {w, w + 1}, a runner-up within 1e-4 of the winner.
+# ------------------------------------------------------------------------------------------------
+def _abc(yc=0.02, phi_a=0, phi_c=(0,), xc=(0.0,)):
+    """a = (10, 5, 50), b = (9, 4.5, 25) -> slopes 0.04, 0.02; prediction at z = 0: (8, 4); c = (8 + xc, 4 + yc, 0)."""
+    n_c = len(xc)
+    x = np.array([8.0 + v for v in xc] + [9.0, 10.0], np.float32)
+    y = np.array([4.0 + yc] * n_c + [4.5, 5.0], np.float32)
+    z = np.array([0.0] * n_c + [25.0, 50.0], np.float32)
+    phi = np.array(list(phi_c) + [0, phi_a], np.int16)
+    lo = np.array([0, n_c, n_c + 1, n_c + 2], np.uint32)
+    return x, y, z, phi, lo
+
+
+def _near(args, params=None):
+    res = oracle.search_hits(*args, dict(P, **(params or {})))
+    return int(res.near_cut_per_event[0]), sorted(res.near_cut_hit_index.tolist()), res.tracks.hit_sets(0)
+
+
+def test_near_cut_counter_far_from_every_cut_is_zero():
+    # S = 0.02^2 = 4e-4: far below s_weak = 7.8e-3; slopes 0.04 / 0.02 against 0.4; all dphi = 0
+    assert _near(_abc()) == (0, [], [(0, 1, 2)])
+
+
+@pytest.mark.parametrize("d,count,found", [(511, 0, True), (512, 1, True), (513, 1, False), (514, 0, False),
+                                           (-512, 1, True), (-513, 1, False)])
+def test_near_cut_counts_phi_differences_at_the_window_edge(d, count, found):
+    # |dphi(a, b)| = w and w + 1 are the two values "within 1e-4 rad of the window cut" (1 LSB = 9.6e-5 rad)
+    n, hits, tracks = _near(_abc(phi_a=d))
+    assert (n, hits, tracks) == (count, [2] * count, [(0, 1, 2)] if found else [])
+    n, hits, tracks = _near(_abc(phi_c=(d,)))
+    assert (n, hits, tracks) == (count, [0] * count, [(0, 1, 2)] if found else [])
+
+
+@pytest.mark.parametrize("rel,count,found", [(5e-5, 1, False), (-5e-5, 1, True), (3e-4, 0, False), (-3e-4, 0, True)])
+def test_near_cut_counts_values_within_1e_4_of_a_cut(rel, count, found):
+    args = _abc()
+    x, y, z = args[:3]
+    S = oracle.scatter((x[2], y[2], z[2]), (x[1], y[1], z[1]), (x[0], y[0], z[0]))
+    assert S == pytest.approx(4e-4, rel=1e-3)
+    # scatter against s_seed: the cut sits at S / (1 + rel), i.e. S exceeds it by `rel` (relative)
+    n, hits, tracks = _near(args, dict(s_seed=S / (1 + rel), s_weak=1.0))
+    assert (n, hits, tracks) == (count, [1] * count, [(0, 1, 2)] if found else [])
+    # three-hit track against s_weak at T5 (seed accepted far from s_seed)
+    n, hits, tracks = _near(args, dict(s_weak=S / (1 + rel)))
+    assert (n, hits, tracks) == (count, [1] * count, [(0, 1, 2)] if found else [])
+    # slope of a -> b against max_slope: tx = 0.04 exactly at the cut, ty = 0.02 far from it
+    tx = (np.float32(9.0) - np.float32(10.0)) / (np.float32(25.0) - np.float32(50.0))
+    n, hits, tracks = _near(args, dict(max_slope=float(tx) / (1 + rel)))
+    assert (n, hits, tracks) == (count, [2] * count, [(0, 1, 2)] if found else [])
+
+
+def test_near_cut_counts_a_runner_up_within_1e_4():
+    # two candidates c at mirror positions about the prediction: equal scatter -> one tie, logged on b; the lower index wins
+    n, hits, tracks = _near(_abc(yc=0.0, xc=(-0.01, 0.01), phi_c=(0, 0)))
+    assert (n, hits) == (1, [2]) and tracks == [(0, 2, 3)]
+    # 2 % apart in distance (4 % in scatter): no tie
+    n, hits, tracks = _near(_abc(yc=0.0, xc=(-0.0102, 0.01), phi_c=(0, 0)))
+    assert (n, hits) == (0, []) and tracks == [(1, 2, 3)]
+
+
+def test_near_cut_counts_forwarding_decisions():
+    # four layers: seed on layers 3, 2, 1 (exact line), forwarding to a hit on layer 0 that is 0.1 mm off in y
+    x = np.array([7.0, 8.0, 9.0, 10.0], np.float32)
+    y = np.array([3.6, 4.0, 4.5, 5.0], np.float32)
+    z = np.array([-25.0, 0.0, 25.0, 50.0], np.float32)
+    lo = np.arange(5, dtype=np.uint32)
+    S = oracle.scatter((x[2], y[2], z[2]), (x[1], y[1], z[1]), (x[0], y[0], z[0]))
+    assert S == pytest.approx(0.01, rel=1e-3)
+    phi0 = np.zeros(4, np.int16)
+    assert _near((x, y, z, phi0, lo)) == (0, [], [(0, 1, 2, 3)])
+    assert _near((x, y, z, phi0, lo), dict(s_fwd=S / (1 - 5e-5))) == (1, [0], [(0, 1, 2, 3)])
+    n, hits, tracks = _near((x, y, z, phi0, lo), dict(s_fwd=S / (1 + 5e-5)))
+    assert (n, hits, tracks) == (1, [0], [(1, 2, 3)])
+    for d, count, found in ((512, 1, True), (513, 1, False), (520, 0, False)):
+        phi = np.array([d, 0, 0, 0], np.int16)
+        n, hits, tracks = _near((x, y, z, phi, lo))
+        assert (n, hits) == (count, [0] * count) and tracks == ([(0, 1, 2, 3)] if found else [(1, 2, 3)])
