@@ -12,8 +12,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "_allen_velo.so")
-SOURCES = ["allen_velo.cu", "velo_cluster.cu", "velo_scan.cu", "velo_track.cu", "velo_pv.cu"]
-HEADERS = ["velo_common.cuh", os.path.join("..", "..", "include", "allen_velo.h")]
+SOURCES = ["allen_velo.cu", "velo_cluster.cu", "velo_scan.cu", "velo_track.cu", "velo_track_flat.cu", "velo_pv.cu"]
+HEADERS = ["velo_common.cuh", "velo_track.cuh", os.path.join("..", "..", "include", "allen_velo.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -38,11 +38,11 @@ const char* const kKernelNames[kKernels] = {"velo_cluster", "scan_clusters", "ve
 constexpr size_t kAlign = 256;
 inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
-// bytes per slab entry (cluster SoA incl. checksum), tracking scratch per cluster (link, hits_slab) and per track
-// slot (trk_hitoff, trk_fit; one slot per 3 clusters)
-constexpr size_t kSlabEntryBytes = 7 * 4 + 2 + 4;
+// bytes per slab entry (two 16-byte records + checksum), tracking scratch per cluster (link, hits_slab) and per track
+// slot (trk_hitoff, trk_fit, trk_final; one slot per 3 clusters)
+constexpr size_t kSlabEntryBytes = 16 + 16 + 4;
 constexpr size_t kTrackScratchBytes = 2 + 2;
-constexpr size_t kTrackSlotBytes = 4 + 16;
+constexpr size_t kTrackSlotBytes = 4 + 16 + 4;
 
 struct Carve {
   unsigned char* base;
@@ -63,7 +63,7 @@ size_t fixed_bytes(uint32_t n_events, uint32_t n_layers, uint32_t n_mid_sms) {
   size_t b = 0;
   b += align_up((size_t)items * 4) * 2 + align_up((size_t)items * 18 * 4);  // counts, slab_base, layer descriptors
   b += align_up(scan_state_words(items) * 8);                     // scan state (clusters)
-  b += align_up(24 + (size_t)n_mid_sms * 4);                      // big-pool counter, deferred-item counters, mid masks
+  b += align_up(32 + (size_t)n_mid_sms * 4);                      // big-pool counter, slab spill cursor, deferred-item counters, mid masks
   b += align_up((size_t)items * 4) * 2;                           // deferred items of the cluster kernel (two lists)
   b += align_up((size_t)n_mid_sms * 32 * cluster_mid_slot_bytes());
   b += align_up((size_t)big_slots(items) * cluster_big_slot_bytes());
@@ -152,6 +152,7 @@ int allen_velo_create(const allen_velo_geometry_t* geo, allen_velo_t** out) {
     cudaFree(h->dev_block); delete h; return ALLEN_VELO_ERR_CUDA;
   }
   h->n_sms = (uint32_t)n_sm;
+  if (cluster_prepare() != cudaSuccess || track_prepare() != cudaSuccess) { cudaFree(h->dev_block); delete h; return ALLEN_VELO_ERR_CUDA; }
   h->n_mid_sms = (uint32_t)n_sm + 16;  // %smid is below the SM count on the parts seen; margin for gaps in the numbering
   for (int i = 0; i < 2; ++i)
     if (cudaStreamCreateWithFlags(&h->side[i], cudaStreamNonBlocking) != cudaSuccess) { allen_velo_destroy(h); return ALLEN_VELO_ERR_CUDA; }
@@ -173,7 +174,8 @@ int allen_velo_create(const allen_velo_geometry_t* geo, allen_velo_t** out) {
 
 size_t allen_velo_workspace_bytes(const allen_velo_t* h, uint32_t n_events, size_t raw_bytes) {
   if (!h) return 0;
-  // slab and tracking scratch: two entries per raw word (a super-pixel holds at most two clusters)
+  // slab and tracking scratch: two entries per raw word (a super-pixel holds at most two clusters): one in the dense
+  // part of the slab, one behind it for layers with more clusters than SP words
   const size_t entries = raw_bytes / 2 + 4096;
   return fixed_bytes(n_events, h->dev.n_layers, h->n_mid_sms) + entries * per_entry_bytes() + 16 * kAlign;
 }
@@ -235,8 +237,8 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   uint32_t* slab_base = cv.take<uint32_t>(items);
   uint32_t* desc = cv.take<uint32_t>((size_t)items * 18);
   unsigned long long* scan_state = cv.take<unsigned long long>(scan_state_words(items));
-  // big-pool counter, deferred-item count and cursor, then the mid masks: zeroed by one memset
-  const size_t state_bytes = 24 + (size_t)h->n_mid_sms * 4;
+  // big-pool counter, slab spill cursor, deferred-item counts and cursors, then the mid masks: zeroed by one memset
+  const size_t state_bytes = 32 + (size_t)h->n_mid_sms * 4;
   unsigned long long* state = reinterpret_cast<unsigned long long*>(cv.take<unsigned char>(state_bytes));
   uint32_t* defer_list = cv.take<uint32_t>(items);
   uint32_t* defer_list2 = cv.take<uint32_t>(items);
@@ -255,20 +257,17 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   if (entries > 0x7FFFFFF0u) entries = 0x7FFFFFF0u;
   ClusterSlab slab{};
   slab.capacity = (uint32_t)entries;
-  slab.key = cv.take<uint32_t>(entries);
-  slab.n_pixels = cv.take<uint32_t>(entries);
-  slab.sum_col = cv.take<uint32_t>(entries);
-  slab.sum_row = cv.take<uint32_t>(entries);
+  slab.dense = (uint32_t)(entries / 2);
+  slab.rec = cv.take<uint4>(entries);
+  slab.info = cv.take<uint4>(entries);
   slab.checksum = cv.take<uint32_t>(entries);
-  slab.x = cv.take<float>(entries);
-  slab.y = cv.take<float>(entries);
-  slab.z = cv.take<float>(entries);
-  slab.phi16 = cv.take<int16_t>(entries);
+  slab.spill_cursor = reinterpret_cast<uint32_t*>(state) + 1;
   // tracking scratch is addressed by output cluster index; it shares the entry count with the slab
   uint16_t* link = cv.take<uint16_t>(entries);
   uint16_t* hits_slab = cv.take<uint16_t>(entries);
   uint32_t* trk_hitoff = cv.take<uint32_t>(entries / 3 + 1);
   float4* trk_fit = cv.take<float4>(entries / 3 + 1);
+  uint32_t* trk_final = cv.take<uint32_t>(entries / 3 + 1);
   if (cv.used > h->ws_bytes) return fail(h, ALLEN_VELO_ERR_WORKSPACE, "workspace carve overflow");
 
   // ---- launch sequence
@@ -294,7 +293,7 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   cl.defer_count = reinterpret_cast<uint32_t*>(state) + 2;
   cl.defer_list[0] = defer_list;
   cl.defer_list[1] = defer_list2;
-  cl.mid_mask = reinterpret_cast<uint32_t*>(state + 3);
+  cl.mid_mask = reinterpret_cast<uint32_t*>(state + 4);
   cl.mid_pool = mid_pool;
   cl.big_pool = big_pool;
   cl.n_mid_sms = h->n_mid_sms;
@@ -323,6 +322,7 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   tl.hits_slab = hits_slab;
   tl.trk_hitoff = trk_hitoff;
   tl.trk_fit = trk_fit;
+  tl.trk_final = trk_final;
   tl.counts = trk_counts;
   tl.level = trk_level;
   tl.ev_list[0] = trk_lists[0]; tl.ev_list[1] = trk_lists[1];

@@ -17,8 +17,9 @@
 // with shared-memory atomics (commutative integer adds / min: deterministic).
 //
 // The layer's clusters are ranked by (phi16, key) with a 256-bucket counting sort on the top byte of phi plus an exact
-// in-bucket rank and written, coalesced and in the normative order, to the layer's region of a slab whose position
-// depends only on the event's bank table (2 entries per SP word before the layer): warps never wait for one another.
+// in-bucket rank and written, coalesced and in the normative order, as two 16-byte records per cluster, to the layer's
+// region of a slab whose position depends only on the event's bank table (the position of the layer's first SP word;
+// the rare layer with more clusters than SP words takes a region behind that dense part): warps never wait for one another.
 // (A decoupled look-back over the 260 k (event, layer) items that wrote the compacted output directly was measured
 // first: in-order publication made every warp wait for its slowest predecessor — 66 % of the issued instructions
 // were the spin — so compaction moved into the track kernel, which reads every hit anyway; profiles/README.md.)
@@ -346,10 +347,22 @@ __device__ __forceinline__ bool ccl_pass(const Pass& p, const ClusterStore& cs, 
 // write in the normative order to the slab region [slab0, slab0 + n_cl).
 template <bool kChecksum>
 __device__ __forceinline__ void finish_layer(const ClusterLaunch& a, const ClusterStore& cs, const SortStore& ss,
-                                             uint32_t item, uint32_t slab0, uint32_t n_cl) {
+                                             uint32_t item, uint32_t slab0, uint32_t region, uint32_t n_cl) {
   const DeviceGeometry& g = a.geo;
   const uint32_t lane = lane_id();
-  if (lane == 0) a.counts[item] = n_cl;  // slab_base[item] = slab0 was written by velo_prepare_kernel
+  if (n_cl > region) {  // warp-uniform: more clusters than SP words -> a region behind the dense part of the slab
+    uint32_t s = 0;
+    if (lane == 0) s = atomicAdd(a.slab.spill_cursor, n_cl);
+    s = __shfl_sync(kFull, s, 0);
+    if ((unsigned long long)a.slab.dense + s + n_cl > a.slab.capacity) {  // workspace smaller than workspace_bytes()
+      if (lane == 0) atomicOr(a.status + item / g.n_layers, ALLEN_VELO_STATUS_STAGE_OVERFLOW);
+      n_cl = 0;
+    } else {
+      slab0 = a.slab.dense + s;
+      if (lane == 0) a.slab_base[item] = slab0;  // otherwise the value velo_prepare_kernel wrote stands
+    }
+  }
+  if (lane == 0) a.counts[item] = n_cl;
   if (n_cl == 0) return;
 #pragma unroll 1
   for (uint32_t s = lane; s < 256; s += 32) ss.cnt256[s] = 0;
@@ -407,14 +420,8 @@ __device__ __forceinline__ void finish_layer(const ClusterLaunch& a, const Clust
     else cluster_local(n, sc, sr, g.pitch, u, v);
     local_to_global(u, v, g.ltg + 9 * (key >> 18), x, y, z);
     const uint32_t o = slab0 + j;
-    a.slab.key[o] = key;
-    a.slab.n_pixels[o] = n;
-    a.slab.sum_col[o] = sc;
-    a.slab.sum_row[o] = sr;
-    a.slab.x[o] = x;
-    a.slab.y[o] = y;
-    a.slab.z[o] = z;
-    a.slab.phi16[o] = (int16_t)(ss.phis[c] ^ 0x8000u);
+    a.slab.rec[o] = make_uint4(__float_as_uint(x), __float_as_uint(y), __float_as_uint(z), (uint32_t)(ss.phis[c] ^ 0x8000u));
+    a.slab.info[o] = make_uint4(key, n, sc, sr);
     if (kChecksum) a.slab.checksum[o] = cs.cks[c];
   }
 }
@@ -429,8 +436,8 @@ __device__ __noinline__ bool ccl_pass_generic(const Pass& p, const ClusterStore&
 }
 template <bool kChecksum>
 __device__ __noinline__ void finish_layer_generic(const ClusterLaunch& a, const ClusterStore& cs, const SortStore& ss,
-                                                  uint32_t item, uint32_t slab0, uint32_t n_cl) {
-  finish_layer<kChecksum>(a, cs, ss, item, slab0, n_cl);
+                                                  uint32_t item, uint32_t slab0, uint32_t region, uint32_t n_cl) {
+  finish_layer<kChecksum>(a, cs, ss, item, slab0, region, n_cl);
 }
 
 template <bool kChecksum, uint32_t kCap>
@@ -506,7 +513,7 @@ __device__ __forceinline__ void cluster_item(const ClusterLaunch& a, WarpSmem<kC
   const uint32_t my_cnt = __shfl_sync(kFull, dv, (lane & 7u) + 8u);  // lanes 0..7: SP words of sensor k
   const uint32_t slab0 = __shfl_sync(kFull, dv, 16);
   if (__shfl_sync(kFull, dv, 17) & 1u) {  // malformed event (BAD_HEADER set by the prepare kernel): no clusters
-    finish_layer<kChecksum>(a, cs, ss, item, 0, 0);
+    finish_layer<kChecksum>(a, cs, ss, item, 0, 0, 0);
     return;
   }
   const uint32_t* spw = a.raw;
@@ -515,9 +522,9 @@ __device__ __forceinline__ void cluster_item(const ClusterLaunch& a, WarpSmem<kC
   const uint32_t cnt_k = lane < K ? my_cnt : 0u;
   const uint32_t n_sp_layer = __reduce_add_sync(kFull, cnt_k);
   const uint32_t max_cnt = __reduce_max_sync(kFull, cnt_k);
-  if ((unsigned long long)slab0 + 2ull * n_sp_layer > a.slab.capacity) {  // workspace smaller than workspace_bytes()
+  if ((unsigned long long)slab0 + n_sp_layer > a.slab.dense) {  // workspace smaller than workspace_bytes()
     if (lane == 0) atomicOr(a.status + e, ALLEN_VELO_STATUS_STAGE_OVERFLOW);
-    finish_layer<kChecksum>(a, cs, ss, item, 0, 0);
+    finish_layer<kChecksum>(a, cs, ss, item, 0, 0, 0);
     return;
   }
 
@@ -535,7 +542,7 @@ __device__ __forceinline__ void cluster_item(const ClusterLaunch& a, WarpSmem<kC
   if (mode == 0) {
     if (ccl_pass<kChecksum>(fast, cs, g, spw, my_sensor, my_off, cnt_k, 0, K, n_cl, bad_sp, &ws.n_edges)) {
       if (__any_sync(kFull, bad_sp) && lane == 0) atomicOr(a.status + e, ALLEN_VELO_STATUS_BAD_SP);
-      finish_layer<kChecksum>(a, cs, ss, item, slab0, n_cl);
+      finish_layer<kChecksum>(a, cs, ss, item, slab0, n_sp_layer, n_cl);
       return;
     }
     mode = 2;  // more clusters or edges than the warp's shared memory holds (not seen on physics-like input)
@@ -611,7 +618,7 @@ __device__ __forceinline__ void cluster_item(const ClusterLaunch& a, WarpSmem<kC
   } else if (__any_sync(kFull, bad_sp) && lane == 0) {
     atomicOr(a.status + e, ALLEN_VELO_STATUS_BAD_SP);
   }
-  finish_layer_generic<kChecksum>(a, cs, ss, item, slab0, n_cl);
+  finish_layer_generic<kChecksum>(a, cs, ss, item, slab0, n_sp_layer, n_cl);
   __syncwarp();
   if (held != 0xFFFFFFFFu && lane == 0) atomicAnd(a.mid_mask + (held >> 5), ~(1u << (held & 31u)));
 }
@@ -700,8 +707,9 @@ __global__ void __launch_bounds__(128) velo_prepare_kernel(const __grid_constant
     carry += __shfl_sync(kFull, incl, 31);
     if (l < L) {
       const uint32_t item = e * L + l;
-      // two slab entries per SP word (a super-pixel holds at most two clusters), placed by the raw position
-      const uint32_t slab0 = bad ? 0u : 2u * (words0 + before);
+      // one slab entry per SP word, placed by the raw position: the layers of the batch tile the dense part of the
+      // slab without gaps (a layer with more clusters than SP words moves behind it, finish_layer)
+      const uint32_t slab0 = bad ? 0u : words0 + before;
       uint32_t* d = a.desc + (size_t)item * kDescWords;
 #pragma unroll
       for (int k = 0; k < kMaxSensorsPerLayer; ++k) { d[k] = off[k]; d[8 + k] = cnt[k]; }
@@ -720,9 +728,6 @@ size_t cluster_big_slot_bytes() { return BigSlot::kBytes; }
 template <bool kChecksum, uint32_t kCap, bool kDefer>
 cudaError_t launch_cluster_instance(const ClusterLaunch& a, uint32_t grid, cudaStream_t stream) {
   const size_t smem = sizeof(WarpSmem<kChecksum, kCap>) * kWarps;
-  cudaError_t err = cudaFuncSetAttribute(velo_cluster_kernel<kChecksum, kCap, kDefer>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (err != cudaSuccess) return err;
   velo_cluster_kernel<kChecksum, kCap, kDefer><<<grid, kWarps * 32, smem, stream>>>(a);
   return cudaGetLastError();
 }
@@ -730,11 +735,18 @@ cudaError_t launch_cluster_instance(const ClusterLaunch& a, uint32_t grid, cudaS
 template <bool kChecksum, uint32_t kCap, bool kDefer, uint32_t kFrom>
 cudaError_t launch_cluster_list(const ClusterLaunch& a, uint32_t grid, cudaStream_t stream) {
   const size_t smem = sizeof(WarpSmem<kChecksum, kCap>) * kWarps;
-  cudaError_t err = cudaFuncSetAttribute(velo_cluster_list_kernel<kChecksum, kCap, kDefer, kFrom>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (err != cudaSuccess) return err;
   velo_cluster_list_kernel<kChecksum, kCap, kDefer, kFrom><<<grid, kWarps * 32, smem, stream>>>(a);
   return cudaGetLastError();
+}
+
+template <bool kChecksum>
+cudaError_t prepare_cluster_kernels() {
+  const auto attr = cudaFuncAttributeMaxDynamicSharedMemorySize;
+  cudaError_t err = cudaFuncSetAttribute(velo_cluster_kernel<kChecksum, 128, true>, attr, (int)sizeof(WarpSmem<kChecksum, 128>) * kWarps);
+  if (err == cudaSuccess) err = cudaFuncSetAttribute(velo_cluster_kernel<kChecksum, 256, true>, attr, (int)sizeof(WarpSmem<kChecksum, 256>) * kWarps);
+  if (err == cudaSuccess) err = cudaFuncSetAttribute(velo_cluster_list_kernel<kChecksum, 256, true, 0>, attr, (int)sizeof(WarpSmem<kChecksum, 256>) * kWarps);
+  if (err == cudaSuccess) err = cudaFuncSetAttribute(velo_cluster_list_kernel<kChecksum, 512, false, 1>, attr, (int)sizeof(WarpSmem<kChecksum, 512>) * kWarps);
+  return err;
 }
 
 template <bool kChecksum>
@@ -748,6 +760,11 @@ cudaError_t launch_cluster_chain(const ClusterLaunch& a, uint32_t grid, uint32_t
   if ((err = launch_cluster_list<kChecksum, 512, false, 1>(a, min(grid, 3 * n_sms), stream)) != cudaSuccess) return err;
   ++*n_launches;
   return cudaSuccess;
+}
+
+cudaError_t cluster_prepare() {
+  cudaError_t err = prepare_cluster_kernels<true>();
+  return err == cudaSuccess ? prepare_cluster_kernels<false>() : err;
 }
 
 // prepare -> cluster kernel with 128 entries per layer over all (event, layer) items -> the 256-entry instance over

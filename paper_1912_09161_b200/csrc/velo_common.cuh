@@ -24,13 +24,19 @@ struct DeviceGeometry {
   allen_velo_params_t params;
 };
 
-// Slab the cluster kernel writes: structure of arrays with `capacity` entries; the region of (event, layer) starts at
-// slab_base[item] and holds counts[item] clusters in the normative order.  The track kernel moves it to the output.
+// Slab the cluster kernel writes: two arrays of 16-byte records with `capacity` entries; the region of (event, layer)
+// starts at slab_base[item] and holds counts[item] clusters in the normative order.  The track kernel stages a layer with
+// one 128-bit load per hit and moves it to the output.
+//   rec[i]  = { x, y, z (fp32 bit patterns), phi16 as u16 in the low half (high half zero) }  = the search's hit record
+//   info[i] = { key, n_pixels, sum_col, sum_row }
+// Entries [0, dense) are placed from the bank tables alone (one entry per raw SP word: the region of a layer starts at
+// the position of its first SP word); a layer with more clusters than SP words (super-pixels holding two clusters)
+// takes its region from [dense, capacity) with a cursor instead.
 struct ClusterSlab {
-  uint32_t capacity;
-  uint32_t *key, *n_pixels, *sum_col, *sum_row, *checksum;
-  float *x, *y, *z;
-  int16_t* phi16;
+  uint32_t capacity, dense;
+  uint4 *rec, *info;
+  uint32_t* checksum;
+  uint32_t* spill_cursor;  // entries handed out of [dense, capacity), zeroed by the launcher
 };
 
 // ---- small device helpers -------------------------------------------------------------------
@@ -158,15 +164,18 @@ struct TrackLaunch {
   uint16_t* hits_slab;             // [cluster capacity] hit lists of the event's output tracks, back to back
   uint32_t* trk_hitoff;            // [capacity/3+1] event-local first entry in hits_slab of every output track
   float4* trk_fit;                 // [capacity/3+1] x0, y0, tx, ty
+  uint32_t* trk_final;             // [capacity/3+1] flat kernel: final state of every track by order of creation
   unsigned long long* counts;      // [n_events] (n_tracks << 32) | n_track_hits
-  uint8_t* level;                  // [n_events] class of the event: searching instance 0..2, 254 copy only, 255 nothing
+  uint8_t* level;                  // [n_events] class of the event (velo_track.cuh): flat kernel, 512 / 1024-hit CTA instance, copy only, nothing
   uint32_t* ev_list[2];            // [n_events] each: events of level 1 / 2
-  uint32_t* redo_list[2];          // [n_events] each: events level 0 / 1 ran out of track slots on (second pass)
-  uint32_t* order;                 // [4][n_events] events of the first instance by size bin
+  uint32_t* redo_list[2];          // [n_events] each: events the flat kernel / the 512-hit instance ran out of track slots on
+  uint32_t* order;                 // [4][n_events] events of the flat kernel by size bin
   uint32_t* counters;              // [12] list sizes and cursors, zeroed by the launcher
 };
 cudaError_t launch_track(const TrackLaunch& a, cudaStream_t stream, cudaStream_t* side, cudaEvent_t* ev,
                          uint32_t n_sms, uint32_t* n_launches);
+cudaError_t track_prepare();    // once per process: dynamic shared-memory limits of the track kernels
+cudaError_t cluster_prepare();  // likewise for the cluster kernels
 
 struct CompactTracksLaunch {
   uint32_t n_events;

@@ -1,5 +1,6 @@
-// Kernel 2 of the VELO hot path: search by triplet (A5 seeding, A6 forwarding, A7 clone/ghost killing) and the
-// straight-line fit (A8) — SURVEY.md §8(a); the algorithm is DESIGN.md reading R5 (T1..T5) of P:181-183 ("forming
+// Kernel 2 of the VELO hot path, CTA-per-event instances for events whose busiest layer exceeds what the flattened
+// kernel (velo_track_flat.cu) stages, and the second pass for events that ran out of its track slots: search by triplet
+// (A5 seeding, A6 forwarding, A7 clone/ghost killing) and the straight-line fit (A8) — SURVEY.md §8(a); the algorithm is DESIGN.md reading R5 (T1..T5) of P:181-183 ("forming
 // seeds of three hits from consecutive layers ('triplets'), and then extending these to the other layers"; "sort hits
 // on every layer by phi for fast look-up") and R6 of P:149 (straight lines).
 //
@@ -19,20 +20,13 @@
 //    by the smallest instance it fits, and an instance that runs out of track slots hands the event to the next one.
 #include <cuda_pipeline.h>
 
-#include "velo_common.cuh"
+#include "velo_track.cuh"
 
 namespace velo {
 namespace {
 
-constexpr unsigned long long kNoClaim = ~0ull;
 constexpr int kBuckets = 128;
 constexpr int kBucketShift = 9;  // 65536 / 128
-constexpr uint32_t kUsedBit = 0x10000u;
-
-struct __align__(16) Hit {
-  float x, y, z;
-  uint32_t w;  // phi16 (low 16 bits, two's complement) | used << 16
-};
 
 template <int kThreads_, int kCap_, int kCapTracks_, int kCapDoublets_, int kLevel_, bool kLast_, bool kCopier_>
 struct Cfg {
@@ -48,25 +42,9 @@ struct Cfg {
   static constexpr int kRoundsB = (kCap + kThreads - 1) / kThreads;
   static constexpr int kRoundsT = (kCapTracks + kThreads - 1) / kThreads;
 };
-#ifndef VELO_TRK_S_THREADS
-#define VELO_TRK_S_THREADS 128
-#endif
-#ifndef VELO_TRK_S_TRACKS
-#define VELO_TRK_S_TRACKS 352
-#endif
-#ifndef VELO_TRK_S_DOUBLETS
-#define VELO_TRK_S_DOUBLETS 576
-#endif
-using CfgS = Cfg<VELO_TRK_S_THREADS, 256, VELO_TRK_S_TRACKS, VELO_TRK_S_DOUBLETS, 0, false, true>;
-using CfgM = Cfg<256, 512, 1024, 4096, 1, false, true>;
-using CfgL = Cfg<512, 1024, 2048, 2048, 2, true, true>;
-// second pass for events a smaller instance ran out of track slots on: their clusters are already in the output
+// second pass for events the flat kernel ran out of track or triplet slots on: their clusters are already in the output
 using CfgMr = Cfg<256, 512, 1024, 4096, 1, false, false>;
 using CfgLr = Cfg<512, 1024, 2048, 2048, 2, true, false>;
-
-// class of an event (TrackLaunch::level), set by classify_events_kernel
-constexpr uint8_t kClsSkip = 255;  // nothing to do (no clusters, or the output cannot hold them)
-constexpr uint8_t kClsCopy = 254;  // clusters are moved to the output, no tracking (incomplete or > 65535 clusters)
 
 template <class C>
 struct Smem {
@@ -109,18 +87,34 @@ __device__ __forceinline__ void tsync() {
   else __syncthreads();
 }
 
+// Where the hits are read from: the cluster kernel's slab of 16-byte records (instances with a copier warp) or the
+// compacted output an earlier kernel has filled (second-pass instances).
 template <class C>
 struct Ctx {
   Smem<C>& sm;
-  const float* __restrict__ X;
+  const uint4* __restrict__ R;       // slab records (kCopier)
+  const float* __restrict__ X;       // output arrays (!kCopier)
   const float* __restrict__ Y;
   const float* __restrict__ Z;
   const int16_t* __restrict__ PHI;
   allen_velo_params_t P;
 };
 
-// Bring layer `l` into ring slot l % 3: x, y, z by cp.async (4-byte copies into the 16-byte records), the phi word and
-// the bucket table by this thread.  Completion: __pipeline_wait_prior(0) + __syncthreads() by the caller.
+// Hit at absolute position s of the source arrays (a track's last hit that has left the ring).
+template <class C>
+__device__ __forceinline__ Hit far_hit(const Ctx<C>& c, uint32_t s) {
+  Hit h;
+  if (C::kCopier) {
+    const uint4 r = __ldg(c.R + s);
+    h.x = __uint_as_float(r.x); h.y = __uint_as_float(r.y); h.z = __uint_as_float(r.z); h.w = r.w;
+  } else {
+    h.x = __ldg(c.X + s); h.y = __ldg(c.Y + s); h.z = __ldg(c.Z + s); h.w = (uint16_t)__ldg(c.PHI + s);
+  }
+  return h;
+}
+
+// Bring layer `l` into ring slot l % 3 by cp.async (one 16-byte copy per hit from the slab, or three 4-byte copies from
+// the output arrays); the bucket table by this thread.  Completion: __pipeline_wait_prior(0) + barrier by the caller.
 template <class C>
 __device__ __forceinline__ void stage_layer(const Ctx<C>& c, uint32_t l) {
   Smem<C>& sm = c.sm;
@@ -134,13 +128,21 @@ __device__ __forceinline__ void stage_layer(const Ctx<C>& c, uint32_t l) {
   }
 #pragma unroll 1
   for (uint32_t k = threadIdx.x; k < n; k += C::kThreads) {
-    __pipeline_memcpy_async(&rec[k].x, c.X + base + k, 4);
-    __pipeline_memcpy_async(&rec[k].y, c.Y + base + k, 4);
-    __pipeline_memcpy_async(&rec[k].z, c.Z + base + k, 4);
-    const uint32_t ph = (uint16_t)__ldg(c.PHI + base + k);
-    rec[k].w = ph;
+    uint32_t ph, ph_prev = 0;
+    if (C::kCopier) {
+      __pipeline_memcpy_async(&rec[k], c.R + base + k, 16);  // the record's last word is phi16 with a clear used bit
+      ph = __ldg(reinterpret_cast<const uint32_t*>(c.R + base + k) + 3) & 0xFFFFu;
+      if (k) ph_prev = __ldg(reinterpret_cast<const uint32_t*>(c.R + base + k - 1) + 3) & 0xFFFFu;
+    } else {
+      __pipeline_memcpy_async(&rec[k].x, c.X + base + k, 4);
+      __pipeline_memcpy_async(&rec[k].y, c.Y + base + k, 4);
+      __pipeline_memcpy_async(&rec[k].z, c.Z + base + k, 4);
+      ph = (uint16_t)__ldg(c.PHI + base + k);
+      rec[k].w = ph;
+      if (k) ph_prev = (uint16_t)__ldg(c.PHI + base + k - 1);
+    }
     const int bk = (int)((ph ^ 0x8000u) >> kBucketShift);
-    const int bp = k ? (int)((((uint32_t)(uint16_t)__ldg(c.PHI + base + k - 1)) ^ 0x8000u) >> kBucketShift) : -1;
+    const int bp = k ? (int)((ph_prev ^ 0x8000u) >> kBucketShift) : -1;
 #pragma unroll 1
     for (int b = bp + 1; b <= bk; ++b) bucket[b] = (uint16_t)k;
     if (k + 1 == n)
@@ -182,18 +184,16 @@ __device__ __forceinline__ void process_doublet(const Ctx<C>& c, const Hit* __re
   if (best != kNoClaim) atomicMin(&c.sm.best[kb], best);
 }
 
-// Copy clusters [k0, k1) of layer l (layer-local indices) from the slab to the compacted output.
+// Copy n clusters from slab position src to position dst of the compacted output.
 __device__ __forceinline__ void copy_clusters(const TrackLaunch& a, uint32_t src, uint32_t dst, uint32_t n,
                                               uint32_t first, uint32_t step) {
 #pragma unroll 1
   for (uint32_t k = first; k < n; k += step) {
     const uint32_t s = src + k, d = dst + k;
-    const uint32_t key = __ldg(a.slab.key + s), np = __ldg(a.slab.n_pixels + s);
-    const uint32_t sc = __ldg(a.slab.sum_col + s), sr = __ldg(a.slab.sum_row + s);
-    const float x = __ldg(a.slab.x + s), y = __ldg(a.slab.y + s), z = __ldg(a.slab.z + s);
-    const int16_t ph = __ldg(a.slab.phi16 + s);
-    a.clusters.key[d] = key; a.clusters.n_pixels[d] = np; a.clusters.sum_col[d] = sc; a.clusters.sum_row[d] = sr;
-    a.clusters.x[d] = x; a.clusters.y[d] = y; a.clusters.z[d] = z; a.clusters.phi16[d] = ph;
+    const uint4 r = __ldg(a.slab.rec + s), q = __ldg(a.slab.info + s);
+    a.clusters.key[d] = q.x; a.clusters.n_pixels[d] = q.y; a.clusters.sum_col[d] = q.z; a.clusters.sum_row[d] = q.w;
+    a.clusters.x[d] = __uint_as_float(r.x); a.clusters.y[d] = __uint_as_float(r.y); a.clusters.z[d] = __uint_as_float(r.z);
+    a.clusters.phi16[d] = (int16_t)(uint16_t)r.w;
     if (a.clusters.checksum) a.clusters.checksum[d] = __ldg(a.slab.checksum + s);
   }
 }
@@ -230,9 +230,7 @@ __device__ __forceinline__ void track_event(const TrackLaunch& a, uint32_t e, Sm
     return;
   }
 
-  Ctx<C> c{sm,
-           C::kCopier ? a.slab.x : a.clusters.x, C::kCopier ? a.slab.y : a.clusters.y,
-           C::kCopier ? a.slab.z : a.clusters.z, C::kCopier ? a.slab.phi16 : a.clusters.phi16, g.params};
+  Ctx<C> c{sm, a.slab.rec, a.clusters.x, a.clusters.y, a.clusters.z, a.clusters.phi16, g.params};
   const allen_velo_params_t& P = c.P;
   uint16_t* link = a.link + co;
 
@@ -281,8 +279,8 @@ __device__ __forceinline__ void track_event(const TrackLaunch& a, uint32_t e, Sm
         uint32_t l = (uint32_t)i + 1;
 #pragma unroll 1
         while (q >= sm.lo[l + 1]) ++l;
-        const uint32_t s = sm.src[l] + (q - sm.lo[l]);
-        xq = __ldg(c.X + s); yq = __ldg(c.Y + s); zq = __ldg(c.Z + s); phq = (int)__ldg(c.PHI + s);
+        const Hit hq = far_hit(c, sm.src[l] + (q - sm.lo[l]));
+        xq = hq.x; yq = hq.y; zq = hq.z; phq = phi_of(hq.w);
       }
       const float tx = sm.ttx[t], ty = sm.tty[t];
       const int w = P.w_fwd_phi16;
@@ -367,8 +365,8 @@ __device__ __forceinline__ void track_event(const TrackLaunch& a, uint32_t e, Sm
           uint32_t l = (uint32_t)i + 1;
 #pragma unroll 1
           while (q >= sm.lo[l + 1]) ++l;
-          const uint32_t s = sm.src[l] + (q - sm.lo[l]);
-          xq = __ldg(c.X + s); yq = __ldg(c.Y + s); zq = __ldg(c.Z + s);
+          const Hit hq = far_hit(c, sm.src[l] + (q - sm.lo[l]));
+          xq = hq.x; yq = hq.y; zq = hq.z;
         }
         const Hit hc = recC[fc];
         const float dz = __fsub_rn(hc.z, zq);
@@ -552,25 +550,30 @@ __device__ __forceinline__ void track_event(const TrackLaunch& a, uint32_t e, Sm
     if (n) {
       const uint32_t ot = out_tracks + (off >> 20), oh = out_hits + (off & 0xFFFFFu);
       // hits in order of addition: walk the links from the newest hit backwards
-      double sz = 0, sx = 0, sy = 0;
+      uint16_t* out_h = a.hits_slab + co + oh;
       uint32_t h = st >> 16;
 #pragma unroll 1
       for (int k = (int)n - 1; k >= 0; --k) {
-        a.hits_slab[co + oh + k] = (uint16_t)h;
-        sz += (double)__ldcg(Z + h); sx += (double)__ldcg(X + h); sy += (double)__ldcg(Y + h);
+        out_h[k] = (uint16_t)h;
         if (k) h = link[h];
       }
-      const double inv = 1.0 / (double)n;
-      const double zm = sz * inv, xm = sx * inv, ym = sy * inv;
-      double szz = 0, szx = 0, szy = 0;
-      h = st >> 16;
+      // A8: the oracle's operations in the oracle's order (R6) -> bit-identical parameters
+      const double dn = (double)n;
+      double zm = 0, xm = 0, ym = 0;
 #pragma unroll 1
-      for (int k = (int)n - 1; k >= 0; --k) {
+      for (uint32_t k = 0; k < n; ++k) {
+        h = out_h[k];
+        zm += (double)__ldcg(Z + h); xm += (double)__ldcg(X + h); ym += (double)__ldcg(Y + h);
+      }
+      zm /= dn; xm /= dn; ym /= dn;
+      double szz = 0, szx = 0, szy = 0;
+#pragma unroll 1
+      for (uint32_t k = 0; k < n; ++k) {
+        h = out_h[k];
         const double dz = (double)__ldcg(Z + h) - zm;
         szz += dz * dz;
         szx += dz * ((double)__ldcg(X + h) - xm);
         szy += dz * ((double)__ldcg(Y + h) - ym);
-        if (k) h = link[h];
       }
       const double tx = szx / szz, ty = szy / szz;
       a.trk_hitoff[trk0 + ot] = oh;
@@ -670,8 +673,8 @@ __global__ void __launch_bounds__(128) compact_tracks_kernel(const CompactTracks
 
 // One thread per event: class of the event (which instance searches it, or copy only / nothing) and the event lists
 // of the two larger instances.  counters: [0], [1] events of level 1, 2; [2], [3] second-pass events; [4..7] cursors;
-// [8..11] events of the first instance (and copy-only events) in four size bins: it takes them largest first, so that
-// the last CTAs of the grid are short ones.
+// [8..11] events of the flat kernel (and copy-only events) in four size bins: it takes them largest first, so that the
+// last warps of the grid are short ones.
 __global__ void __launch_bounds__(256) classify_events_kernel(const __grid_constant__ TrackLaunch a) {
   const uint32_t e = blockIdx.x * blockDim.x + threadIdx.x;
   if (e >= a.n_events) return;
@@ -698,50 +701,22 @@ __global__ void __launch_bounds__(256) classify_events_kernel(const __grid_const
       mx = max(mx, o - prev);
       prev = o;
     }
-    if (mx <= (uint32_t)CfgS::kCap) cls = 0;
-    else if (mx <= (uint32_t)CfgM::kCap) cls = 1;
-    else if (mx <= (uint32_t)CfgL::kCap) cls = 2;
+    if (mx <= (uint32_t)kFlatCap) cls = kClsFlat;
+    else if (mx <= (uint32_t)CfgMr::kCap) cls = kClsMid;
+    else if (mx <= (uint32_t)CfgLr::kCap) cls = kClsLarge;
     else {  // busiest layer beyond the largest staging capacity
       atomicOr(a.clusters.status + e, ALLEN_VELO_STATUS_STAGE_OVERFLOW);
       cls = kClsCopy;
     }
-    if (cls == 1 || cls == 2) a.ev_list[cls - 1][atomicAdd(a.counters + (cls - 1), 1u)] = e;
+    if (cls == kClsMid || cls == kClsLarge) a.ev_list[cls - 1][atomicAdd(a.counters + (cls - 1), 1u)] = e;
   }
-  if (cls == 0 || cls == kClsCopy) {
+  if (cls == kClsFlat || cls == kClsCopy) {
     const uint32_t avg = a.clusters.event_offsets[a.n_events] / a.n_events + 1u;
     const uint32_t bin = cls == kClsCopy ? 3u : 20u * n_cl >= 30u * avg ? 0u : 20u * n_cl >= 23u * avg ? 1u : 20u * n_cl >= 17u * avg ? 2u : 3u;
     a.order[(size_t)bin * a.n_events + atomicAdd(a.counters + 8 + bin, 1u)] = e;
   }
   a.level[e] = cls;
   if (cls >= kClsCopy) a.counts[e] = 0;
-}
-
-// First instance: one CTA per event of class 0; it also moves the clusters of copy-only events.
-template <class C>
-__global__ void __launch_bounds__(C::kBlock) velo_track_kernel(const __grid_constant__ TrackLaunch a) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  Smem<C>& sm = *reinterpret_cast<Smem<C>*>(smem_raw);
-  uint32_t j = blockIdx.x, bin = 0;  // events in four size bins, largest first
-#pragma unroll 1
-  for (; bin < 4; ++bin) {
-    const uint32_t n = a.counters[8 + bin];
-    if (j < n) break;
-    j -= n;
-  }
-  if (bin == 4) return;
-  const uint32_t e = a.order[(size_t)bin * a.n_events + j];
-  const uint8_t cls = a.level[e];
-  if (cls == kClsCopy) {
-    const uint32_t co = a.clusters.event_offsets[e], L = a.geo.n_layers;
-    load_offsets<C>(a, e, sm, co);
-    __syncthreads();
-#pragma unroll 1
-    for (uint32_t l = 0; l < L; ++l)
-      copy_clusters(a, sm.src[l], co + sm.lo[l], sm.lo[l + 1] - sm.lo[l], threadIdx.x, C::kBlock);
-    return;
-  }
-  if (cls != 0) return;
-  track_event<C>(a, e, sm);
 }
 
 // Larger instances: a few resident CTAs take events from a list (most batches have few or none of them).
@@ -765,11 +740,13 @@ __global__ void __launch_bounds__(C::kBlock) velo_track_list_kernel(const __grid
 }
 
 template <class C>
-cudaError_t launch_list(const TrackLaunch& a, uint32_t which, uint32_t grid, cudaStream_t stream) {
+cudaError_t prepare_list() {
   static_assert(sizeof(Smem<C>) <= 227 * 1024, "shared memory of one CTA");
-  cudaError_t err = cudaFuncSetAttribute(velo_track_list_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)sizeof(Smem<C>));
-  if (err != cudaSuccess) return err;
+  return cudaFuncSetAttribute(velo_track_list_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem<C>));
+}
+
+template <class C>
+cudaError_t launch_list(const TrackLaunch& a, uint32_t which, uint32_t grid, cudaStream_t stream) {
   const uint32_t* list = which < 2 ? a.ev_list[which] : a.redo_list[which - 2];
   velo_track_list_kernel<C><<<grid, C::kBlock, sizeof(Smem<C>), stream>>>(a, list, a.counters + which,
                                                                           a.counters + 4 + which);
@@ -778,9 +755,18 @@ cudaError_t launch_list(const TrackLaunch& a, uint32_t which, uint32_t grid, cud
 
 }  // namespace
 
-// classify -> [first instance over all events | level-1 list | level-2 list, on three streams] -> second pass for
-// events that ran out of track slots (level 1, then level 2).  `side`/`ev`: two extra streams and three events owned
-// by the handle; everything is ordered after and before the work on `stream` by events, nothing synchronises.
+// Once per process (allen_velo_create): the kernels' dynamic shared-memory limits.
+cudaError_t track_prepare() {
+  cudaError_t err = track_flat_prepare();
+  if (err == cudaSuccess) err = prepare_list<CfgMr>();
+  if (err == cudaSuccess) err = prepare_list<CfgLr>();
+  return err;
+}
+
+// classify -> [flat kernel over the events of its class | 512-hit list | 1024-hit list, on three streams] -> second pass
+// for events that ran out of track slots (512-hit instance, then 1024).  `side`/`ev`: two extra streams and three events
+// owned by the handle; everything is ordered after and before the work on `stream` by events (a fork/join a CUDA graph
+// can capture), nothing synchronises.
 cudaError_t launch_track(const TrackLaunch& a, cudaStream_t stream, cudaStream_t* side, cudaEvent_t* ev,
                          uint32_t n_sms, uint32_t* n_launches) {
   *n_launches = 0;
@@ -794,17 +780,12 @@ cudaError_t launch_track(const TrackLaunch& a, cudaStream_t stream, cudaStream_t
   if ((err = cudaStreamWaitEvent(side[0], ev[0], 0)) != cudaSuccess) return err;
   if ((err = cudaStreamWaitEvent(side[1], ev[0], 0)) != cudaSuccess) return err;
 
-  static_assert(sizeof(Smem<CfgS>) <= 227 * 1024, "shared memory of one CTA");
-  err = cudaFuncSetAttribute(velo_track_kernel<CfgS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)sizeof(Smem<CfgS>));
-  if (err != cudaSuccess) return err;
-  velo_track_kernel<CfgS><<<a.n_events, CfgS::kBlock, sizeof(Smem<CfgS>), stream>>>(a);
-  if ((err = cudaGetLastError()) != cudaSuccess) return err;
-  ++*n_launches;
   const uint32_t grid_m = min(a.n_events, 3 * n_sms), grid_l = min(a.n_events, n_sms);
-  if ((err = launch_list<CfgM>(a, 0, grid_m, side[0])) != cudaSuccess) return err;
+  if ((err = launch_track_flat_list(a, 0, min(a.n_events, 4 * n_sms), side[0])) != cudaSuccess) return err;
   ++*n_launches;
-  if ((err = launch_list<CfgL>(a, 1, grid_l, side[1])) != cudaSuccess) return err;
+  if ((err = launch_track_flat_list(a, 1, min(a.n_events, 2 * n_sms), side[1])) != cudaSuccess) return err;
+  ++*n_launches;
+  if ((err = launch_track_flat(a, stream)) != cudaSuccess) return err;
   ++*n_launches;
   if ((err = cudaEventRecord(ev[1], side[0])) != cudaSuccess) return err;
   if ((err = cudaEventRecord(ev[2], side[1])) != cudaSuccess) return err;
