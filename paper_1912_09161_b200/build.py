@@ -12,7 +12,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "_allen_velo.so")
-SOURCES = ["allen_velo.cu", "velo_cluster.cu", "velo_scan.cu", "velo_track.cu", "velo_track_flat.cu", "velo_pv.cu"]
+SOURCES = ["allen_velo.cu", "velo_cluster.cu", "velo_scan.cu", "velo_track.cu", "velo_seed.cu", "velo_follow.cu", "velo_pv.cu"]
 HEADERS = ["velo_common.cuh", "velo_track.cuh", os.path.join("..", "..", "include", "allen_velo.h")]
 
 NVCC_FLAGS = [

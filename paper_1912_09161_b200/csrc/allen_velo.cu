@@ -22,7 +22,7 @@ struct allen_velo {
   uint32_t sp_words_per_layer = 0;  // caller's hint (0: none)
   allen_velo_vertices_t vertices{};  // optional primary-vertex output (vertices == nullptr: off)
   cudaStream_t side[2] = {nullptr, nullptr};  // the larger track-kernel instances run beside the first one
-  cudaEvent_t fork_join[3] = {nullptr, nullptr, nullptr};
+  cudaEvent_t fork_join[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
   std::string last_error;
   // optional per-kernel timing: a ring of (kKernels + 1) events per call
   std::vector<cudaEvent_t> events;
@@ -38,10 +38,10 @@ const char* const kKernelNames[kKernels] = {"velo_cluster", "scan_clusters", "ve
 constexpr size_t kAlign = 256;
 inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
-// bytes per slab entry (two 16-byte records + checksum), tracking scratch per cluster (link, hits_slab) and per track
+// bytes per slab entry (two 16-byte records + checksum), tracking scratch per cluster (link, hits_slab, fwd_win, trip) and per track
 // slot (trk_hitoff, trk_fit, trk_final; one slot per 3 clusters)
 constexpr size_t kSlabEntryBytes = 16 + 16 + 4;
-constexpr size_t kTrackScratchBytes = 2 + 2;
+constexpr size_t kTrackScratchBytes = 2 + 2 + 8 + 8;  // link, hits_slab, forwarding windows, seed candidates
 constexpr size_t kTrackSlotBytes = 4 + 16 + 4;
 
 struct Carve {
@@ -70,8 +70,9 @@ size_t fixed_bytes(uint32_t n_events, uint32_t n_layers, uint32_t n_mid_sms) {
   b += align_up((size_t)n_events * 8) + align_up(((size_t)n_events + 1) * 8);  // track counts, offsets
   b += align_up(scan_state_words(n_events) * 8);                  // scan state (tracks)
   b += align_up(n_events);                                        // class of every event
-  b += align_up((size_t)n_events * 4) * 4 + align_up(12 * 4);     // event lists of the larger instances, counters
-  b += align_up((size_t)n_events * 16);                           // size-binned event order of the first instance
+  b += align_up((size_t)n_events * 4) * 6 + align_up(16 * 4);     // event lists of the track kernels, event flags, counters
+  b += align_up((size_t)items * 4);                               // seed candidates per (event, layer)
+  b += align_up((size_t)items * kPhiTabStride * 2);               // phi look-up table per (event, layer)
   return b + 16 * kAlign;
 }
 
@@ -156,7 +157,7 @@ int allen_velo_create(const allen_velo_geometry_t* geo, allen_velo_t** out) {
   h->n_mid_sms = (uint32_t)n_sm + 16;  // %smid is below the SM count on the parts seen; margin for gaps in the numbering
   for (int i = 0; i < 2; ++i)
     if (cudaStreamCreateWithFlags(&h->side[i], cudaStreamNonBlocking) != cudaSuccess) { allen_velo_destroy(h); return ALLEN_VELO_ERR_CUDA; }
-  for (int i = 0; i < 3; ++i)
+  for (int i = 0; i < 5; ++i)
     if (cudaEventCreateWithFlags(&h->fork_join[i], cudaEventDisableTiming) != cudaSuccess) { allen_velo_destroy(h); return ALLEN_VELO_ERR_CUDA; }
   DeviceGeometry& g = h->dev;
   g.n_sensors = S; g.n_layers = L; g.n_cols = geo->n_cols; g.n_rows = geo->n_rows;
@@ -249,10 +250,11 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   unsigned long long* trk_offsets = cv.take<unsigned long long>((size_t)n_events + 1);
   unsigned long long* trk_scan_state = cv.take<unsigned long long>(scan_state_words(n_events));
   uint8_t* trk_level = cv.take<uint8_t>(n_events);
-  uint32_t* trk_lists[4];
+  uint32_t* trk_lists[6];
   for (uint32_t*& p : trk_lists) p = cv.take<uint32_t>(n_events);
-  uint32_t* trk_counters = cv.take<uint32_t>(12);
-  uint32_t* trk_order = cv.take<uint32_t>((size_t)n_events * 4);
+  uint32_t* trk_counters = cv.take<uint32_t>(16);
+  uint32_t* trip_count = cv.take<uint32_t>(items);
+  uint16_t* phi_tab = cv.take<uint16_t>((size_t)items * kPhiTabStride);
   size_t entries = (h->ws_bytes - cv.used - 16 * kAlign) / per_entry_bytes();
   if (entries > 0x7FFFFFF0u) entries = 0x7FFFFFF0u;
   ClusterSlab slab{};
@@ -262,9 +264,12 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   slab.info = cv.take<uint4>(entries);
   slab.checksum = cv.take<uint32_t>(entries);
   slab.spill_cursor = reinterpret_cast<uint32_t*>(state) + 1;
+  slab.phi_tab = phi_tab;
   // tracking scratch is addressed by output cluster index; it shares the entry count with the slab
   uint16_t* link = cv.take<uint16_t>(entries);
   uint16_t* hits_slab = cv.take<uint16_t>(entries);
+  uint2* fwd_win = cv.take<uint2>(entries);
+  unsigned long long* trip = cv.take<unsigned long long>(entries);
   uint32_t* trk_hitoff = cv.take<uint32_t>(entries / 3 + 1);
   float4* trk_fit = cv.take<float4>(entries / 3 + 1);
   uint32_t* trk_final = cv.take<uint32_t>(entries / 3 + 1);
@@ -325,10 +330,13 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   tl.trk_final = trk_final;
   tl.counts = trk_counts;
   tl.level = trk_level;
-  tl.ev_list[0] = trk_lists[0]; tl.ev_list[1] = trk_lists[1];
-  tl.redo_list[0] = trk_lists[2]; tl.redo_list[1] = trk_lists[3];
+  tl.flw_list[0] = trk_lists[0]; tl.flw_list[1] = trk_lists[1]; tl.flw_list[2] = trk_lists[2];
+  tl.redo_list[0] = trk_lists[3]; tl.redo_list[1] = trk_lists[4];
+  tl.ev_flags = trk_lists[5];
+  tl.fwd_win = fwd_win;
+  tl.trip = trip;
+  tl.trip_count = trip_count;
   tl.counters = trk_counters;
-  tl.order = trk_order;
   uint32_t n_track_launches = 0;
   if ((err = launch_track(tl, stream, h->side, h->fork_join, h->n_sms, &n_track_launches)) != cudaSuccess) return fail(h, ALLEN_VELO_ERR_CUDA, "track kernel", err);
   h->last_launches += n_track_launches;
@@ -347,6 +355,10 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   ct.trk_hitoff = trk_hitoff;
   ct.trk_fit = trk_fit;
   ct.offsets = trk_offsets;
+  ct.ev_flags = tl.ev_flags;
+  ct.trk_final = trk_final;
+  ct.link = link;
+  ct.s_weak = h->dev.params.s_weak;
   ct.out = *ot;
   if ((err = launch_compact_tracks(ct, stream)) != cudaSuccess) return fail(h, ALLEN_VELO_ERR_CUDA, "track compaction", err);
   h->last_launches++;

@@ -363,7 +363,13 @@ __device__ __forceinline__ void finish_layer(const ClusterLaunch& a, const Clust
     }
   }
   if (lane == 0) a.counts[item] = n_cl;
-  if (n_cl == 0) return;
+  // the phi look-up table of the layer for the track search (velo_seed.cu): first cluster of every slice of phi16
+  uint4* tab = reinterpret_cast<uint4*>(a.slab.phi_tab + (size_t)item * kPhiTabStride);
+  if (n_cl == 0) {
+    tab[lane] = make_uint4(0, 0, 0, 0);
+    if (lane == 0) tab[32] = make_uint4(0, 0, 0, 0);
+    return;
+  }
 #pragma unroll 1
   for (uint32_t s = lane; s < 256; s += 32) ss.cnt256[s] = 0;
   __syncwarp();
@@ -389,8 +395,12 @@ __device__ __forceinline__ void finish_layer(const ClusterLaunch& a, const Clust
       if (lane >= (uint32_t)d) incl += t;
     }
     uint32_t run = incl - sum;
+    uint32_t st[8];
 #pragma unroll
-    for (int q = 0; q < 8; ++q) { ss.cnt256[lane * 8 + q] = run; run += v[q]; }
+    for (int q = 0; q < 8; ++q) { ss.cnt256[lane * 8 + q] = run; st[q] = run; run += v[q]; }
+    // the exclusive sums are the table (the by-product of this sort that the track search wants): 8 entries per lane
+    tab[lane] = make_uint4(st[0] | (st[1] << 16), st[2] | (st[3] << 16), st[4] | (st[5] << 16), st[6] | (st[7] << 16));
+    if (lane == 0) tab[32] = make_uint4(n_cl, 0, 0, 0);
   }
   __syncwarp();
 #pragma unroll 1

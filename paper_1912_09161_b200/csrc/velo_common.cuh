@@ -37,7 +37,10 @@ struct ClusterSlab {
   uint4 *rec, *info;
   uint32_t* checksum;
   uint32_t* spill_cursor;  // entries handed out of [dense, capacity), zeroed by the launcher
+  uint16_t* phi_tab;       // [n_events*n_layers][kPhiTabStride] first cluster of every 256-unit slice of phi16 (+ total), per layer
 };
+constexpr uint32_t kPhiSlices = 256;      // the buckets of the cluster kernel's counting sort on the top byte of phi16
+constexpr uint32_t kPhiTabStride = 264;   // u16 per (event, layer): kPhiSlices + 1 entries, padded to 16 bytes
 
 // ---- small device helpers -------------------------------------------------------------------
 __device__ __forceinline__ uint32_t lane_id() { return threadIdx.x & 31u; }
@@ -164,13 +167,16 @@ struct TrackLaunch {
   uint16_t* hits_slab;             // [cluster capacity] hit lists of the event's output tracks, back to back
   uint32_t* trk_hitoff;            // [capacity/3+1] event-local first entry in hits_slab of every output track
   float4* trk_fit;                 // [capacity/3+1] x0, y0, tx, ty
-  uint32_t* trk_final;             // [capacity/3+1] flat kernel: final state of every track by order of creation
+  uint32_t* trk_final;             // [capacity/3+1] final state of every track by order of creation
   unsigned long long* counts;      // [n_events] (n_tracks << 32) | n_track_hits
-  uint8_t* level;                  // [n_events] class of the event (velo_track.cuh): flat kernel, 512 / 1024-hit CTA instance, copy only, nothing
-  uint32_t* ev_list[2];            // [n_events] each: events of level 1 / 2
-  uint32_t* redo_list[2];          // [n_events] each: events the flat kernel / the 512-hit instance ran out of track slots on
-  uint32_t* order;                 // [4][n_events] events of the flat kernel by size bin
-  uint32_t* counters;              // [12] list sizes and cursors, zeroed by the launcher
+  uint8_t* level;                  // [n_events] class of the event (velo_track.cuh): hits per layer 256 / 512 / 1024, copy only, nothing
+  uint2* fwd_win;                  // [cluster capacity] velo_seed.cu: forwarding phi windows of every hit (layer below, the one below that)
+  unsigned long long* trip;        // [cluster capacity] velo_seed.cu: seed candidates of every (event, layer B), at the layer's hits
+  uint32_t* trip_count;            // [n_events*n_layers] entries in the list of every (event, layer)
+  uint32_t* ev_flags;              // [n_events] kEvRedo: the event goes to the CTA-per-event kernel
+  uint32_t* flw_list[3];           // [n_events] each: events of class 0 / 1 / 2 (velo_follow.cu)
+  uint32_t* redo_list[2];          // [n_events] each: events for the CTA-per-event kernel with 512 / 1024 hits per layer
+  uint32_t* counters;              // [kCtrCount] list sizes and cursors (velo_track.cuh), zeroed by the launcher
 };
 cudaError_t launch_track(const TrackLaunch& a, cudaStream_t stream, cudaStream_t* side, cudaEvent_t* ev,
                          uint32_t n_sms, uint32_t* n_launches);
@@ -185,6 +191,10 @@ struct CompactTracksLaunch {
   const uint32_t* trk_hitoff;
   const float4* trk_fit;
   const unsigned long long* offsets;  // [n_events+1] exclusive scan of counts
+  const uint32_t* ev_flags;           // [n_events] kEvFinal: tracks as final states + links (velo_follow.cu), else as slabs
+  const uint32_t* trk_final;
+  const uint16_t* link;
+  float s_weak;
   allen_velo_tracks_t out;
 };
 cudaError_t launch_compact_tracks(const CompactTracksLaunch& a, cudaStream_t stream);

@@ -1,5 +1,5 @@
-// Kernel 2 of the VELO hot path, CTA-per-event instances for events whose busiest layer exceeds what the flattened
-// kernel (velo_track_flat.cu) stages, and the second pass for events that ran out of its track slots: search by triplet
+// Kernel 2 of the VELO hot path, CTA-per-event instances: the second pass for the events the two-kernel path
+// (velo_seed.cu + velo_follow.cu) hands on (seed list or track slots exhausted, event too large to stage): search by triplet
 // (A5 seeding, A6 forwarding, A7 clone/ghost killing) and the straight-line fit (A8) — SURVEY.md §8(a); the algorithm is DESIGN.md reading R5 (T1..T5) of P:181-183 ("forming
 // seeds of three hits from consecutive layers ('triplets'), and then extending these to the other layers"; "sort hits
 // on every layer by phi for fast look-up") and R6 of P:149 (straight lines).
@@ -42,7 +42,7 @@ struct Cfg {
   static constexpr int kRoundsB = (kCap + kThreads - 1) / kThreads;
   static constexpr int kRoundsT = (kCapTracks + kThreads - 1) / kThreads;
 };
-// second pass for events the flat kernel ran out of track or triplet slots on: their clusters are already in the output
+// second pass for events the two-kernel path ran out of track or list slots on: their clusters are already in the output
 using CfgMr = Cfg<256, 512, 1024, 4096, 1, false, false>;
 using CfgLr = Cfg<512, 1024, 2048, 2048, 2, true, false>;
 
@@ -507,7 +507,7 @@ __device__ __forceinline__ void track_event(const TrackLaunch& a, uint32_t e, Sm
   if (sm.flags) {  // out of track slots: the next larger instance redoes the event in the second pass
     if (tid == 0) {
       if (C::kLast) { atomicOr(a.clusters.status + e, ALLEN_VELO_STATUS_STAGE_OVERFLOW); a.counts[e] = 0; }
-      else a.redo_list[C::kLevel][atomicAdd(a.counters + 2 + C::kLevel, 1u)] = e;
+      else a.redo_list[C::kLevel][atomicAdd(a.counters + kCtrRedo + C::kLevel, 1u)] = e;
     }
     return;
   }
@@ -603,26 +603,104 @@ __global__ void __launch_bounds__(128) compact_tracks_kernel(const CompactTracks
   }
   const uint32_t co = a.clusters.event_offsets[e];
   const uint32_t trk0 = co / 3;
+  const uint32_t fl = a.ev_flags[e];
+  if (fl & kEvFinal) {
+    // ---- tracks as velo_follow.cu left them: final state of every track by order of creation + links between the hits.
+    //      T5 (R5): keep >= 4 hits, or 3 hits with S_seed <= s_weak (bit 15 of the state).  A thread per track: offsets by
+    //      a block scan in order of creation, hit list by walking the links back from the newest hit, then A8: the
+    //      oracle's operations in the oracle's order (R6: fp64 means, then centred sums, over the hits in order
+    //      of addition, from the fp32 coordinates) -> bit-identical parameters.
+    __shared__ uint32_t warp_tot[4];
+    const uint32_t n_created = fl >> 8, lane = lane_id(), warp = threadIdx.x >> 5;
+    const uint16_t* link = a.link + co;
+    const float* X = a.clusters.x + co;
+    const float* Y = a.clusters.y + co;
+    const float* Z = a.clusters.z + co;
+    uint32_t run_t = 0, run_h = 0;
 #pragma unroll 1
-  for (uint32_t t = threadIdx.x; t < nT; t += blockDim.x) {
-    const float4 f = a.trk_fit[trk0 + t];
-    a.out.x0[T0 + t] = f.x; a.out.y0[T0 + t] = f.y; a.out.tx[T0 + t] = f.z; a.out.ty[T0 + t] = f.w;
-    a.out.hit_offsets[T0 + t] = H0 + a.trk_hitoff[trk0 + t];
+    for (uint32_t base = 0; base < n_created; base += 128) {
+      const uint32_t t = base + threadIdx.x;
+      uint32_t n = 0, st = 0;
+      if (t < n_created) {
+        st = a.trk_final[trk0 + t];
+        n = track_n_hits(st);
+        if (n == 3 && !(st & 0x8000u)) n = 0;
+      }
+      const uint32_t v = n ? ((1u << 20) | n) : 0u;
+      uint32_t incl = v;
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t u = __shfl_up_sync(kFull, incl, d);
+        if (lane >= (uint32_t)d) incl += u;
+      }
+      if (lane == 31) warp_tot[warp] = incl;
+      __syncthreads();
+      uint32_t off = incl - v, total = 0;
+#pragma unroll
+      for (int w = 0; w < 4; ++w) {
+        const uint32_t u = warp_tot[w];
+        if (w < (int)warp) off += u;
+        total += u;
+      }
+      __syncthreads();
+      if (n) {
+        const uint32_t ot = T0 + run_t + (off >> 20), oh = H0 + run_h + (off & 0xFFFFFu);
+        uint16_t* out_h = a.out.hits + oh;
+        uint32_t h = st >> 16;
+#pragma unroll 1
+        for (int k = (int)n - 1; k >= 0; --k) {
+          out_h[k] = (uint16_t)h;
+          if (k) h = link[h];
+        }
+        const double dn = (double)n;
+        double zm = 0, xm = 0, ym = 0;
+#pragma unroll 1
+        for (uint32_t k = 0; k < n; ++k) {
+          h = out_h[k];
+          zm += (double)Z[h]; xm += (double)X[h]; ym += (double)Y[h];
+        }
+        zm /= dn; xm /= dn; ym /= dn;
+        double szz = 0, szx = 0, szy = 0;
+#pragma unroll 1
+        for (uint32_t k = 0; k < n; ++k) {
+          h = out_h[k];
+          const double dz = (double)Z[h] - zm;
+          szz += dz * dz;
+          szx += dz * ((double)X[h] - xm);
+          szy += dz * ((double)Y[h] - ym);
+        }
+        const double tx = szx / szz, ty = szy / szz;
+        a.out.x0[ot] = (float)(xm - tx * zm); a.out.y0[ot] = (float)(ym - ty * zm);
+        a.out.tx[ot] = (float)tx; a.out.ty[ot] = (float)ty;
+        a.out.hit_offsets[ot] = oh;
+      }
+      run_t += total >> 20;
+      run_h += total & 0xFFFFFu;
+    }
+  } else {
+    // ---- tracks as the CTA-per-event kernel left them: hit lists and fits in per-event slabs
+#pragma unroll 1
+    for (uint32_t t = threadIdx.x; t < nT; t += blockDim.x) {
+      const float4 f = a.trk_fit[trk0 + t];
+      a.out.x0[T0 + t] = f.x; a.out.y0[T0 + t] = f.y; a.out.tx[T0 + t] = f.z; a.out.ty[T0 + t] = f.w;
+      a.out.hit_offsets[T0 + t] = H0 + a.trk_hitoff[trk0 + t];
+    }
+#pragma unroll 1
+    for (uint32_t k = threadIdx.x; k < nH; k += blockDim.x) a.out.hits[H0 + k] = a.hits_slab[co + k];
   }
-#pragma unroll 1
-  for (uint32_t k = threadIdx.x; k < nH; k += blockDim.x) a.out.hits[H0 + k] = a.hits_slab[co + k];
   // ---- simple Kalman fit (R9), one thread per track, x and y independent: start at the first hit
   //      with (measured position, slope 0), C = diag(var_m, 1); per further hit add the scattering of a 400 MeV pT
   //      track to C11, propagate, update.  (1 - K0) = var_m / S keeps the covariance update free of cancellation.
   if (a.out.kalman) {
+    __syncthreads();  // the hit lists above are complete
     const float* X = a.clusters.x + co;
     const float* Y = a.clusters.y + co;
     const float* Z = a.clusters.z + co;
     const float var_m = a.pitch * a.pitch * (1.0f / 12.0f);
 #pragma unroll 1
     for (uint32_t t = threadIdx.x; t < nT; t += blockDim.x) {
-      const uint32_t h0 = a.trk_hitoff[trk0 + t], h1 = t + 1 < nT ? a.trk_hitoff[trk0 + t + 1] : nH;
-      const uint16_t* hits = a.hits_slab + co + h0;
+      const uint32_t h0 = a.out.hit_offsets[T0 + t], h1 = t + 1 < nT ? a.out.hit_offsets[T0 + t + 1] : H0 + nH;
+      const uint16_t* hits = a.out.hits + h0;
       uint32_t h = hits[0], hn = hits[1];
       float zp = Z[h];
       const float dz01 = Z[hn] - zp, tx0 = (X[hn] - X[h]) / dz01, ty0 = (Y[hn] - Y[h]) / dz01;
@@ -671,10 +749,8 @@ __global__ void __launch_bounds__(128) compact_tracks_kernel(const CompactTracks
   }
 }
 
-// One thread per event: class of the event (which instance searches it, or copy only / nothing) and the event lists
-// of the two larger instances.  counters: [0], [1] events of level 1, 2; [2], [3] second-pass events; [4..7] cursors;
-// [8..11] events of the flat kernel (and copy-only events) in four size bins: it takes them largest first, so that the
-// last warps of the grid are short ones.
+// One thread per event: class of the event (hits per layer its search needs, or copy only / nothing) and the event lists of
+// the three instances of velo_follow.cu.
 __global__ void __launch_bounds__(256) classify_events_kernel(const __grid_constant__ TrackLaunch a) {
   const uint32_t e = blockIdx.x * blockDim.x + threadIdx.x;
   if (e >= a.n_events) return;
@@ -708,14 +784,10 @@ __global__ void __launch_bounds__(256) classify_events_kernel(const __grid_const
       atomicOr(a.clusters.status + e, ALLEN_VELO_STATUS_STAGE_OVERFLOW);
       cls = kClsCopy;
     }
-    if (cls == kClsMid || cls == kClsLarge) a.ev_list[cls - 1][atomicAdd(a.counters + (cls - 1), 1u)] = e;
-  }
-  if (cls == kClsFlat || cls == kClsCopy) {
-    const uint32_t avg = a.clusters.event_offsets[a.n_events] / a.n_events + 1u;
-    const uint32_t bin = cls == kClsCopy ? 3u : 20u * n_cl >= 30u * avg ? 0u : 20u * n_cl >= 23u * avg ? 1u : 20u * n_cl >= 17u * avg ? 2u : 3u;
-    a.order[(size_t)bin * a.n_events + atomicAdd(a.counters + 8 + bin, 1u)] = e;
+    if (cls <= kClsLarge) a.flw_list[cls][atomicAdd(a.counters + kCtrFollow + cls, 1u)] = e;
   }
   a.level[e] = cls;
+  a.ev_flags[e] = 0;
   if (cls >= kClsCopy) a.counts[e] = 0;
 }
 
@@ -747,9 +819,8 @@ cudaError_t prepare_list() {
 
 template <class C>
 cudaError_t launch_list(const TrackLaunch& a, uint32_t which, uint32_t grid, cudaStream_t stream) {
-  const uint32_t* list = which < 2 ? a.ev_list[which] : a.redo_list[which - 2];
-  velo_track_list_kernel<C><<<grid, C::kBlock, sizeof(Smem<C>), stream>>>(a, list, a.counters + which,
-                                                                          a.counters + 4 + which);
+  velo_track_list_kernel<C><<<grid, C::kBlock, sizeof(Smem<C>), stream>>>(a, a.redo_list[which], a.counters + kCtrRedo + which,
+                                                                          a.counters + kCtrRedoCursor + which);
   return cudaGetLastError();
 }
 
@@ -757,43 +828,44 @@ cudaError_t launch_list(const TrackLaunch& a, uint32_t which, uint32_t grid, cud
 
 // Once per process (allen_velo_create): the kernels' dynamic shared-memory limits.
 cudaError_t track_prepare() {
-  cudaError_t err = track_flat_prepare();
+  cudaError_t err = seed_prepare();
+  if (err == cudaSuccess) err = follow_prepare();
   if (err == cudaSuccess) err = prepare_list<CfgMr>();
   if (err == cudaSuccess) err = prepare_list<CfgLr>();
   return err;
 }
 
-// classify -> [flat kernel over the events of its class | 512-hit list | 1024-hit list, on three streams] -> second pass
-// for events that ran out of track slots (512-hit instance, then 1024).  `side`/`ev`: two extra streams and three events
-// owned by the handle; everything is ordered after and before the work on `stream` by events (a fork/join a CUDA graph
-// can capture), nothing synchronises.
-cudaError_t launch_track(const TrackLaunch& a, cudaStream_t stream, cudaStream_t* side, cudaEvent_t* ev,
-                         uint32_t n_sms, uint32_t* n_launches) {
+// classify -> velo_seed -> velo_follow (three instances beside each other)
+// -> second pass (CTA per event, 512 hits per layer, then 1024) for the events those handed on.  `side`/`ev`: two extra
+// streams and five events owned by the handle; everything is ordered after and before the work on `stream` by events (a
+// fork/join a CUDA graph can capture), nothing synchronises.
+cudaError_t launch_track(const TrackLaunch& a, cudaStream_t stream, cudaStream_t* side, cudaEvent_t* ev, uint32_t n_sms,
+                         uint32_t* n_launches) {
   *n_launches = 0;
   if (a.n_events == 0) return cudaSuccess;
-  cudaError_t err = cudaMemsetAsync(a.counters, 0, 12 * sizeof(uint32_t), stream);
+  cudaError_t err = cudaMemsetAsync(a.counters, 0, kCtrCount * sizeof(uint32_t), stream);
   if (err != cudaSuccess) return err;
   classify_events_kernel<<<(a.n_events + 255) / 256, 256, 0, stream>>>(a);
   if ((err = cudaGetLastError()) != cudaSuccess) return err;
   ++*n_launches;
-  if ((err = cudaEventRecord(ev[0], stream)) != cudaSuccess) return err;
-  if ((err = cudaStreamWaitEvent(side[0], ev[0], 0)) != cudaSuccess) return err;
-  if ((err = cudaStreamWaitEvent(side[1], ev[0], 0)) != cudaSuccess) return err;
-
-  const uint32_t grid_m = min(a.n_events, 3 * n_sms), grid_l = min(a.n_events, n_sms);
-  if ((err = launch_track_flat_list(a, 0, min(a.n_events, 4 * n_sms), side[0])) != cudaSuccess) return err;
+  if ((err = launch_seed(a, stream)) != cudaSuccess) return err;
   ++*n_launches;
-  if ((err = launch_track_flat_list(a, 1, min(a.n_events, 2 * n_sms), side[1])) != cudaSuccess) return err;
+  if ((err = cudaEventRecord(ev[2], stream)) != cudaSuccess) return err;
+  if ((err = cudaStreamWaitEvent(side[0], ev[2], 0)) != cudaSuccess) return err;
+  if ((err = cudaStreamWaitEvent(side[1], ev[2], 0)) != cudaSuccess) return err;
+  if ((err = launch_follow(a, 1, n_sms, side[0])) != cudaSuccess) return err;
   ++*n_launches;
-  if ((err = launch_track_flat(a, stream)) != cudaSuccess) return err;
+  if ((err = launch_follow(a, 2, n_sms, side[1])) != cudaSuccess) return err;
   ++*n_launches;
-  if ((err = cudaEventRecord(ev[1], side[0])) != cudaSuccess) return err;
-  if ((err = cudaEventRecord(ev[2], side[1])) != cudaSuccess) return err;
-  if ((err = cudaStreamWaitEvent(stream, ev[1], 0)) != cudaSuccess) return err;
-  if ((err = cudaStreamWaitEvent(stream, ev[2], 0)) != cudaSuccess) return err;
-  if ((err = launch_list<CfgMr>(a, 2, min(grid_m, 2 * n_sms), stream)) != cudaSuccess) return err;
+  if ((err = launch_follow(a, 0, n_sms, stream)) != cudaSuccess) return err;
   ++*n_launches;
-  if ((err = launch_list<CfgLr>(a, 3, grid_l, stream)) != cudaSuccess) return err;
+  if ((err = cudaEventRecord(ev[3], side[0])) != cudaSuccess) return err;
+  if ((err = cudaEventRecord(ev[4], side[1])) != cudaSuccess) return err;
+  if ((err = cudaStreamWaitEvent(stream, ev[3], 0)) != cudaSuccess) return err;
+  if ((err = cudaStreamWaitEvent(stream, ev[4], 0)) != cudaSuccess) return err;
+  if ((err = launch_list<CfgMr>(a, 0, min(a.n_events, 2 * n_sms), stream)) != cudaSuccess) return err;
+  ++*n_launches;
+  if ((err = launch_list<CfgLr>(a, 1, min(a.n_events, n_sms), stream)) != cudaSuccess) return err;
   ++*n_launches;
   return cudaSuccess;
 }
