@@ -2,6 +2,10 @@
 """bench.py — VELO events/s on B200 for the nu=6, 10k-event batch (BASELINE.json metric), with roofline and CPU baseline.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--events 10000] [--impl ours|reference]
+    python bench.py --sweep            # BASELINE.json configs[4] (500 / 2 000 / 10 000 / 50 000 events at nu = 6) and
+                                       # configs[3] (nu = 12, 10 000 events): one JSON line per point, the headline last
+    python bench.py --paper-protocol   # e2e as the paper measures: 12 streams x 1000-event chunks, 100
+                                       # repetitions, mean +- sigma over 10 different event sets
 
 A "step" is one pass of the whole hot path (allen_velo_reconstruct: decode -> cluster -> phi sort -> search by triplet
 -> fit -> compaction) over one batch of synthetic events.  `value` is events/s with inputs resident in
@@ -42,17 +46,33 @@ def peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def source_hash():
+    """Hash of the CUDA sources the library is built from: the committed ncu counters name the sources they were taken
+    with, and are not used for any other (the GPU box has the sources, not the git history)."""
+    import glob
+    import hashlib
+
+    h = hashlib.sha256()
+    for path in sorted(glob.glob(os.path.join(ROOT, "paper_1912_09161_b200", "csrc", "*"))):
+        h.update(os.path.basename(path).encode())
+        with open(path, "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()[:16]
+
+
 def ncu_counters(workload_key):
     """Per-kernel counters of one launch from the newest profiles/*_counters.csv (written from an `ncu --set full`
-    capture of this very command; the file names the command).  {} if there is none for this workload."""
+    capture of this very command; the file names the command).  Only rows whose `source_hash` equals the hash of the
+    sources in the tree are used: counters of other sources would divide a stale count by a fresh time."""
     import csv
     import glob
 
     out = {}
+    want = source_hash()
     for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_counters.csv"))):
         with open(path) as f:
             for row in csv.DictReader(f):
-                if row["workload"] == workload_key:
+                if row.get("workload") == workload_key and row.get("source_hash") == want:
                     out[row["kernel"]] = dict(dram_bytes=int(row["dram_read_bytes"]) + int(row["dram_write_bytes"]),
                                               warp_instructions=int(row["warp_instructions"]),
                                               lanes=float(row["active_lanes_per_instruction"]))
@@ -128,9 +148,10 @@ def algorithmic_bytes(n_events, n_layers, raw_bytes, n_clusters, n_tracks, n_tra
     tracks = 4 * (n_events + 1) + 4 * (n_tracks + 1) + 2 * n_track_hits + 16 * n_tracks
     return dict(raw=raw, clusters=clusters, tracks=tracks, total=raw + clusters + tracks,
                 # per-kernel shares: each compulsory byte is charged to the kernel that moves it.  The
-                # cluster kernel reads the raw banks; the track kernel writes the compacted clusters (it carries the
-                # compaction) and the tracks.  The slab between the two is overhead, not algorithmic traffic.
-                velo_cluster=raw, velo_track=clusters + tracks)
+                # cluster kernel reads the raw banks; the seed kernel writes the compacted clusters (it carries that
+                # compaction); follow + compact_tracks write the tracks.  The slab, the candidate lists and the
+                # forwarding windows between them are overhead, not algorithmic traffic.
+                velo_cluster=raw, velo_seed=clusters, velo_follow=tracks, compact_tracks=tracks)
 
 
 def run_reference(args):
@@ -163,7 +184,9 @@ def run_reference(args):
     return 0
 
 
-def run_ours(args):
+def measure_ours(args, headline=True):
+    """One measurement of the hot path on args.config / args.events.  headline=False (points of --sweep): no single-call
+    e2e, no CPU baseline, no near-cut comparison.  Returns the JSON line as a dict (None on ranks other than 0)."""
     import torch
 
     from paper_1912_09161_b200 import binding, workload
@@ -278,20 +301,26 @@ def run_ours(args):
         stream.synchronize()
         d2h_holder[0] = 4 * (n_events + 1) * 2 + 4 * n_events + 4 * (nt + 1) + 16 * nt + 2 * nh
 
-    for _ in range(2):
-        e2e_step()
-    barrier()
-    torch.cuda.synchronize()
-    e0 = time.time()
-    for _ in range(args.steps):
-        e2e_step()
-    torch.cuda.synchronize()
-    e1 = time.time()
-    barrier()
-    single_ms = max_over_ranks((e1 - e0) * 1e3 / args.steps)
-    single_value = total_events / (single_ms * 1e-3)
+    e0 = e1 = time.time()
+    single_ms = single_value = None
+    if headline:
+        for _ in range(2):
+            e2e_step()
+        barrier()
+        torch.cuda.synchronize()
+        e0 = time.time()
+        for _ in range(args.steps):
+            e2e_step()
+        torch.cuda.synchronize()
+        e1 = time.time()
+        barrier()
+        single_ms = max_over_ranks((e1 - e0) * 1e3 / args.steps)
+        single_value = total_events / (single_ms * 1e-3)
 
     # ---- the same, streamed: chunks of the batch on several streams so that copies and kernels overlap
+    paper = None
+    if headline and args.paper_protocol and world == 1:
+        paper = paper_protocol(args, geo, device)
     chunk = min(args.e2e_chunk, n_events)
     chunk_raw = int(1.25 * raw_bytes * chunk / n_events) + (1 << 20)
     sv = binding.StreamedVelo(geo, chunk, chunk_raw, n_streams=args.e2e_streams, device=device)
@@ -318,7 +347,7 @@ def run_ours(args):
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
-        return 0
+        return None
 
     # ---- roofline of the dominant kernel (own algorithmic bytes / own mean duration) and of the whole path
     names = velo.kernel_names()
@@ -349,8 +378,8 @@ def run_ours(args):
                          frac_of_8TBs_nominal=path_gbs / 8000.0, algorithmic_bytes_per_step=ab["total"],
                          bytes_per_event=ab["total"] / n_events)
 
-    cpu_baseline = None
-    if world == 1 and not args.no_cpu_baseline:
+    cpu_baseline = near_cut = None
+    if headline and world == 1 and not args.no_cpu_baseline:
         import oracle
 
         cores = os.cpu_count() or 1
@@ -364,10 +393,29 @@ def run_ours(args):
         t0 = time.perf_counter()
         oracle.reconstruct(geo, subm.raw, subm.event_offsets, n_threads=cores, export=False)
         multi = nm / (time.perf_counter() - t0)
-        cpu_baseline = dict(value=multi, unit=UNIT, cores=cores, kind="oracle",
+        cpu_baseline = dict(value=multi, unit=UNIT, cores=cores, kind="oracle (a plain, unoptimised restatement of the "
+                            "paper's definitions: linear window scans, no phi look-up; a reported baseline, not a target)",
                             sample=f"first {nm} events of the same batch on {cores} threads (contiguous ranges); "
                                    f"single thread over the first {n1} events: {single:.1f} events/s",
                             single_thread_value=single)
+        # near-cut accounting (BASELINE.json: "counted and reported"): the oracle's log over the same sample, and the
+        # tracks of the timed batch that differ from the oracle's on it (outside the timed regions)
+        ref = oracle.reconstruct(geo, subm.raw, subm.event_offsets, n_threads=cores)
+        rt = ref.tracks
+        g_ho = ot.hit_offsets.cpu().numpy().view(np.uint32)
+        g_hits = ot.hits.cpu().numpy().view(np.uint16)
+        t1 = int(te[nm])
+        same = (np.array_equal(te[:nm + 1], rt.event_offsets) and np.array_equal(g_ho[:t1 + 1], rt.hit_offsets)
+                and np.array_equal(g_hits[:int(g_ho[t1])], rt.hits))
+        mismatched = 0
+        if not same:
+            for e in range(nm):
+                got = {tuple(sorted(g_hits[g_ho[t]:g_ho[t + 1]].tolist())) for t in range(int(te[e]), int(te[e + 1]))}
+                want = set(rt.hit_sets(e))
+                mismatched += len(got ^ want)
+        near_cut = dict(events=nm, tracks=int(rt.event_offsets[-1]), near_cut_decisions=int(ref.near_cut_per_event.sum()),
+                        events_with_near_cut_decisions=int((ref.near_cut_per_event > 0).sum()),
+                        near_cut_mismatches=mismatched, identical_hit_lists_and_order=bool(same))
 
     line = dict(
         metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
@@ -381,16 +429,74 @@ def run_ours(args):
                     raw_bytes_per_event=raw_bytes / n_events, generator_s=round(t_gen, 2)),
         e2e=dict(value=e2e_value, unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h_holder[0],
                  ms_per_step=e2e_ms, how=f"binding.StreamedVelo: chunks of {chunk} events on {args.e2e_streams} streams, "
-                                         "pinned host buffers, H2D raw + offsets and D2H tracks inside the timed region",
-                 single_call=dict(value=single_value, ms_per_step=single_ms)),
+                                         "pinned host buffers, H2D raw + offsets and D2H tracks inside the timed region; "
+                                         "the clusters stay on the device (P:132: only tracks and vertices are copied back)",
+                 single_call=dict(value=single_value, ms_per_step=single_ms) if single_ms else None,
+                 paper_protocol=paper),
         gpu_launches=launches,
         kernels={n: float(m) for n, m in zip(names, mean_ms)},
         roofline=roofline, roofline_path=roofline_path, roofline_issue=roofline_issue, cpu_baseline=cpu_baseline,
-        clocks=clocks,
+        near_cut=near_cut, clocks=clocks, source_hash=source_hash(),
     )
-    print(json.dumps(line, default=float))
     if dist is not None:
         dist.destroy_process_group()
+    return line
+
+
+def paper_protocol(args, geo, device):
+    """The paper's own throughput protocol: 12 host-thread/stream pairs with 1000 events each, processed 100
+    times, for 10 different sets of events; mean and standard deviation over the sets.  Here: binding.StreamedVelo with
+    12 streams and 1000-event chunks over a 12 000-event batch (every stream one chunk per repetition), H2D of the raw
+    banks and D2H of the tracks inside the timed region, wall clock from the first launch to the last stream's return."""
+    import torch
+
+    from paper_1912_09161_b200 import binding, workload
+
+    n_streams, chunk, reps, n_sets = 12, 1000, args.paper_reps, args.paper_sets
+    values = []
+    sv = None
+    for k in range(n_sets):
+        batch = workload.generate(args.config, n_events=n_streams * chunk, batch_index=100 + k)
+        if sv is None:
+            sv = binding.StreamedVelo(geo, chunk, int(1.3 * batch.raw.size / n_streams) + (1 << 20), n_streams=n_streams,
+                                      device=device)
+        h_raw = torch.from_numpy(batch.raw).pin_memory()
+        off64 = batch.event_offsets.astype(np.int64)
+        sv.reconstruct(h_raw, off64)
+        torch.cuda.synchronize()
+        t0 = time.time()
+        for _ in range(reps):
+            sv.reconstruct(h_raw, off64)
+        torch.cuda.synchronize()
+        values.append(batch.n_events * reps / (time.time() - t0))
+    sv.destroy()
+    return dict(value=float(np.mean(values)), sigma=float(np.std(values)), unit=UNIT, streams=n_streams, events_per_stream=chunk,
+                repetitions=reps, event_sets=n_sets, per_set=[float(v) for v in values],
+                how="P:277-279 with binding.StreamedVelo; copies inside the timed region, clusters stay on the device")
+
+
+def run_ours(args):
+    import copy
+
+    if args.sweep:
+        if env_int("WORLD_SIZE", 1) != 1:
+            raise RuntimeError("--sweep is a single-GPU measurement")
+        for config, events in ((2, 500), (2, 2000), (2, 50000), (3, 10000)):
+            a = copy.copy(args)
+            a.config, a.events = config, events
+            line = measure_ours(a, headline=False)
+            line["sweep_point"] = True
+            print(json.dumps(line, default=float), flush=True)
+            import gc
+
+            import torch
+
+            del line
+            gc.collect()
+            torch.cuda.empty_cache()
+    line = measure_ours(args, headline=True)
+    if line is not None:
+        print(json.dumps(line, default=float))
     return 0
 
 
@@ -412,6 +518,13 @@ def main():
                     help="also find primary vertices (SURVEY 8(f2), beyond the headline path; implies --with-kalman)")
     ap.add_argument("--e2e-chunk", type=int, default=1250, help="events per chunk of the streamed end-to-end run")
     ap.add_argument("--e2e-streams", type=int, default=4)
+    ap.add_argument("--sweep", action="store_true",
+                    help="also measure BASELINE.json configs[4] (500 / 2k / 50k events) and configs[3] (nu = 12): one line each, "
+                         "the headline line last")
+    ap.add_argument("--paper-protocol", action="store_true",
+                    help="add e2e.paper_protocol: 12 streams x 1000-event chunks, repeated, mean +- sigma over event sets (P:277-279)")
+    ap.add_argument("--paper-reps", type=int, default=100)
+    ap.add_argument("--paper-sets", type=int, default=10)
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

@@ -28,13 +28,13 @@ extern "C" {
 #define ALLEN_VELO_OK 0
 #define ALLEN_VELO_ERR_INVALID (-1)   /* null pointer, misalignment, unsupported geometry or parameter */
 #define ALLEN_VELO_ERR_CUDA (-2)      /* a CUDA runtime call failed (cudaGetLastError text via allen_velo_last_error) */
-#define ALLEN_VELO_ERR_WORKSPACE (-3) /* workspace missing or smaller than allen_velo_workspace_bytes() */
+#define ALLEN_VELO_ERR_WORKSPACE (-3) /* workspace missing, or too small for the per-event tables of n_events plus a minimal slab */
 
 /* ---- per-event status bits (asynchronous conditions, written to clusters.status[e]; R8) ---- */
 #define ALLEN_VELO_STATUS_BAD_HEADER 1u         /* magic / bank count / sizes / offsets inconsistent: event skipped */
 #define ALLEN_VELO_STATUS_BAD_SP 2u             /* an SP word addressed a pixel outside the sensor: word ignored */
 #define ALLEN_VELO_STATUS_TOO_MANY_CLUSTERS 4u  /* > 65535 clusters: clusters written, tracking skipped */
-#define ALLEN_VELO_STATUS_CLUSTER_CAPACITY 8u   /* out_clusters.capacity exceeded: layers of this event that do not fit are not written */
+#define ALLEN_VELO_STATUS_CLUSTER_CAPACITY 8u   /* out_clusters.capacity exceeded: this event's clusters (and tracks) are not written */
 #define ALLEN_VELO_STATUS_TRACK_CAPACITY 16u    /* out_tracks capacities exceeded: this event's tracks not written */
 #define ALLEN_VELO_STATUS_STAGE_OVERFLOW 32u    /* an on-chip staging capacity was exceeded: event incomplete */
 
@@ -90,7 +90,9 @@ typedef struct {
   uint32_t capacity_hits;
   uint32_t* event_offsets; /* DEVICE [n_events+1]        first track of every event */
   uint32_t* hit_offsets;   /* DEVICE [capacity_tracks+1] first entry of hits[] of every track; the last element
-                              [capacity_tracks] also receives the total number of hits (= hit_offsets[n_tracks]) */
+                              [capacity_tracks] always receives the total number of hits of the batch (the value
+                              hit_offsets[n_tracks] has when the tracks fit), also when TRACK_CAPACITY is flagged; the
+                              entries of the tracks that are written, and the end of the last of them, are valid */
   uint16_t* hits;          /* DEVICE [capacity_hits] */
   float* x0;               /* DEVICE [capacity_tracks] straight-line fit x(z) = x0 + tx*z, y(z) = y0 + ty*z (R6) */
   float* y0;
@@ -118,7 +120,11 @@ void allen_velo_default_params(allen_velo_params_t* params /* HOST out */);
  * ALLEN_VELO_ERR_INVALID (unsupported geometry / parameters) / ALLEN_VELO_ERR_CUDA. */
 int allen_velo_create(const allen_velo_geometry_t* geometry /* HOST */, allen_velo_t** out /* HOST out */);
 
-/* Upper bound of the scratch memory reconstruct() needs for a batch of n_events whose raw data take raw_bytes. */
+/* Upper bound of the scratch memory reconstruct() needs for a batch of n_events whose raw data take raw_bytes
+ * (0 if n_events * n_layers >= 2^31: such a batch is refused).  reconstruct() itself cannot know raw_bytes (the offsets
+ * are on the device): it returns ALLEN_VELO_ERR_WORKSPACE only if the workspace cannot hold the tables that scale with
+ * n_events plus a minimal slab; with a workspace smaller than this bound the events whose clusters do not fit the slab
+ * are flagged STAGE_OVERFLOW, nothing is written out of bounds. */
 size_t allen_velo_workspace_bytes(const allen_velo_t* handle, uint32_t n_events, size_t raw_bytes);
 
 /* Registers a caller-owned DEVICE buffer (256-byte aligned) as workspace for subsequent reconstruct() calls. */
@@ -143,22 +149,6 @@ int allen_velo_set_vertex_output(allen_velo_t* handle, const allen_velo_vertices
 int allen_velo_reconstruct(allen_velo_t* handle, const void* raw_banks, const uint32_t* event_offsets,
                            uint32_t n_events, void* cuda_stream,
                            const allen_velo_clusters_t* out_clusters, const allen_velo_tracks_t* out_tracks);
-
-/* Optional per-kernel timing for bench.py's roofline: keeps a ring of CUDA events for the next `n_calls`
- * reconstruct() calls (n_calls = 0 switches it off and frees the events).  Events are recorded on the caller's
- * stream between the kernels; nothing synchronises. */
-int allen_velo_enable_timing(allen_velo_t* handle, uint32_t n_calls);
-
-/* Kernels launched per reconstruct() call and their names (static strings), in launch order. */
-uint32_t allen_velo_kernel_count(void);
-const char* allen_velo_kernel_name(uint32_t i);
-
-/* Device time in ms of each kernel of call number `call` (0-based since enable_timing, modulo the ring size).
- * out_ms: HOST [allen_velo_kernel_count()].  The caller must have synchronised the stream first. */
-int allen_velo_kernel_times(allen_velo_t* handle, uint32_t call, float* out_ms /* HOST out */);
-
-/* Number of kernels the last reconstruct() call launched (bench.py's gpu_launches). */
-uint32_t allen_velo_last_launch_count(const allen_velo_t* handle);
 
 /* Text of the last CUDA error seen by this handle ("" if none).  HOST string owned by the handle. */
 const char* allen_velo_last_error(const allen_velo_t* handle);

@@ -84,6 +84,8 @@ def load_library():
         L.allen_velo_kernel_times.restype = ctypes.c_int
         L.allen_velo_last_launch_count.argtypes = [ctypes.c_void_p]
         L.allen_velo_last_launch_count.restype = ctypes.c_uint32
+        L.allen_velo_debug_track_counters.argtypes = [ctypes.c_void_p, ctypes.c_void_p]
+        L.allen_velo_debug_track_counters.restype = ctypes.c_int
         L.allen_velo_last_error.argtypes = [ctypes.c_void_p]
         L.allen_velo_last_error.restype = ctypes.c_char_p
         L.allen_velo_destroy.argtypes = [ctypes.c_void_p]
@@ -247,6 +249,14 @@ class AllenVelo:
 
     def last_launch_count(self) -> int:
         return int(self._lib.allen_velo_last_launch_count(self._h))
+
+    def track_counters(self) -> dict:
+        """List sizes of the track search of the last call (include/allen_velo_debug.h; synchronises the device)."""
+        out = (ctypes.c_uint32 * 16)()
+        rc = self._lib.allen_velo_debug_track_counters(self._h, out)
+        if rc != OK:
+            raise RuntimeError(f"allen_velo_debug_track_counters -> {rc}")
+        return dict(follow=[int(out[0]), int(out[1]), int(out[2])], second_pass=[int(out[12]), int(out[13])])
 
     def last_error(self) -> str:
         return self._lib.allen_velo_last_error(self._h).decode()

@@ -7,6 +7,7 @@
 #include <vector>
 
 #include "velo_common.cuh"
+#include "../../include/allen_velo_debug.h"
 
 using namespace velo;
 
@@ -17,12 +18,13 @@ struct allen_velo {
   void* ws = nullptr;
   size_t ws_bytes = 0;
   uint32_t last_launches = 0;
+  const uint32_t* last_track_counters = nullptr;  // device: list sizes of the last call (workspace memory)
   uint32_t n_mid_sms = 0;      // SM ids the mid-slot pool of the cluster kernel covers
   uint32_t n_sms = 0;
   uint32_t sp_words_per_layer = 0;  // caller's hint (0: none)
   allen_velo_vertices_t vertices{};  // optional primary-vertex output (vertices == nullptr: off)
   cudaStream_t side[2] = {nullptr, nullptr};  // the larger track-kernel instances run beside the first one
-  cudaEvent_t fork_join[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+  cudaEvent_t fork_join[3] = {nullptr, nullptr, nullptr};
   std::string last_error;
   // optional per-kernel timing: a ring of (kKernels + 1) events per call
   std::vector<cudaEvent_t> events;
@@ -32,8 +34,10 @@ struct allen_velo {
 
 namespace {
 
-constexpr uint32_t kKernels = 5;  // timed segments; velo_track is six launches (classification, three staging capacities, second pass)
-const char* const kKernelNames[kKernels] = {"velo_cluster", "scan_clusters", "velo_track", "scan_tracks",
+// timed segments: velo_cluster = prepare + the chain of cluster instances; velo_seed = classification + velo_seed_kernel;
+// velo_follow = the three instances of velo_follow_kernel + the second pass
+constexpr uint32_t kKernels = 6;
+const char* const kKernelNames[kKernels] = {"velo_cluster", "scan_clusters", "velo_seed", "velo_follow", "scan_tracks",
                                             "compact_tracks"};
 constexpr size_t kAlign = 256;
 inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
@@ -63,7 +67,7 @@ size_t fixed_bytes(uint32_t n_events, uint32_t n_layers, uint32_t n_mid_sms) {
   size_t b = 0;
   b += align_up((size_t)items * 4) * 2 + align_up((size_t)items * 18 * 4);  // counts, slab_base, layer descriptors
   b += align_up(scan_state_words(items) * 8);                     // scan state (clusters)
-  b += align_up(32 + (size_t)n_mid_sms * 4);                      // big-pool counter, slab spill cursor, deferred-item counters, mid masks
+  b += align_up(32 + (size_t)n_mid_sms * 4 + (size_t)(big_slots(items) + 31) / 32 * 4);  // slab spill cursor, deferred-item counters, mid and big masks
   b += align_up((size_t)items * 4) * 2;                           // deferred items of the cluster kernel (two lists)
   b += align_up((size_t)n_mid_sms * 32 * cluster_mid_slot_bytes());
   b += align_up((size_t)big_slots(items) * cluster_big_slot_bytes());
@@ -157,7 +161,7 @@ int allen_velo_create(const allen_velo_geometry_t* geo, allen_velo_t** out) {
   h->n_mid_sms = (uint32_t)n_sm + 16;  // %smid is below the SM count on the parts seen; margin for gaps in the numbering
   for (int i = 0; i < 2; ++i)
     if (cudaStreamCreateWithFlags(&h->side[i], cudaStreamNonBlocking) != cudaSuccess) { allen_velo_destroy(h); return ALLEN_VELO_ERR_CUDA; }
-  for (int i = 0; i < 5; ++i)
+  for (int i = 0; i < 3; ++i)
     if (cudaEventCreateWithFlags(&h->fork_join[i], cudaEventDisableTiming) != cudaSuccess) { allen_velo_destroy(h); return ALLEN_VELO_ERR_CUDA; }
   DeviceGeometry& g = h->dev;
   g.n_sensors = S; g.n_layers = L; g.n_cols = geo->n_cols; g.n_rows = geo->n_rows;
@@ -175,6 +179,7 @@ int allen_velo_create(const allen_velo_geometry_t* geo, allen_velo_t** out) {
 
 size_t allen_velo_workspace_bytes(const allen_velo_t* h, uint32_t n_events, size_t raw_bytes) {
   if (!h) return 0;
+  if ((uint64_t)n_events * h->dev.n_layers >= (1ull << 31)) return 0;  // reconstruct() refuses such a batch
   // slab and tracking scratch: two entries per raw word (a super-pixel holds at most two clusters): one in the dense
   // part of the slab, one behind it for layers with more clusters than SP words
   const size_t entries = raw_bytes / 2 + 4096;
@@ -238,8 +243,8 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   uint32_t* slab_base = cv.take<uint32_t>(items);
   uint32_t* desc = cv.take<uint32_t>((size_t)items * 18);
   unsigned long long* scan_state = cv.take<unsigned long long>(scan_state_words(items));
-  // big-pool counter, slab spill cursor, deferred-item counts and cursors, then the mid masks: zeroed by one memset
-  const size_t state_bytes = 32 + (size_t)h->n_mid_sms * 4;
+  // slab spill cursor, deferred-item counts and cursors, then the mid and big masks: zeroed by one memset
+  const size_t state_bytes = 32 + (size_t)h->n_mid_sms * 4 + (size_t)(big_slots(items) + 31) / 32 * 4;
   unsigned long long* state = reinterpret_cast<unsigned long long*>(cv.take<unsigned char>(state_bytes));
   uint32_t* defer_list = cv.take<uint32_t>(items);
   uint32_t* defer_list2 = cv.take<uint32_t>(items);
@@ -294,7 +299,7 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   cl.slab_base = slab_base;
   cl.desc = desc;
   cl.status = oc->status;
-  cl.big_ctr = reinterpret_cast<uint32_t*>(state);
+  cl.big_mask = reinterpret_cast<uint32_t*>(state + 4) + h->n_mid_sms;
   cl.defer_count = reinterpret_cast<uint32_t*>(state) + 2;
   cl.defer_list[0] = defer_list;
   cl.defer_list[1] = defer_list2;
@@ -337,15 +342,19 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   tl.trip = trip;
   tl.trip_count = trip_count;
   tl.counters = trk_counters;
+  h->last_track_counters = trk_counters;
   uint32_t n_track_launches = 0;
-  if ((err = launch_track(tl, stream, h->side, h->fork_join, h->n_sms, &n_track_launches)) != cudaSuccess) return fail(h, ALLEN_VELO_ERR_CUDA, "track kernel", err);
+  if ((err = launch_track_seed(tl, stream, &n_track_launches)) != cudaSuccess) return fail(h, ALLEN_VELO_ERR_CUDA, "seed kernel", err);
   h->last_launches += n_track_launches;
   mark(3);
+  if ((err = launch_track_follow(tl, stream, h->side, h->fork_join, h->n_sms, &n_track_launches)) != cudaSuccess) return fail(h, ALLEN_VELO_ERR_CUDA, "follow kernel", err);
+  h->last_launches += n_track_launches;
+  mark(4);
 
   if ((err = launch_scan_u64(trk_counts, trk_offsets, n_events, trk_scan_state, stream)) != cudaSuccess)
     return fail(h, ALLEN_VELO_ERR_CUDA, "track scan", err);
   h->last_launches++;
-  mark(4);
+  mark(5);
 
   CompactTracksLaunch ct{};
   ct.n_events = n_events;
@@ -362,7 +371,7 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   ct.out = *ot;
   if ((err = launch_compact_tracks(ct, stream)) != cudaSuccess) return fail(h, ALLEN_VELO_ERR_CUDA, "track compaction", err);
   h->last_launches++;
-  mark(5);
+  mark(6);
   if (h->vertices.vertices) {  // beyond the timed segments of the headline path
     PvLaunch pv{};
     pv.n_events = n_events;
@@ -404,6 +413,12 @@ int allen_velo_kernel_times(allen_velo_t* h, uint32_t call, float* out_ms) {
 }
 
 uint32_t allen_velo_last_launch_count(const allen_velo_t* h) { return h ? h->last_launches : 0; }
+
+int allen_velo_debug_track_counters(allen_velo_t* h, uint32_t* out) {
+  if (!h || !out || !h->last_track_counters) return ALLEN_VELO_ERR_INVALID;
+  const cudaError_t err = cudaMemcpy(out, h->last_track_counters, 16 * sizeof(uint32_t), cudaMemcpyDeviceToHost);
+  return err == cudaSuccess ? ALLEN_VELO_OK : fail(h, ALLEN_VELO_ERR_CUDA, "cudaMemcpy", err);
+}
 
 const char* allen_velo_last_error(const allen_velo_t* h) { return h ? h->last_error.c_str() : "null handle"; }
 

@@ -29,9 +29,10 @@
 // appends the layers that are too large for it to a list, and the next larger one takes that list with resident warps.
 // Beyond 512: MID — every sensor of the layer fits: one pass per sensor group in shared memory, cluster records and
 // sort scratch in a pool slot in global memory; BIG — everything in a (larger) pool slot in global memory.  Same code,
-// same results, decreasing speed; a layer is flagged STAGE_OVERFLOW only if it exceeds 8192 SP words or the BIG pool
-// (counter-allocated) is exhausted.  MID slots belong to resident warps (per-SM bit masks), so they never run out and
-// nobody waits for one.
+// same results, decreasing speed; a layer is flagged STAGE_OVERFLOW only if it
+// holds more than 8192 SP words.  MID slots belong to resident warps (per-SM bit masks), so they never run out and
+// nobody waits for one; BIG slots are taken from a bit mask for the time of one item and given back (a warp that finds
+// none free waits for one), so their number bounds concurrency, not the batch.
 #include "velo_common.cuh"
 
 namespace velo {
@@ -209,13 +210,13 @@ __device__ __forceinline__ bool ccl_pass(const Pass& p, const ClusterStore& cs, 
 #pragma unroll 1
   for (uint32_t i = lane; i < n; i += 32) {
     const uint32_t w = p.sp[i];
+    const uint32_t nA = 2 * i, nB = 2 * i + 1;
+    p.lab[nA] = (uint16_t)nA;  // (dead entries too: the pointer-jumping pass reads every label)
+    p.lab[nB] = (uint16_t)nB;
     if (!w) continue;
     const uint32_t h = w & 0xFFu, R = (w >> 8) & 0x3Fu, C = (w >> 14) & 0x1FFu;
     const uint32_t key = (w >> 8) & 0x3FFFFu;
     const Comps mine = split_rows(h);
-    const uint32_t nA = 2 * i, nB = 2 * i + 1;
-    p.lab[nA] = (uint16_t)nA;
-    p.lab[nB] = (uint16_t)nB;
     auto push = [&](uint32_t u, uint32_t v) {
       const uint32_t idx = atomicAdd(n_edges_ctr, 1u);
       if (idx < p.cap_edges) p.edges[idx] = u | (v << 16);
@@ -266,9 +267,13 @@ __device__ __forceinline__ bool ccl_pass(const Pass& p, const ClusterStore& cs, 
   if (n_edges > p.cap_edges) return false;
 
   // ---- propagate the minimum node id over the edges until nothing changes (exact for any cluster size)
+  //      A label is always the id of a node of the same component and only ever decreases, so the fix point (every edge
+  //      joins equal labels) gives every node the smallest id of its component.  From the third pass on every node also
+  //      takes the label of its label (pointer jumping): a long thin cluster then needs O(log diameter) passes, not one
+  //      pass per hop.
   if (n_edges) {
 #pragma unroll 1
-    for (;;) {
+    for (uint32_t pass = 0;; ++pass) {
       bool changed = false;
 #pragma unroll 1
       for (uint32_t j = lane; j < n_edges; j += 32) {
@@ -280,6 +285,15 @@ __device__ __forceinline__ bool ccl_pass(const Pass& p, const ClusterStore& cs, 
       }
       __syncwarp();
       if (!__any_sync(kFull, changed)) break;
+      if (pass >= 2) {
+#pragma unroll 1
+        for (uint32_t x = lane; x < 2 * n; x += 32) {
+          const uint16_t l = p.lab[x];
+          const uint16_t ll = p.lab[l];
+          if (ll < l) p.lab[x] = ll;
+        }
+        __syncwarp();
+      }
     }
   }
 
@@ -555,7 +569,13 @@ __device__ __forceinline__ void cluster_item(const ClusterLaunch& a, WarpSmem<kC
       finish_layer<kChecksum>(a, cs, ss, item, slab0, n_sp_layer, n_cl);
       return;
     }
-    mode = 2;  // more clusters or edges than the warp's shared memory holds (not seen on physics-like input)
+    // more clusters or edges than the warp's shared memory holds (not seen on physics-like input): the next larger
+    // instance takes the layer; the last one uses a slot of the big pool
+    if (kDefer) {
+      if (lane == 0) a.defer_list[Caps<kCap>::kLevel][atomicAdd(a.defer_count + 2 * Caps<kCap>::kLevel, 1u)] = item;
+      return;
+    }
+    mode = 2;
   }
   uint32_t held = 0xFFFFFFFFu;  // mid slot of this warp (released at the end)
   if (mode == 1) {
@@ -601,13 +621,31 @@ __device__ __forceinline__ void cluster_item(const ClusterLaunch& a, WarpSmem<kC
       if (!ok) mode = 2;
     }
   }
+  uint32_t held_big = 0xFFFFFFFFu;  // big slot of this warp (released at the end)
   if (mode == 2) {
-    uint32_t slot = 0;
-    if (lane == 0) slot = n_sp_layer <= kBigSp ? atomicAdd(a.big_ctr, 1u) : 0xFFFFFFFFu;
+    // a slot of the big pool: bit b of big_mask[w] <-> slot 32 * w + b, taken for the time of this item.  If all are
+    // taken the warp waits: holders never wait for anything, so a slot always comes back.
+    uint32_t slot = 0xFFFFFFFFu;
+    if (lane == 0 && n_sp_layer <= kBigSp) {
+      const uint32_t words = (a.n_big_slots + 31) / 32;
+#pragma unroll 1
+      while (slot == 0xFFFFFFFFu) {
+#pragma unroll 1
+        for (uint32_t w = 0; w < words && slot == 0xFFFFFFFFu; ++w) {
+          const uint32_t valid = (w + 1) * 32 <= a.n_big_slots ? 0xFFFFFFFFu : (1u << (a.n_big_slots & 31u)) - 1u;
+          const uint32_t free_bits = ~*reinterpret_cast<volatile uint32_t*>(a.big_mask + w) & valid;
+          if (!free_bits) continue;
+          const uint32_t b = __ffs(free_bits) - 1;
+          if (!(atomicOr(a.big_mask + w, 1u << b) >> b & 1u)) slot = 32 * w + b;
+        }
+        if (slot == 0xFFFFFFFFu) __nanosleep(500);
+      }
+    }
     slot = __shfl_sync(kFull, slot, 0);
-    if (slot >= a.n_big_slots) {
+    if (slot == 0xFFFFFFFFu) {  // beyond kBigSp super-pixels in one layer
       overflow = true;
     } else {
+      held_big = slot;
       unsigned char* base = a.big_pool + (size_t)slot * BigSlot::kBytes;
       Pass big;
       big.sp = reinterpret_cast<uint32_t*>(base + BigSlot::kSp);
@@ -631,17 +669,29 @@ __device__ __forceinline__ void cluster_item(const ClusterLaunch& a, WarpSmem<kC
   finish_layer_generic<kChecksum>(a, cs, ss, item, slab0, n_sp_layer, n_cl);
   __syncwarp();
   if (held != 0xFFFFFFFFu && lane == 0) atomicAnd(a.mid_mask + (held >> 5), ~(1u << (held & 31u)));
+  if (held_big != 0xFFFFFFFFu && lane == 0) {
+    __threadfence();  // this warp is done with the slot's memory before the next holder starts
+    atomicAnd(a.big_mask + (held_big >> 5), ~(1u << (held_big & 31u)));
+  }
 }
 
 
-// One warp per item of the batch, in grid order.
+// Every warp takes kItemsPerWarp items of the batch, in grid order (more than one item per warp, or resident warps
+// taking items from a counter, was measured: no gain at 10 000 events, a loss at 1 000).
+constexpr uint32_t kItemsPerWarp = 1;
 template <bool kChecksum, uint32_t kCap, bool kDefer>
 __global__ void __launch_bounds__(kWarps * 32) velo_cluster_kernel(const __grid_constant__ ClusterLaunch a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   using WS = WarpSmem<kChecksum, kCap>;
-  const uint32_t item = blockIdx.x * kWarps + (threadIdx.x >> 5);
-  if (item >= a.n_events * a.geo.n_layers) return;
-  cluster_item<kChecksum, kCap, kDefer>(a, reinterpret_cast<WS*>(smem_raw)[threadIdx.x >> 5], item);
+  WS& ws = reinterpret_cast<WS*>(smem_raw)[threadIdx.x >> 5];
+  const uint32_t n = a.n_events * a.geo.n_layers;
+#pragma unroll 1
+  for (uint32_t r = 0; r < kItemsPerWarp; ++r) {
+    const uint32_t item = (blockIdx.x * kItemsPerWarp + r) * kWarps + (threadIdx.x >> 5);
+    if (item >= n) return;
+    cluster_item<kChecksum, kCap, kDefer>(a, ws, item);
+    __syncwarp();
+  }
 }
 
 // Resident warps take the deferred items of list `kFrom` (a few per cent of the layers at most for the last list).
@@ -762,7 +812,7 @@ cudaError_t prepare_cluster_kernels() {
 template <bool kChecksum>
 cudaError_t launch_cluster_chain(const ClusterLaunch& a, uint32_t grid, uint32_t n_sms, uint32_t* n_launches,
                                  cudaStream_t stream) {
-  cudaError_t err = launch_cluster_instance<kChecksum, 128, true>(a, grid, stream);
+  cudaError_t err = launch_cluster_instance<kChecksum, 128, true>(a, (grid + kItemsPerWarp - 1) / kItemsPerWarp, stream);
   if (err != cudaSuccess) return err;
   ++*n_launches;
   if ((err = launch_cluster_list<kChecksum, 256, true, 0>(a, min(grid, 6 * n_sms), stream)) != cudaSuccess) return err;
@@ -792,8 +842,8 @@ cudaError_t launch_cluster(const ClusterLaunch& a, bool big_layers, uint32_t n_s
   ++*n_launches;
   const uint32_t grid = (items + kWarps - 1) / kWarps;
   if (big_layers) {  // 256 -> 512
-    err = a.with_checksum ? launch_cluster_instance<true, 256, true>(a, grid, stream)
-                          : launch_cluster_instance<false, 256, true>(a, grid, stream);
+    err = a.with_checksum ? launch_cluster_instance<true, 256, true>(a, (grid + kItemsPerWarp - 1) / kItemsPerWarp, stream)
+                          : launch_cluster_instance<false, 256, true>(a, (grid + kItemsPerWarp - 1) / kItemsPerWarp, stream);
     if (err != cudaSuccess) return err;
     ++*n_launches;
     const uint32_t lg = min(grid, 3 * n_sms);

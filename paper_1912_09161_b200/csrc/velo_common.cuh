@@ -134,7 +134,7 @@ struct ClusterLaunch {
   uint32_t* status;           // [n_events], zeroed before
   uint32_t* defer_list[2];    // [n_events*n_layers] each: items left to the 256-entry / the 512-entry instance
   uint32_t* defer_count;      // [2][2] list size, cursor; zeroed before
-  uint32_t* big_ctr;          // slots handed out of the big pool, zeroed before
+  uint32_t* big_mask;         // [(n_big_slots + 31) / 32] busy bits of the big slots, zeroed before
   uint32_t* mid_mask;         // [n_mid_sms] busy bits of the mid slots of every SM, zeroed before
   unsigned char* mid_pool;    // [32 * n_mid_sms] slots
   unsigned char* big_pool;    // [n_big_slots] slots
@@ -178,8 +178,9 @@ struct TrackLaunch {
   uint32_t* redo_list[2];          // [n_events] each: events for the CTA-per-event kernel with 512 / 1024 hits per layer
   uint32_t* counters;              // [kCtrCount] list sizes and cursors (velo_track.cuh), zeroed by the launcher
 };
-cudaError_t launch_track(const TrackLaunch& a, cudaStream_t stream, cudaStream_t* side, cudaEvent_t* ev,
-                         uint32_t n_sms, uint32_t* n_launches);
+cudaError_t launch_track_seed(const TrackLaunch& a, cudaStream_t stream, uint32_t* n_launches);
+cudaError_t launch_track_follow(const TrackLaunch& a, cudaStream_t stream, cudaStream_t* side, cudaEvent_t* ev,
+                                uint32_t n_sms, uint32_t* n_launches);
 cudaError_t track_prepare();    // once per process: dynamic shared-memory limits of the track kernels
 cudaError_t cluster_prepare();  // likewise for the cluster kernels
 

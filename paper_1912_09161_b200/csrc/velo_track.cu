@@ -593,12 +593,20 @@ __global__ void __launch_bounds__(128) compact_tracks_kernel(const CompactTracks
   const uint32_t nT = (uint32_t)(o1 >> 32) - T0, nH = (uint32_t)o1 - H0;
   if (threadIdx.x == 0) {
     a.out.event_offsets[e] = T0;
-    if (e + 1 == a.n_events) a.out.event_offsets[e + 1] = T0 + nT;
+    if (e + 1 == a.n_events) {
+      a.out.event_offsets[e + 1] = T0 + nT;
+      // the total number of hits also at a fixed place (the last element), whether or not the tracks fit, so that a host
+      // needs one read for both totals (it equals hit_offsets[n_tracks] when n_tracks == capacity_tracks)
+      a.out.hit_offsets[a.out.capacity_tracks] = H0 + nH;
+    }
   }
   const bool fits = (unsigned long long)T0 + nT <= a.out.capacity_tracks &&
                     (unsigned long long)H0 + nH <= a.out.capacity_hits;
   if (!fits) {
-    if (threadIdx.x == 0 && nT) atomicOr(a.clusters.status + e, ALLEN_VELO_STATUS_TRACK_CAPACITY);
+    if (threadIdx.x == 0 && nT) {
+      atomicOr(a.clusters.status + e, ALLEN_VELO_STATUS_TRACK_CAPACITY);
+      if (T0 < a.out.capacity_tracks) a.out.hit_offsets[T0] = H0;  // closes the hit list of the last track before this event
+    }
     return;
   }
   const uint32_t co = a.clusters.event_offsets[e];
@@ -742,11 +750,7 @@ __global__ void __launch_bounds__(128) compact_tracks_kernel(const CompactTracks
       o[6] = ax; o[7] = bx; o[8] = cx; o[9] = ay; o[10] = by; o[11] = cy;
     }
   }
-  if (threadIdx.x == 0 && e + 1 == a.n_events) {
-    a.out.hit_offsets[T0 + nT] = H0 + nH;
-    // the total number of hits also at a fixed place (the last element), so that a host needs one read for both totals
-    if (T0 + nT < a.out.capacity_tracks) a.out.hit_offsets[a.out.capacity_tracks] = H0 + nH;
-  }
+  if (threadIdx.x == 0 && e + 1 == a.n_events) a.out.hit_offsets[T0 + nT] = H0 + nH;
 }
 
 // One thread per event: class of the event (hits per layer its search needs, or copy only / nothing) and the event lists of
@@ -835,12 +839,11 @@ cudaError_t track_prepare() {
   return err;
 }
 
-// classify -> velo_seed -> velo_follow (three instances beside each other)
-// -> second pass (CTA per event, 512 hits per layer, then 1024) for the events those handed on.  `side`/`ev`: two extra
-// streams and five events owned by the handle; everything is ordered after and before the work on `stream` by events (a
-// fork/join a CUDA graph can capture), nothing synchronises.
-cudaError_t launch_track(const TrackLaunch& a, cudaStream_t stream, cudaStream_t* side, cudaEvent_t* ev, uint32_t n_sms,
-                         uint32_t* n_launches) {
+// classify -> velo_seed.  Then launch_track_follow: velo_follow (three instances beside each other) -> second pass (CTA
+// per event, 512 hits per layer, then 1024) for the events those handed on.  `side`/`ev`: two extra streams and events
+// owned by the handle; everything is ordered after and before the work on `stream` by events (a fork/join a CUDA graph
+// can capture), nothing synchronises.
+cudaError_t launch_track_seed(const TrackLaunch& a, cudaStream_t stream, uint32_t* n_launches) {
   *n_launches = 0;
   if (a.n_events == 0) return cudaSuccess;
   cudaError_t err = cudaMemsetAsync(a.counters, 0, kCtrCount * sizeof(uint32_t), stream);
@@ -850,19 +853,27 @@ cudaError_t launch_track(const TrackLaunch& a, cudaStream_t stream, cudaStream_t
   ++*n_launches;
   if ((err = launch_seed(a, stream)) != cudaSuccess) return err;
   ++*n_launches;
-  if ((err = cudaEventRecord(ev[2], stream)) != cudaSuccess) return err;
-  if ((err = cudaStreamWaitEvent(side[0], ev[2], 0)) != cudaSuccess) return err;
-  if ((err = cudaStreamWaitEvent(side[1], ev[2], 0)) != cudaSuccess) return err;
+  return cudaSuccess;
+}
+
+cudaError_t launch_track_follow(const TrackLaunch& a, cudaStream_t stream, cudaStream_t* side, cudaEvent_t* ev,
+                                uint32_t n_sms, uint32_t* n_launches) {
+  *n_launches = 0;
+  if (a.n_events == 0) return cudaSuccess;
+  cudaError_t err;
+  if ((err = cudaEventRecord(ev[0], stream)) != cudaSuccess) return err;
+  if ((err = cudaStreamWaitEvent(side[0], ev[0], 0)) != cudaSuccess) return err;
+  if ((err = cudaStreamWaitEvent(side[1], ev[0], 0)) != cudaSuccess) return err;
   if ((err = launch_follow(a, 1, n_sms, side[0])) != cudaSuccess) return err;
   ++*n_launches;
   if ((err = launch_follow(a, 2, n_sms, side[1])) != cudaSuccess) return err;
   ++*n_launches;
   if ((err = launch_follow(a, 0, n_sms, stream)) != cudaSuccess) return err;
   ++*n_launches;
-  if ((err = cudaEventRecord(ev[3], side[0])) != cudaSuccess) return err;
-  if ((err = cudaEventRecord(ev[4], side[1])) != cudaSuccess) return err;
-  if ((err = cudaStreamWaitEvent(stream, ev[3], 0)) != cudaSuccess) return err;
-  if ((err = cudaStreamWaitEvent(stream, ev[4], 0)) != cudaSuccess) return err;
+  if ((err = cudaEventRecord(ev[1], side[0])) != cudaSuccess) return err;
+  if ((err = cudaEventRecord(ev[2], side[1])) != cudaSuccess) return err;
+  if ((err = cudaStreamWaitEvent(stream, ev[1], 0)) != cudaSuccess) return err;
+  if ((err = cudaStreamWaitEvent(stream, ev[2], 0)) != cudaSuccess) return err;
   if ((err = launch_list<CfgMr>(a, 0, min(a.n_events, 2 * n_sms), stream)) != cudaSuccess) return err;
   ++*n_launches;
   if ((err = launch_list<CfgLr>(a, 1, min(a.n_events, n_sms), stream)) != cudaSuccess) return err;

@@ -300,3 +300,34 @@ def brute_force_tracking(x, y, z, phi, layer_offsets, P, scatter):
         if len(t["hits"]) >= 4 or t["s_seed"] <= P["s_weak"]:
             out.append(tuple(sorted(t["hits"])))
     return sorted(out)
+
+
+# ------------------------------------------------------------------------------------------------
+# Raw format v1 assembled from explicit SP words (R1): for inputs that pack_events cannot make (a repeated
+# SP address inside a bank, a zero hit map).  Format assembly only; no arithmetic of the method.
+# ------------------------------------------------------------------------------------------------
+def sp_word(sp_col: int, sp_row: int, hitmap: int) -> int:
+    return (sp_col << 14) | (sp_row << 8) | (hitmap & 0xFF)
+
+
+def raw_from_sp_words(n_sensors: int, events: list[dict[int, list[int]]]):
+    """events: per event {sensor: [sp words in bank order]}.  Returns (raw u8 array, event_offsets u32 array)."""
+    chunks, offsets = [], [0]
+    for banks in events:
+        words = [0x56454C4F, n_sensors, sum(len(v) for v in banks.values()), 0]
+        off = 0
+        for s in range(n_sensors):
+            words.append(off)
+            off += len(banks.get(s, ()))
+        words.append(off)
+        while len(words) % 4:
+            words.append(0)
+        for s in range(n_sensors):
+            words.extend(int(w) for w in banks.get(s, ()))
+        while len(words) % 4:
+            words.append(0)
+        a = np.array(words, dtype=np.uint32)
+        chunks.append(a.view(np.uint8))
+        offsets.append(offsets[-1] + a.nbytes)
+    raw = np.concatenate(chunks) if chunks else np.zeros(0, np.uint8)
+    return raw, np.array(offsets, dtype=np.uint32)

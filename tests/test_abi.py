@@ -1,4 +1,4 @@
-"""The C-ABI library loads without a GPU and exports every function include/allen_velo.h declares (no compute calls)."""
+"""The C-ABI library loads without a GPU and exports every function include/*.h declares (no compute calls)."""
 import ctypes
 import os
 import re
@@ -6,17 +6,22 @@ import re
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def declared_functions():
-    text = open(os.path.join(ROOT, "include", "allen_velo.h")).read()
-    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    names = re.findall(r"\b(allen_velo_[a-z_]+)\s*\(", text)
+def declared_functions(headers=("allen_velo.h", "allen_velo_debug.h")):
+    names = []
+    for h in headers:
+        text = open(os.path.join(ROOT, "include", h)).read()
+        text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+        names += re.findall(r"\b(allen_velo_[a-z_]+)\s*\(", text)
     return sorted(set(names))
 
 
 def test_header_declares_the_three_calls_of_the_north_star():
-    names = declared_functions()
+    names = declared_functions(("allen_velo.h",))
     for n in ("allen_velo_create", "allen_velo_reconstruct", "allen_velo_destroy"):
         assert n in names
+    # measurement hooks live in their own header, not in the product ABI
+    assert not [n for n in names if "timing" in n or "kernel_" in n or "launch_count" in n]
+    assert "allen_velo_enable_timing" in declared_functions(("allen_velo_debug.h",))
 
 
 def test_library_exports_every_declared_symbol():
@@ -35,7 +40,7 @@ def test_calls_that_need_no_device():
     assert (p.w_seed_phi16, p.w_fwd_phi16, p.max_skipped) == (512, 512, 1)
     assert (p.max_slope, p.s_seed, p.s_fwd, p.s_weak) == (ctypes.c_float(0.4).value, 2.0 ** -6, 2.0 ** -4, 2.0 ** -7)
     names = [lib.allen_velo_kernel_name(i).decode() for i in range(lib.allen_velo_kernel_count())]
-    assert "velo_cluster" in names and "velo_track" in names
+    assert "velo_cluster" in names and "velo_seed" in names and "velo_follow" in names
     # null handle / null arguments are rejected, not dereferenced
     assert lib.allen_velo_create(None, None) == binding.ERR_INVALID
     assert lib.allen_velo_workspace_bytes(None, 10, 1000) == 0
@@ -52,6 +57,10 @@ def test_binding_structs_match_the_header_layout():
     assert ctypes.sizeof(binding.allen_velo_geometry_t) == 24 + 3 * 8 + 28 + 4  # padded to 8
     assert ctypes.sizeof(binding.allen_velo_clusters_t) == 8 + 12 * 8
     assert ctypes.sizeof(binding.allen_velo_tracks_t) == 8 + 8 * 8
+    assert ctypes.sizeof(binding.allen_velo_vertices_t) == 8 + 2 * 8  # u32 padded to 8, two pointers
+    for struct, fields in ((binding.allen_velo_clusters_t, 13), (binding.allen_velo_tracks_t, 10),
+                           (binding.allen_velo_vertices_t, 3), (binding.allen_velo_params_t, 7)):
+        assert len(struct._fields_) == fields
 
 
 def test_product_path_refuses_to_run_without_cuda(geometry):
