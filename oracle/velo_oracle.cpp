@@ -57,6 +57,9 @@ enum : uint32_t {
 };
 
 // ------------------------------------------------------------------------------------------------
+// O2-local (D:R11): region size in super-pixels, 0 = off.  Set by oracle_set_cluster_regions before a run.
+static uint32_t region_sp_cols = 0, region_sp_rows = 0;
+
 // O2 helper: membership checksum (D:R2) — sum over the cluster's pixels of mix32(row*n_cols+col), mod 2^32.
 // ------------------------------------------------------------------------------------------------
 uint32_t mix32(uint32_t v) {
@@ -227,6 +230,12 @@ void cluster_event(const Geometry& g, const uint8_t* raw, size_t bytes, EventRes
             int r2 = (int)row + dr, c2 = (int)col + dc;
             if (r2 < 0 || c2 < 0 || r2 >= (int)g.n_rows || c2 >= (int)g.n_cols) continue;
             uint32_t j = (uint32_t)r2 * g.n_cols + (uint32_t)c2;
+            // O2-local ("searches for clusters locally in small regions. Every region can be treated
+            // independently"; D:R11): with regions switched on, a cluster never leaves its region of
+            // region_sp_cols x region_sp_rows super-pixels.  Off (0, 0) = the exact definition above.
+            if (region_sp_cols && ((uint32_t)c2 / 2 / region_sp_cols != col / 2 / region_sp_cols ||
+                                   (uint32_t)r2 / 4 / region_sp_rows != row / 4 / region_sp_rows))
+              continue;
             if (sc.grid[j] == -2) { sc.grid[j] = id; stack.push_back(j); }
           }
       }
@@ -676,6 +685,12 @@ uint32_t oracle_pv_candidates(uint32_t n, const float* x0, const float* y0, cons
                               const double* kal, double* out /* [32][8] */, uint32_t* n_candidates, double* cand,
                               uint32_t cand_cap) {
   return find_pvs(n, x0, y0, tx, ty, kal, out, n_candidates, 8, cand, cand_cap);
+}
+
+// O2-local: region size in super-pixels for the runs that follow (0, 0 = exact connected components).
+void oracle_set_cluster_regions(uint32_t sp_cols, uint32_t sp_rows) {
+  region_sp_cols = sp_cols && sp_rows ? sp_cols : 0;
+  region_sp_rows = sp_cols && sp_rows ? sp_rows : 0;
 }
 
 void* oracle_run(const Geometry* g, const uint8_t* raw, const uint32_t* event_offsets, uint32_t n_events,

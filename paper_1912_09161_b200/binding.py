@@ -84,6 +84,8 @@ def load_library():
         L.allen_velo_kernel_times.restype = ctypes.c_int
         L.allen_velo_last_launch_count.argtypes = [ctypes.c_void_p]
         L.allen_velo_last_launch_count.restype = ctypes.c_uint32
+        L.allen_velo_set_cluster_regions.argtypes = [ctypes.c_void_p, ctypes.c_uint32, ctypes.c_uint32]
+        L.allen_velo_set_cluster_regions.restype = ctypes.c_int
         L.allen_velo_debug_track_counters.argtypes = [ctypes.c_void_p, ctypes.c_void_p]
         L.allen_velo_debug_track_counters.restype = ctypes.c_int
         L.allen_velo_last_error.argtypes = [ctypes.c_void_p]
@@ -249,6 +251,12 @@ class AllenVelo:
 
     def last_launch_count(self) -> int:
         return int(self._lib.allen_velo_last_launch_count(self._h))
+
+    def set_cluster_regions(self, sp_cols: int, sp_rows: int) -> None:
+        """Local clustering variant (R11); (0, 0) = exact connected components."""
+        rc = self._lib.allen_velo_set_cluster_regions(self._h, sp_cols, sp_rows)
+        if rc != OK:
+            raise RuntimeError(f"allen_velo_set_cluster_regions -> {rc}: {self.last_error()}")
 
     def track_counters(self) -> dict:
         """List sizes of the track search of the last call (include/allen_velo_debug.h; synchronises the device)."""

@@ -167,6 +167,7 @@ int allen_velo_create(const allen_velo_geometry_t* geo, allen_velo_t** out) {
   g.n_sensors = S; g.n_layers = L; g.n_cols = geo->n_cols; g.n_rows = geo->n_rows;
   g.sp_cols = geo->n_cols / 2; g.sp_rows = geo->n_rows / 4;
   g.table_words = (S + 1 + 3) / 4 * 4;
+  g.region_shift_c = g.region_shift_r = 31;
   g.pitch = geo->pitch_mm;
   g.ltg = reinterpret_cast<const float*>(d);
   g.sensor_layer = reinterpret_cast<const uint16_t*>(d + b_ltg);
@@ -189,6 +190,18 @@ size_t allen_velo_workspace_bytes(const allen_velo_t* h, uint32_t n_events, size
 int allen_velo_set_occupancy_hint(allen_velo_t* h, uint32_t sp_words_per_layer) {
   if (!h) return ALLEN_VELO_ERR_INVALID;
   h->sp_words_per_layer = sp_words_per_layer;
+  return ALLEN_VELO_OK;
+}
+
+int allen_velo_set_cluster_regions(allen_velo_t* h, uint32_t sp_cols, uint32_t sp_rows) {
+  if (!h) return ALLEN_VELO_ERR_INVALID;
+  if (sp_cols == 0 || sp_rows == 0) { h->dev.region_shift_c = h->dev.region_shift_r = 31; return ALLEN_VELO_OK; }
+  if ((sp_cols & (sp_cols - 1)) || (sp_rows & (sp_rows - 1))) return fail(h, ALLEN_VELO_ERR_INVALID, "region size not a power of two");
+  uint32_t sc = 0, sr = 0;
+  while ((1u << sc) < sp_cols) ++sc;
+  while ((1u << sr) < sp_rows) ++sr;
+  h->dev.region_shift_c = sc;
+  h->dev.region_shift_r = sr;
   return ALLEN_VELO_OK;
 }
 

@@ -223,15 +223,20 @@ __device__ __forceinline__ bool ccl_pass(const Pass& p, const ClusterStore& cs, 
     };
     const uint32_t r4 = mine.rA | mine.rB;
     const uint32_t n_row3 = (mine.rA & 8u) ? nA : nB;  // our component holding row 3
+    // local clustering variant (R11; "locally in small regions"): edges stay inside a region of
+    // 2^shift super-pixels; shift 31 (the default) puts the whole sensor in one region = exact components
+    const bool same_c = ((C + 1) >> g.region_shift_c) == (C >> g.region_shift_c);
+    const bool same_up = ((R + 1) >> g.region_shift_r) == (R >> g.region_shift_r);
+    const bool same_dn = R >= 1 && ((R - 1) >> g.region_shift_r) == (R >> g.region_shift_r);
     // (C, R+1): our row 3 touches their row 0 whatever the columns
-    if ((r4 & 8u) && R + 1 < g.sp_rows) {
+    if ((r4 & 8u) && R + 1 < g.sp_rows && same_up) {
       const int t = lookup(p.tab, bits, key + 1);
       if (t >= 0) {
         const uint32_t q = p.sp[t] & 0xFFu;
         if ((q | (q >> 4)) & 1u) push(n_row3, 2 * t);
       }
     }
-    if (C + 1 < g.sp_cols) {
+    if (C + 1 < g.sp_cols && same_c) {
       // (C+1, R): our column-1 pixels touch their column-0 pixels within one row
       if (h & 0xF0u) {
         const int t = lookup(p.tab, bits, key + 64);
@@ -248,12 +253,12 @@ __device__ __forceinline__ bool ccl_pass(const Pass& p, const ClusterStore& cs, 
         }
       }
       // (C+1, R+1): our pixel (dc=1, dr=3) touches their pixel (dc=0, dr=0)
-      if ((h & 0x80u) && R + 1 < g.sp_rows) {
+      if ((h & 0x80u) && R + 1 < g.sp_rows && same_up) {
         const int t = lookup(p.tab, bits, key + 65);
         if (t >= 0 && (p.sp[t] & 1u)) push(n_row3, 2 * t);
       }
       // (C+1, R-1): our pixel (dc=1, dr=0) touches their pixel (dc=0, dr=3)
-      if ((h & 0x10u) && R >= 1) {
+      if ((h & 0x10u) && same_dn) {
         const int t = lookup(p.tab, bits, key + 63);
         if (t >= 0 && (p.sp[t] & 8u)) {
           const Comps theirs = split_rows(p.sp[t] & 0xFFu);

@@ -16,6 +16,7 @@ constexpr uint32_t kFull = 0xFFFFFFFFu;
 struct DeviceGeometry {
   uint32_t n_sensors, n_layers, n_cols, n_rows, sp_cols, sp_rows;
   uint32_t table_words;  // bank table incl. padding, in u32 words
+  uint32_t region_shift_c, region_shift_r;  // local clustering variant (R11): log2 of the region size in SPs; 31 = exact CCL
   float pitch;
   const uint16_t* sensor_layer;     // [n_sensors]
   const uint16_t* layer_sensors;    // [n_layers][kMaxSensorsPerLayer]

@@ -171,3 +171,33 @@ def test_loose_cuts_overflow_the_candidate_lists_and_track_slots(geometry, batch
     assert rep["n_got"] == rep["n_ref"] and rep["mismatched_tracks"] == 0 and rep["bad_fits"] == 0, rep
     assert np.array_equal(t.hits, ref.tracks.hits)
     assert not clusters["status"].any()
+
+
+@pytest.mark.parametrize("regions", [(1, 1), (2, 2), (8, 8), (4, 1)])
+def test_local_clustering_variant_against_the_oracle(geometry, batch_of, regions):
+    """SURVEY 8(f4) / DESIGN.md R11 ("searches for clusters locally in small regions"): clusters confined to regions
+    of sp_cols x sp_rows super-pixels.  Everything (clusters bit for bit, tracks, fit) equals the oracle run with the same
+    regions; the deviation from the exact components is what the oracle counts (tests/test_oracle_local_clusters.py)."""
+    import oracle
+    from paper_1912_09161_b200 import binding
+    from tests.helpers import compare_clusters, compare_tracks
+
+    batch = batch_of(2, 64)
+    ref = oracle.reconstruct(geometry, batch.raw, batch.event_offsets, cluster_regions=regions, n_threads=8)
+    exact = oracle.reconstruct(geometry, batch.raw, batch.event_offsets, n_threads=8)
+    assert len(ref.clusters.key) > len(exact.clusters.key)  # the variant does split clusters on this batch
+    v = binding.AllenVelo(geometry)
+    try:
+        v.set_cluster_regions(*regions)
+        clusters, tracks = binding.reconstruct_batch(v, batch.raw, batch.event_offsets)
+        v.set_cluster_regions(0, 0)
+        back = binding.reconstruct_batch(v, batch.raw, batch.event_offsets)
+    finally:
+        v.destroy()
+    c, t = as_oracle_types(clusters, tracks)
+    assert not compare_clusters(c, ref.clusters)
+    rep = compare_tracks(t, ref.tracks, ref)
+    assert rep["n_got"] == rep["n_ref"] and rep["mismatched_tracks"] == 0 and rep["bad_fits"] == 0, rep
+    assert np.array_equal(t.hits, ref.tracks.hits)
+    c0, _ = as_oracle_types(*back)
+    assert not compare_clusters(c0, exact.clusters)  # switched off again: exact components
