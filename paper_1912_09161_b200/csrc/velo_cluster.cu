@@ -151,28 +151,58 @@ __device__ __forceinline__ bool ccl_pass(const Pass& p, const ClusterStore& cs, 
     const uint32_t st = __shfl_sync(kFull, my_start, kk);
     start_of[kk] = ((uint32_t)kk > k0 && (uint32_t)kk < k1) ? st : 0xFFFFFFFFu;
   }
+  auto stage_word = [&](uint32_t i, uint32_t w) {  // staged index i (< n), raw word w
+    uint32_t k = k0;
+#pragma unroll
+    for (int kk = 1; kk < kMaxSensorsPerLayer; ++kk) k += i >= start_of[kk];
+    const uint32_t R = (w >> 8) & 0x3Fu, C = (w >> 14) & 0x1FFu;
+    uint32_t staged = (w & 0x7FFFFFu) | (k << 23);
+    if ((w & 0xFFu) == 0) staged = 0;
+    if (C >= g.sp_cols || R >= g.sp_rows) { bad_sp = true; staged = 0; }
+    p.sp[i] = staged;
+  };
+  // The banks of a layer's sensors usually follow one another in the raw event (G0: sensors 4k .. 4k+3): the group is
+  // then ONE range of SP words, read with 128-bit loads (ld.global.nc.v4: the SP area of an event starts on a 16-byte
+  // boundary and is padded to one, R1), two loads per lane in flight.  Otherwise word by word.
+  const uint32_t has = __ballot_sync(kFull, in_group != 0);
+  const uint32_t rel = my_off - my_start;  // raw position of staged index 0, if the group is one range
+  const uint32_t g0 = __shfl_sync(kFull, rel, has ? __ffs(has) - 1 : 0);
+  if (__all_sync(kFull, in_group == 0 || rel == g0)) {
+    const uint32_t a0 = g0 & ~3u;
+    const uint4* __restrict__ v4 = reinterpret_cast<const uint4*>(spw + a0);
+    const uint32_t nv = n ? ((g0 + n + 3u) >> 2) - (a0 >> 2) : 0u;
+    const int skew = (int)(a0 - g0);  // staged index of the first word of vector 0 (<= 0)
 #pragma unroll 1
-  for (uint32_t i0 = 0; i0 < n; i0 += 128) {
-    uint32_t w[4], ks[4];
+    for (uint32_t v0 = 0; v0 < nv; v0 += 64) {
+      const uint32_t va = v0 + lane, vb = v0 + 32 + lane;
+      uint4 wa = make_uint4(0, 0, 0, 0), wb = wa;
+      if (va < nv) wa = __ldg(v4 + va);
+      if (vb < nv) wb = __ldg(v4 + vb);
+      const uint32_t ua[4] = {wa.x, wa.y, wa.z, wa.w}, ub[4] = {wb.x, wb.y, wb.z, wb.w};
 #pragma unroll
-    for (int u = 0; u < 4; ++u) {
-      const uint32_t i = i0 + 32 * u + lane;
-      uint32_t k = k0;
-#pragma unroll
-      for (int kk = 1; kk < kMaxSensorsPerLayer; ++kk) k += i >= start_of[kk];
-      const uint32_t src = __shfl_sync(kFull, my_off, k) + (i - __shfl_sync(kFull, my_start, k));
-      ks[u] = k;
-      w[u] = i < n ? __ldg(spw + src) : 0u;
+      for (int u = 0; u < 4; ++u) {
+        const int ia = skew + (int)(4 * va) + u, ib = skew + (int)(4 * vb) + u;
+        if (va < nv && ia >= 0 && ia < (int)n) stage_word((uint32_t)ia, ua[u]);
+        if (vb < nv && ib >= 0 && ib < (int)n) stage_word((uint32_t)ib, ub[u]);
+      }
     }
+  } else {
+#pragma unroll 1
+    for (uint32_t i0 = 0; i0 < n; i0 += 128) {
+      uint32_t w[4];
 #pragma unroll
-    for (int u = 0; u < 4; ++u) {
-      const uint32_t i = i0 + 32 * u + lane;
-      const uint32_t R = (w[u] >> 8) & 0x3Fu, C = (w[u] >> 14) & 0x1FFu;
-      uint32_t staged = (w[u] & 0x7FFFFFu) | (ks[u] << 23);
-      if ((w[u] & 0xFFu) == 0) staged = 0;
-      if (i < n) {
-        if (C >= g.sp_cols || R >= g.sp_rows) { bad_sp = true; staged = 0; }
-        p.sp[i] = staged;
+      for (int u = 0; u < 4; ++u) {
+        const uint32_t i = i0 + 32 * u + lane;
+        uint32_t k = k0;
+#pragma unroll
+        for (int kk = 1; kk < kMaxSensorsPerLayer; ++kk) k += i >= start_of[kk];
+        const uint32_t src = __shfl_sync(kFull, my_off, k) + (i - __shfl_sync(kFull, my_start, k));
+        w[u] = i < n ? __ldg(spw + src) : 0u;
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const uint32_t i = i0 + 32 * u + lane;
+        if (i < n) stage_word(i, w[u]);
       }
     }
   }
