@@ -28,6 +28,12 @@ int allen_velo_kernel_times(allen_velo_t* handle, uint32_t call, float* out_ms /
 /* Number of kernels the last reconstruct() call launched (bench.py's gpu_launches). */
 uint32_t allen_velo_last_launch_count(const allen_velo_t* handle);
 
+/* Bounds checks (the library built with -DVELO_DEBUG: paper_1912_09161_b200/build.py --debug).  1 if this library was
+ * built with them.  allen_velo_debug_fault: the highest code of a check that failed since the last call of this function
+ * (0 = none; codes in csrc/velo_common.cuh), read from the device (SYNCHRONISES) and cleared. */
+int allen_velo_debug_checks_compiled(void);
+int allen_velo_debug_fault(allen_velo_t* handle, uint32_t* out /* HOST out */);
+
 /* List sizes of the track search of the last reconstruct() call, copied from the workspace (SYNCHRONISES the device):
  * out[0..2] events searched by the three instances of velo_follow_kernel (at most 256 / 512 / 1024 hits per layer),
  * out[12], out[13] events handed on to the CTA-per-event kernel with 512 / 1024 hits per layer (candidate list or

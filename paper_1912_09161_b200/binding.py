@@ -50,14 +50,19 @@ class allen_velo_vertices_t(ctypes.Structure):
 _lib = None
 
 
-def load_library():
-    """dlopen the in-tree extension.  Raises if it has not been built (no fallback)."""
-    global _lib
-    if _lib is None:
-        if not os.path.exists(LIB_PATH):
-            raise RuntimeError(f"CUDA extension {LIB_PATH} is missing: run `python -m paper_1912_09161_b200.build` "
+_debug_lib = None
+
+
+def load_library(debug: bool = False):
+    """dlopen the in-tree extension (debug=True: the build with bounds checks, _allen_velo_debug.so).  Raises if it has
+    not been built (no fallback)."""
+    global _lib, _debug_lib
+    if (_debug_lib if debug else _lib) is None:
+        path = os.path.join(_HERE, "_allen_velo_debug.so") if debug else LIB_PATH
+        if not os.path.exists(path):
+            raise RuntimeError(f"CUDA extension {path} is missing: run `python -m paper_1912_09161_b200.build` "
                                "(or __graft_entry__.build()); there is no CPU fallback")
-        L = ctypes.CDLL(LIB_PATH)
+        L = ctypes.CDLL(path)
         L.allen_velo_default_params.argtypes = [ctypes.POINTER(allen_velo_params_t)]
         L.allen_velo_default_params.restype = None
         L.allen_velo_create.argtypes = [ctypes.POINTER(allen_velo_geometry_t), ctypes.POINTER(ctypes.c_void_p)]
@@ -92,8 +97,15 @@ def load_library():
         L.allen_velo_last_error.restype = ctypes.c_char_p
         L.allen_velo_destroy.argtypes = [ctypes.c_void_p]
         L.allen_velo_destroy.restype = None
-        _lib = L
-    return _lib
+        L.allen_velo_debug_fault.argtypes = [ctypes.c_void_p, ctypes.c_void_p]
+        L.allen_velo_debug_fault.restype = ctypes.c_int
+        L.allen_velo_debug_checks_compiled.argtypes = []
+        L.allen_velo_debug_checks_compiled.restype = ctypes.c_int
+        if debug:
+            _debug_lib = L
+        else:
+            _lib = L
+    return _debug_lib if debug else _lib
 
 
 def allen_velo_default_params() -> allen_velo_params_t:
@@ -172,12 +184,12 @@ def alloc_outputs(n_events: int, n_layers: int, cluster_capacity: int, track_cap
 class AllenVelo:
     """RAII wrapper of the handle: allen_velo_create / set_workspace / reconstruct / destroy."""
 
-    def __init__(self, geometry, params: dict | None = None):
+    def __init__(self, geometry, params: dict | None = None, debug: bool = False):
         import torch
 
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1912_09161_b200 needs a CUDA device (sm_100a); there is no CPU fallback")
-        self._lib = load_library()
+        self._lib = load_library(debug)
         p = allen_velo_default_params()
         for k, v in (params or {}).items():
             setattr(p, k, v)
@@ -257,6 +269,17 @@ class AllenVelo:
         rc = self._lib.allen_velo_set_cluster_regions(self._h, sp_cols, sp_rows)
         if rc != OK:
             raise RuntimeError(f"allen_velo_set_cluster_regions -> {rc}: {self.last_error()}")
+
+    def debug_fault(self) -> int:
+        """Highest code of a failed bounds check since the last call (debug build; 0 = none).  Synchronises."""
+        out = ctypes.c_uint32(0)
+        rc = self._lib.allen_velo_debug_fault(self._h, ctypes.byref(out))
+        if rc != OK:
+            raise RuntimeError(f"allen_velo_debug_fault -> {rc}")
+        return int(out.value)
+
+    def checks_compiled(self) -> bool:
+        return bool(self._lib.allen_velo_debug_checks_compiled())
 
     def track_counters(self) -> dict:
         """List sizes of the track search of the last call (include/allen_velo_debug.h; synchronises the device)."""

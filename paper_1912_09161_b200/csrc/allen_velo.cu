@@ -142,7 +142,8 @@ int allen_velo_create(const allen_velo_geometry_t* geo, allen_velo_t** out) {
   // one device block: ltg | sensor_layer | layer_sensors | layer_n_sensors
   const size_t b_ltg = align_up((size_t)S * 9 * 4), b_sl = align_up((size_t)S * 2),
                b_ls = align_up(layer_sensors.size() * 2), b_ln = align_up(L);
-  cudaError_t err = cudaMalloc(&h->dev_block, b_ltg + b_sl + b_ls + b_ln);
+  cudaError_t err = cudaMalloc(&h->dev_block, b_ltg + b_sl + b_ls + b_ln + kAlign);
+  if (err == cudaSuccess) err = cudaMemset(static_cast<unsigned char*>(h->dev_block) + b_ltg + b_sl + b_ls + b_ln, 0, kAlign);
   if (err != cudaSuccess) { delete h; return ALLEN_VELO_ERR_CUDA; }
   unsigned char* d = static_cast<unsigned char*>(h->dev_block);
   err = cudaMemcpy(d, geo->sensor_ltg, (size_t)S * 9 * 4, cudaMemcpyHostToDevice);
@@ -174,6 +175,7 @@ int allen_velo_create(const allen_velo_geometry_t* geo, allen_velo_t** out) {
   g.layer_sensors = reinterpret_cast<const uint16_t*>(d + b_ltg + b_sl);
   g.layer_n_sensors = reinterpret_cast<const uint8_t*>(d + b_ltg + b_sl + b_ls);
   g.params = geo->params;
+  g.debug_fault = reinterpret_cast<uint32_t*>(d + b_ltg + b_sl + b_ls + b_ln);
   *out = h;
   return ALLEN_VELO_OK;
 }
@@ -426,6 +428,21 @@ int allen_velo_kernel_times(allen_velo_t* h, uint32_t call, float* out_ms) {
 }
 
 uint32_t allen_velo_last_launch_count(const allen_velo_t* h) { return h ? h->last_launches : 0; }
+
+int allen_velo_debug_fault(allen_velo_t* h, uint32_t* out) {
+  if (!h || !out) return ALLEN_VELO_ERR_INVALID;
+  cudaError_t err = cudaMemcpy(out, h->dev.debug_fault, sizeof(uint32_t), cudaMemcpyDeviceToHost);
+  if (err == cudaSuccess) err = cudaMemset(h->dev.debug_fault, 0, sizeof(uint32_t));
+  return err == cudaSuccess ? ALLEN_VELO_OK : fail(h, ALLEN_VELO_ERR_CUDA, "cudaMemcpy", err);
+}
+
+int allen_velo_debug_checks_compiled(void) {
+#ifdef VELO_DEBUG
+  return 1;
+#else
+  return 0;
+#endif
+}
 
 int allen_velo_debug_track_counters(allen_velo_t* h, uint32_t* out) {
   if (!h || !out || !h->last_track_counters) return ALLEN_VELO_ERR_INVALID;

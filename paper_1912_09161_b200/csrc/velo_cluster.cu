@@ -222,8 +222,10 @@ __device__ __forceinline__ bool ccl_pass(const Pass& p, const ClusterStore& cs, 
     if (!w) continue;
     const uint32_t key = (w >> 8) & 0x3FFFFu;
     uint32_t s = hash_slot(key, bits);
+    uint32_t probes = 0;
 #pragma unroll 1
     for (;;) {
+      VELO_CHECK(g, ++probes <= (1u << bits), 101);  // the table has twice as many slots as entries: a free one exists
       const uint32_t old = atomicCAS(p.tab + s, 0u, (key << 14) | (i + 1));
       if (old == 0) break;
       if ((old >> 14) == key) {
@@ -300,6 +302,7 @@ __device__ __forceinline__ bool ccl_pass(const Pass& p, const ClusterStore& cs, 
   __syncwarp();
   const uint32_t n_edges = *n_edges_ctr;
   if (n_edges > p.cap_edges) return false;
+  VELO_CHECK(g, n <= p.cap_sp && 2 * n <= 0x10000u, 102);  // staged words fit the pass, node ids fit 16 bits
 
   // ---- propagate the minimum node id over the edges until nothing changes (exact for any cluster size)
   //      A label is always the id of a node of the same component and only ever decreases, so the fix point (every edge
@@ -379,6 +382,7 @@ __device__ __forceinline__ bool ccl_pass(const Pass& p, const ClusterStore& cs, 
         const uint32_t node = 2 * i + comp;
         if (!rows || p.lab[node] == node) continue;
         const uint32_t cid = cidmap[p.lab[node]];
+        VELO_CHECK(g, p.lab[node] < 2 * n && cid < n_cl, 103);
         const Stats s = comp_stats<kChecksum>(h & (rows | (rows << 4)), C, R, g.n_cols);
         atomicMin(&cs.key[cid], (cs.key[cid] & ~0x3FFFFu) | s.minpix);
         atomicAdd(&cs.n[cid], s.n);
@@ -467,6 +471,7 @@ __device__ __forceinline__ void finish_layer(const ClusterLaunch& a, const Clust
       const uint32_t o = ss.tmp[q];
       rank += (((unsigned long long)ss.phis[o] << 32) | cs.key[o]) < mine;
     }
+    VELO_CHECK(g, start + rank < n_cl && c < n_cl && end <= n_cl, 104);
     ss.order[start + rank] = (uint16_t)c;
   }
   __syncwarp();
@@ -479,6 +484,7 @@ __device__ __forceinline__ void finish_layer(const ClusterLaunch& a, const Clust
     else cluster_local(n, sc, sr, g.pitch, u, v);
     local_to_global(u, v, g.ltg + 9 * (key >> 18), x, y, z);
     const uint32_t o = slab0 + j;
+    VELO_CHECK(g, o < a.slab.capacity && c < n_cl, 105);
     a.slab.rec[o] = make_uint4(__float_as_uint(x), __float_as_uint(y), __float_as_uint(z), (uint32_t)(ss.phis[c] ^ 0x8000u));
     a.slab.info[o] = make_uint4(key, n, sc, sr);
     if (kChecksum) a.slab.checksum[o] = cs.cks[c];

@@ -17,6 +17,7 @@ struct DeviceGeometry {
   uint32_t n_sensors, n_layers, n_cols, n_rows, sp_cols, sp_rows;
   uint32_t table_words;  // bank table incl. padding, in u32 words
   uint32_t region_shift_c, region_shift_r;  // local clustering variant (R11): log2 of the region size in SPs; 31 = exact CCL
+  uint32_t* debug_fault;  // one word in the handle's device block: highest VELO_CHECK code that failed (VELO_DEBUG builds)
   float pitch;
   const uint16_t* sensor_layer;     // [n_sensors]
   const uint16_t* layer_sensors;    // [n_layers][kMaxSensorsPerLayer]
@@ -42,6 +43,17 @@ struct ClusterSlab {
 };
 constexpr uint32_t kPhiSlices = 256;      // the buckets of the cluster kernel's counting sort on the top byte of phi16
 constexpr uint32_t kPhiTabStride = 264;   // u16 per (event, layer): kPhiSlices + 1 entries, padded to 16 bytes
+
+// ---- bounds checks of the debug build (compute-sanitizer is closed on this pool) ---------------------------------------
+// Built with -DVELO_DEBUG (paper_1912_09161_b200/build.py --debug -> _allen_velo_debug.so) every index into a shared-memory
+// or workspace capacity is tested where it is formed; a failing test records its code in DeviceGeometry::debug_fault
+// (read and cleared with allen_velo_debug_fault) and the access is still made, so that results show the damage too.
+// Codes: 1xx velo_cluster.cu, 2xx velo_seed.cu, 3xx velo_follow.cu, 4xx velo_track.cu.
+#ifdef VELO_DEBUG
+#define VELO_CHECK(geo, cond, code) do { if (!(cond)) atomicMax((geo).debug_fault, (uint32_t)(code)); } while (0)
+#else
+#define VELO_CHECK(geo, cond, code) ((void)0)
+#endif
 
 // ---- small device helpers -------------------------------------------------------------------
 __device__ __forceinline__ uint32_t lane_id() { return threadIdx.x & 31u; }

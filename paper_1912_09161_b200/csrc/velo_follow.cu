@@ -170,11 +170,13 @@ __device__ __forceinline__ void follow_event(const TrackLaunch& a, uint32_t e, F
           if (t < n_act) {
             const uint32_t st = sm.tstate[t], m = st & 0xFFu, q = st >> 16;
             const uint32_t lq = (uint32_t)i - 1u + m;
+            VELO_CHECK(g, lq < L && q >= sm.lo[lq] && q < sm.lo[lq + 1], 301);
             const Hit hq = load_hit(slab + sm.src[lq] + (q - sm.lo[lq]));
             const uint2 tw = sm.twin[t];
             const uint32_t win = m == 0 ? tw.x : m == 1 ? tw.y : window_slab(recC, nC, phi_of(hq.w), P.w_fwd_phi16);
             const uint32_t cnt = win >> 16;
             uint32_t ic = win & 0xFFFFu;
+            VELO_CHECK(g, cnt <= nC && ic <= nC && nC <= (uint32_t)C::kCap, 302);  // (a wrapped window may start at nC = index 0)
             const float tx = sm.ttx[t], ty = sm.tty[t];
             const int phq = phi_of(hq.w);
             unsigned long long best = kNoClaim;
@@ -265,6 +267,7 @@ __device__ __forceinline__ void follow_event(const TrackLaunch& a, uint32_t e, F
         kept += __popc(bal);
       }
       n_act = kept;
+      VELO_CHECK(g, n_act <= kSeg, 305);
       __syncwarp();
     }
 
@@ -284,6 +287,7 @@ __device__ __forceinline__ void follow_event(const TrackLaunch& a, uint32_t e, F
         const uint32_t ia = ((uint32_t)en >> 20) & 0x3FFu, kb = ((uint32_t)en >> 10) & 0x3FFu, ic = (uint32_t)en & 0x3FFu;
         const bool valid = en != kNoClaim && !((usedA[ia >> 5] >> (ia & 31u)) & 1u) && !((usedB[kb >> 5] >> (kb & 31u)) & 1u) &&
                            !((usedC[ic >> 5] >> (ic & 31u)) & 1u);
+        VELO_CHECK(g, en == kNoClaim || (ia < sm.lo[i + 1] - A0 && kb < A0 - B0 && ic < nC && ia < (uint32_t)C::kCap && kb < (uint32_t)C::kCap), 303);
         if (valid) atomicMin(&sm.bestB[kb], (en & 0xFFFFFFFF00000000ull) | (ia << 16) | ic);
       }
       __syncwarp();
@@ -345,6 +349,7 @@ __device__ __forceinline__ void follow_event(const TrackLaunch& a, uint32_t e, F
           if ((sm.acce[r] >> lane) & 1u) {
             const uint32_t rank = below + __popc(word & ((1u << (kb & 31u)) - 1u));
             const uint32_t slot = n_act + rank, cid = n_created + rank;
+            VELO_CHECK(g, 3 * (cid + 1) <= sm.lo[L], 304);  // a track has three hits of its own: slots [co/3, (co+n)/3)
             if (slot < kSeg) {
               const Hit hb = load_hit(recB + kb), hc = load_hit(recC + ic);
               const float dz = __fsub_rn(hc.z, hb.z);

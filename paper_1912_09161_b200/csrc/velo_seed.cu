@@ -137,6 +137,7 @@ __device__ __forceinline__ void score_doublets(SeedCtx& c, uint32_t n_valid) {
 #pragma unroll 1
     for (uint32_t j = 0; j < c_n; ++j, ++ic) {
       if (ic >= nC) ic -= nC;
+      VELO_CHECK(c.a.geo, ic < nC, 201);
       const uint4 r = __ldg(c.C.rec + ic);
       const float dz = __fsub_rn(__uint_as_float(r.z), zb);
       const float ex = __fsub_rn(__fmaf_rn(tx, dz, xb), __uint_as_float(r.x));
@@ -251,6 +252,7 @@ __device__ __forceinline__ void seed_unit(const TrackLaunch& a, SeedWarp& ws, ui
       const uint32_t nonempty = __ballot_sync(kFull, nd != 0);
       if (nd) {
         const uint32_t s = __popc(nonempty & lanemask_lt());
+        VELO_CHECK(a.geo, s < 32 && a_first <= A.n && c_first <= Cv.n && nd <= A.n && c_n <= Cv.n && kb < 1024, 202);
         ws.bslot[s][0] = r;
         ws.bslot[s][1] = make_uint4(kb, a_first, c_first | (c_n << 16), p);
       }
@@ -270,6 +272,7 @@ __device__ __forceinline__ void seed_unit(const TrackLaunch& a, SeedWarp& ws, ui
         const uint4 hb = ws.bslot[owner][0], bs = ws.bslot[owner][1];
         uint32_t ia = bs.y + (j - bs.w);
         if (ia >= A.n) ia -= A.n;
+        VELO_CHECK(a.geo, owner < 32 && ia < A.n && j - bs.w < A.n, 203);
         const uint4 ha = __ldg(A.rec + ia);
         const float dz_ab = __fsub_rn(__uint_as_float(hb.z), __uint_as_float(ha.z));
         const float tx = __fdiv_rn(__fsub_rn(__uint_as_float(hb.x), __uint_as_float(ha.x)), dz_ab);
@@ -285,6 +288,7 @@ __device__ __forceinline__ void seed_unit(const TrackLaunch& a, SeedWarp& ws, ui
         ws.ring[slot][1] = o1;
       }
       c.ring_n += __popc(bal);
+      VELO_CHECK(a.geo, c.ring_n <= kRing, 204);
       __syncwarp();
       if (c.ring_n >= 32) score_doublets(c, 32);
     }
