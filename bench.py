@@ -516,7 +516,7 @@ def main():
                     help="also produce the simple Kalman fit (SURVEY 8(f1), beyond the headline path; +48 B per track)")
     ap.add_argument("--with-vertices", action="store_true",
                     help="also find primary vertices (SURVEY 8(f2), beyond the headline path; implies --with-kalman)")
-    ap.add_argument("--e2e-chunk", type=int, default=1250, help="events per chunk of the streamed end-to-end run")
+    ap.add_argument("--e2e-chunk", type=int, default=2500, help="events per chunk of the streamed end-to-end run")
     ap.add_argument("--e2e-streams", type=int, default=4)
     ap.add_argument("--sweep", action="store_true",
                     help="also measure BASELINE.json configs[4] (500 / 2k / 50k events) and configs[3] (nu = 12): one line each, "

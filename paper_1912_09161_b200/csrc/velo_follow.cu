@@ -40,7 +40,8 @@ struct __align__(16) FollowSmem {
                                        // marked in `beste` by then)
   float ttx[C::kSeg], tty[C::kSeg];    // active tracks: slopes of the last segment (older -> newest hit)
   uint32_t tstate[C::kSeg];            // newest hit (event-local) << 16 | weak_ok << 15 | n_hits << 8 | missed
-  uint2 twin[C::kSeg];                 // phi windows of the newest hit on the next layer down (.x) and the one below (.y)
+  uint32_t twin[C::kSeg];              // phi windows of the newest hit on the next layer down (low half) and the one below
+                                       // (high half), each first | count << 10; count 63 = "more: search the layer"
   uint16_t tseed[C::kSeg];             // track_key: event-local index of the seed's middle hit
   uint16_t tcid[C::kSeg];              // order of creation within the event
   uint16_t fsel[C::kSeg];              // hit of layer C chosen in T1 (kNone16: none)
@@ -48,7 +49,7 @@ struct __align__(16) FollowSmem {
   uint32_t accw[C::kWords];            // T4: accepted middle hits
   uint32_t acce[C::kWords];            // T4: accepted entries of the list, by round
   uint32_t beste[C::kWords];           // T3: entries that are the best of their middle hit, by round
-  uint32_t lo[kMaxLayers + 1];         // first cluster of every layer, relative to the event
+  uint16_t lo[kMaxLayers + 2];         // first cluster of every layer, relative to the event (an event has < 65536)
   uint32_t src[kMaxLayers];            // first slab entry of every layer
 };
 
@@ -59,6 +60,12 @@ __device__ __forceinline__ uint32_t warp_incl_scan(uint32_t v, uint32_t lane) {
     if (lane >= (uint32_t)d) v += t;
   }
   return v;
+}
+
+// The two forwarding windows of a hit (velo_seed.cu: first | count << 16 each) in 32 bits.
+__device__ __forceinline__ uint32_t pack_windows(uint2 w) {
+  const uint32_t c0 = min(w.x >> 16, 63u), c1 = min(w.y >> 16, 63u);
+  return (w.x & 0x3FFu) | (c0 << 10) | ((w.y & 0x3FFu) << 16) | (c1 << 26);
 }
 
 __device__ __forceinline__ Hit load_hit(const uint4* __restrict__ p) {
@@ -114,7 +121,7 @@ __device__ __forceinline__ void follow_event(const TrackLaunch& a, uint32_t e, F
   const uint2* __restrict__ fwd_win = a.fwd_win + co;
 
 #pragma unroll 1
-  for (uint32_t l = lane; l <= L; l += 32) sm.lo[l] = a.clusters.layer_offsets[e * L + l] - co;
+  for (uint32_t l = lane; l <= L; l += 32) sm.lo[l] = (uint16_t)(a.clusters.layer_offsets[e * L + l] - co);  // (65535 at most: n_cl <= 65535)
 #pragma unroll 1
   for (uint32_t l = lane; l < L; l += 32) sm.src[l] = a.slab_base[e * L + l];
   if (lane < 3 * kWords) (&sm.used[0][0])[lane] = 0;
@@ -172,10 +179,13 @@ __device__ __forceinline__ void follow_event(const TrackLaunch& a, uint32_t e, F
             const uint32_t lq = (uint32_t)i - 1u + m;
             VELO_CHECK(g, lq < L && q >= sm.lo[lq] && q < sm.lo[lq + 1], 301);
             const Hit hq = load_hit(slab + sm.src[lq] + (q - sm.lo[lq]));
-            const uint2 tw = sm.twin[t];
-            const uint32_t win = m == 0 ? tw.x : m == 1 ? tw.y : window_slab(recC, nC, phi_of(hq.w), P.w_fwd_phi16);
-            const uint32_t cnt = win >> 16;
-            uint32_t ic = win & 0xFFFFu;
+            const uint32_t tw = sm.twin[t] >> (m == 0 ? 0 : 16);
+            uint32_t cnt = (tw >> 10) & 0x3Fu, ic = tw & 0x3FFu;
+            if (m >= 2 || cnt == 63u) {  // missed two layers or more (max_skipped >= 2), or a window of 63 hits or more
+              const uint32_t win = window_slab(recC, nC, phi_of(hq.w), P.w_fwd_phi16);
+              cnt = win >> 16;
+              ic = win & 0xFFFFu;
+            }
             VELO_CHECK(g, cnt <= nC && ic <= nC && nC <= (uint32_t)C::kCap, 302);  // (a wrapped window may start at nC = index 0)
             const float tx = sm.ttx[t], ty = sm.tty[t];
             const int phq = phi_of(hq.w);
@@ -227,7 +237,7 @@ __device__ __forceinline__ void follow_event(const TrackLaunch& a, uint32_t e, F
         bool keep = false;
         uint32_t st = 0, seed = 0, cid = 0;
         float tx = 0.f, ty = 0.f;
-        uint2 tw = make_uint2(0, 0);
+        uint32_t tw = 0;
         if (t < n_act) {
           st = sm.tstate[t]; seed = sm.tseed[t]; cid = sm.tcid[t];
           tx = sm.ttx[t]; ty = sm.tty[t]; tw = sm.twin[t];
@@ -237,7 +247,7 @@ __device__ __forceinline__ void follow_event(const TrackLaunch& a, uint32_t e, F
             const uint32_t m = st & 0xFFu, q = st >> 16, lq = (uint32_t)i - 1u + m;
             const Hit hq = load_hit(slab + sm.src[lq] + (q - sm.lo[lq]));
             const Hit hc = load_hit(recC + fc);
-            tw = __ldg(fwd_win + C0 + fc);
+            tw = pack_windows(__ldg(fwd_win + C0 + fc));
             const float dz = __fsub_rn(hc.z, hq.z);
             tx = __fdiv_rn(__fsub_rn(hc.x, hq.x), dz);
             ty = __fdiv_rn(__fsub_rn(hc.y, hq.y), dz);
@@ -359,7 +369,7 @@ __device__ __forceinline__ void follow_event(const TrackLaunch& a, uint32_t e, F
               sm.tstate[slot] = ((C0 + ic) << 16) | (S <= P.s_weak ? 0x8000u : 0u) | (3u << 8);
               sm.tseed[slot] = (uint16_t)(B0 + kb);
               sm.tcid[slot] = (uint16_t)cid;
-              sm.twin[slot] = __ldg(fwd_win + C0 + ic);
+              sm.twin[slot] = pack_windows(__ldg(fwd_win + C0 + ic));
               link[B0 + kb] = (uint16_t)(A0 + ia);
               link[C0 + ic] = (uint16_t)(B0 + kb);
               // layer A leaves after this iteration: its used flags are never read again

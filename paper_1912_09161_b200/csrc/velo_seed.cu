@@ -237,6 +237,8 @@ __device__ __forceinline__ void seed_unit(const TrackLaunch& a, SeedWarp& ws, ui
         uint32_t f1 = c_first, n1 = c_n, f2 = 0, n2 = 0;
         if (P.w_fwd_phi16 != P.w_seed_phi16) phi_window(Cv, phb, P.w_fwd_phi16, f1, n1);
         if (l >= 2) phi_window_slices(D, phb, P.w_fwd_phi16, f2, n2);
+        if (f1 >= Cv.n) f1 = 0;  // (a wrapped window may start "behind the last hit" = at hit 0)
+        if (f2 >= D.n) f2 = 0;
         a.fwd_win[dst + kb] = make_uint2(f1 | (n1 << 16), f2 | (n2 << 16));
         if (middle && c_n) phi_window(A, phb, P.w_seed_phi16, a_first, nd);
       }
