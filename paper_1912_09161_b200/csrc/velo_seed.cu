@@ -213,6 +213,20 @@ __device__ __forceinline__ void seed_unit(const TrackLaunch& a, SeedWarp& ws, ui
     A.n = A1 - A0;
   }
   if (lane == 0) ws.n_trip = 0;
+  // Ask for everything the unit will read before the first dependent load needs it: its own records, the records and
+  // phi tables of the neighbouring layers (the cluster kernel's output is long gone from the L2 for a batch this size).
+  {
+    auto prefetch = [&](const void* ptr, uint32_t bytes) {
+      const char* q = reinterpret_cast<const char*>(ptr);
+#pragma unroll 1
+      for (uint32_t o = lane * 128u; o < bytes; o += 32u * 128u) asm volatile("prefetch.global.L1 [%0];" ::"l"(q + o));
+    };
+    prefetch(recB, 16u * nB);
+    prefetch(infoB, 16u * nB);
+    if (Cv.n) { prefetch(Cv.rec, 16u * Cv.n); prefetch(Cv.tab, 2u * (kPhiSlices + 1)); }
+    if (A.n) { prefetch(A.rec, 16u * A.n); prefetch(A.tab, 2u * (kPhiSlices + 1)); }
+    if (D.n) prefetch(D.tab, 2u * (kPhiSlices + 1));
+  }
   __syncwarp();
   SeedCtx c{a, ws, Cv, a.trip + co + B0, nB, lane, 0u, 0u};
   const uint32_t dst = co + B0;
