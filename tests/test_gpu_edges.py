@@ -201,3 +201,26 @@ def test_local_clustering_variant_against_the_oracle(geometry, batch_of, regions
     assert np.array_equal(t.hits, ref.tracks.hits)
     c0, _ = as_oracle_types(*back)
     assert not compare_clusters(c0, exact.clusters)  # switched off again: exact components
+
+
+def test_more_than_65535_clusters_in_one_event(velo, geometry):
+    """R8: hit indices are 16 bit, so an event with more than 65535 clusters gets its clusters (all exact) but no tracks,
+    and is flagged TOO_MANY_CLUSTERS; the oracle does the same.  The other event of the batch is untouched."""
+    import oracle
+    from paper_1912_09161_b200 import binding, workload
+    from tests.helpers import compare_clusters
+
+    # isolated pixels on a 3 x 3 grid over all 104 sensors: 256 x 85 per sensor would be too many; 700 per sensor = 72 800
+    big = [(s, 3 * (k % 256), 3 * (k // 256)) for s in range(geometry.n_sensors) for k in range(700)]
+    small = workload.generate(1, n_events=1)
+    m = small.pixels["event"] == 0
+    other = sorted(set(zip(small.pixels["sensor"][m].tolist(), small.pixels["col"][m].tolist(), small.pixels["row"][m].tolist())))
+    raw, off = workload.pack_events(geometry, [big, other], shuffle_seed=1)
+    ref = oracle.reconstruct(geometry, raw, off)
+    assert int(ref.clusters.event_offsets[1]) == len(big) > 65535
+    assert ref.clusters.status.tolist() == [oracle.STATUS_TOO_MANY_CLUSTERS, 0]
+    clusters, tracks = binding.reconstruct_batch(velo, raw, off)
+    c, t = as_oracle_types(clusters, tracks)
+    assert not compare_clusters(c, ref.clusters)
+    assert np.array_equal(t.event_offsets, ref.tracks.event_offsets) and t.event_offsets[1] == 0
+    assert np.array_equal(t.hits, ref.tracks.hits) and len(t.hits) > 0
