@@ -80,7 +80,10 @@ size_t fixed_bytes(uint32_t n_events, uint32_t n_layers, uint32_t n_mid_sms) {
   return b + 16 * kAlign;
 }
 
-size_t per_entry_bytes() { return kSlabEntryBytes + kTrackScratchBytes + (kTrackSlotBytes + 2) / 3; }
+// Per raw SP word: THREE slab entries (one in the dense part, placed from the bank table; two behind it, because a layer
+// with more clusters than SP words moves there as a whole and a super-pixel holds up to two clusters) and the tracking
+// scratch of TWO clusters.
+size_t per_word_bytes() { return 3 * kSlabEntryBytes + 2 * (kTrackScratchBytes + (kTrackSlotBytes + 2) / 3); }
 
 int fail(allen_velo* h, int code, const char* what, cudaError_t err = cudaSuccess) {
   if (h) {
@@ -183,10 +186,10 @@ int allen_velo_create(const allen_velo_geometry_t* geo, allen_velo_t** out) {
 size_t allen_velo_workspace_bytes(const allen_velo_t* h, uint32_t n_events, size_t raw_bytes) {
   if (!h) return 0;
   if ((uint64_t)n_events * h->dev.n_layers >= (1ull << 31)) return 0;  // reconstruct() refuses such a batch
-  // slab and tracking scratch: two entries per raw word (a super-pixel holds at most two clusters): one in the dense
+  // slab and tracking scratch per raw word (per_word_bytes): a super-pixel holds at most two clusters: one in the dense
   // part of the slab, one behind it for layers with more clusters than SP words
-  const size_t entries = raw_bytes / 2 + 4096;
-  return fixed_bytes(n_events, h->dev.n_layers, h->n_mid_sms) + entries * per_entry_bytes() + 16 * kAlign;
+  const size_t words = raw_bytes / 4 + 2048;
+  return fixed_bytes(n_events, h->dev.n_layers, h->n_mid_sms) + words * per_word_bytes() + 16 * kAlign;
 }
 
 int allen_velo_set_occupancy_hint(allen_velo_t* h, uint32_t sp_words_per_layer) {
@@ -251,7 +254,7 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
 
   // ---- carve the workspace
   const size_t fixed = fixed_bytes(n_events, L, h->n_mid_sms);
-  if (!h->ws || h->ws_bytes < fixed + 1024 * per_entry_bytes() + 16 * kAlign) return fail(h, ALLEN_VELO_ERR_WORKSPACE, "workspace too small");
+  if (!h->ws || h->ws_bytes < fixed + 512 * per_word_bytes() + 16 * kAlign) return fail(h, ALLEN_VELO_ERR_WORKSPACE, "workspace too small");
   const uint32_t items = n_events * L;
   Carve cv{static_cast<unsigned char*>(h->ws)};
   uint32_t* counts = cv.take<uint32_t>(items);
@@ -275,14 +278,16 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
   uint32_t* trk_counters = cv.take<uint32_t>(16);
   uint32_t* trip_count = cv.take<uint32_t>(items);
   uint16_t* phi_tab = cv.take<uint16_t>((size_t)items * kPhiTabStride);
-  size_t entries = (h->ws_bytes - cv.used - 16 * kAlign) / per_entry_bytes();
-  if (entries > 0x7FFFFFF0u) entries = 0x7FFFFFF0u;
+  size_t words = (h->ws_bytes - cv.used - 16 * kAlign) / per_word_bytes();
+  if (words > 0x2AAAAAA0u) words = 0x2AAAAAA0u;
+  const size_t slab_entries = 3 * words;
+  const size_t entries = 2 * words;  // clusters the tracking scratch (indexed by output cluster) can hold
   ClusterSlab slab{};
-  slab.capacity = (uint32_t)entries;
-  slab.dense = (uint32_t)(entries / 2);
-  slab.rec = cv.take<uint4>(entries);
-  slab.info = cv.take<uint4>(entries);
-  slab.checksum = cv.take<uint32_t>(entries);
+  slab.capacity = (uint32_t)slab_entries;
+  slab.dense = (uint32_t)words;
+  slab.rec = cv.take<uint4>(slab_entries);
+  slab.info = cv.take<uint4>(slab_entries);
+  slab.checksum = cv.take<uint32_t>(slab_entries);
   slab.spill_cursor = reinterpret_cast<uint32_t*>(state) + 1;
   slab.phi_tab = phi_tab;
   // tracking scratch is addressed by output cluster index; it shares the entry count with the slab

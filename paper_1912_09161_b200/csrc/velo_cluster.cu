@@ -131,7 +131,7 @@ template <bool kChecksum>
 __device__ __forceinline__ bool ccl_pass(const Pass& p, const ClusterStore& cs, const DeviceGeometry& g,
                                          const uint32_t* __restrict__ spw, uint32_t my_sensor, uint32_t my_off,
                                          uint32_t my_cnt, uint32_t k0, uint32_t k1, uint32_t& n_cl, bool& bad_sp,
-                                         uint32_t* n_edges_ctr) {
+                                         uint32_t* n_edges_ctr, bool sparse) {
   const uint32_t lane = lane_id();
   const uint32_t bits = p.hash_bits;
   // ---- stage the SP words of the group (R1: addresses outside the sensor are ignored and flagged).  The group is
@@ -214,10 +214,68 @@ __device__ __forceinline__ bool ccl_pass(const Pass& p, const ClusterStore& cs, 
   if (lane == 0) *n_edges_ctr = 0;
   __syncwarp();
 
+  // ---- isolated super-pixels (most of them at nu = 6: two thirds of the fired pixels are noise).  A super-pixel with no
+  //      other super-pixel in the coarse cells around it (1 SP column x 32 SP rows per cell; a bit map of the occupied
+  //      cells and one of the cells holding more than one SP, in the cluster-record arrays, which are free until the
+  //      roots are numbered) has no neighbour: it needs no hash entry and no look-up, its components are roots.  Only the
+  //      others are listed (ballot) and go through insert and edges below: two rounds of 32 instead of five for a typical
+  //      layer.  The test is conservative (cells are folded modulo kOccCells; a far SP in a neighbouring cell only costs
+  //      the slow path), and symmetric for true neighbours, so every neighbour of a listed SP is listed too.
+  constexpr uint32_t kOccCells = 4096, kOccWords = kOccCells / 32;
+  uint16_t* nz = nullptr;
+  uint32_t n_nz = n;
+  if (sparse) {
+    uint32_t* occ = cs.key;              // (sparse: the caller's records are in shared memory and n_cl == 0)
+    uint32_t* multi = cs.key + kOccWords;
+    nz = reinterpret_cast<uint16_t*>(cs.key + 2 * kOccWords);
+#pragma unroll 1
+    for (uint32_t s = lane; s < 2 * kOccWords; s += 32) occ[s] = 0;
+    __syncwarp();
+    auto cell_of = [&](uint32_t k, uint32_t C, uint32_t band) { return ((k * g.sp_cols + C) * 2u + band) & (kOccCells - 1u); };
+#pragma unroll 1
+    for (uint32_t i = lane; i < n; i += 32) {
+      const uint32_t w = p.sp[i];
+      if (!w) continue;
+      const uint32_t cell = cell_of(w >> 23, (w >> 14) & 0x1FFu, ((w >> 8) & 0x3Fu) >> 5);
+      const uint32_t bit = 1u << (cell & 31u);
+      if (atomicOr(&occ[cell >> 5], bit) & bit) atomicOr(&multi[cell >> 5], bit);
+    }
+    __syncwarp();
+    n_nz = 0;
+#pragma unroll 1
+    for (uint32_t i0 = 0; i0 < n; i0 += 32) {
+      const uint32_t i = i0 + lane;
+      const uint32_t w = i < n ? p.sp[i] : 0u;
+      bool listed = false;
+      if (w) {
+        const uint32_t k = w >> 23, C = (w >> 14) & 0x1FFu, R = (w >> 8) & 0x3Fu, band = R >> 5;
+        auto hit = [&](const uint32_t* map, uint32_t c, uint32_t b) {
+          const uint32_t cell = cell_of(k, c, b);
+          return (map[cell >> 5] >> (cell & 31u)) & 1u;
+        };
+        uint32_t any = hit(multi, C, band);
+        if (C >= 1) any |= hit(occ, C - 1, band);
+        if (C + 1 < g.sp_cols) any |= hit(occ, C + 1, band);
+        const uint32_t other = R >= 1 && ((R - 1) >> 5) != band ? band - 1 : R + 1 < g.sp_rows && ((R + 1) >> 5) != band ? band + 1 : band;
+        if (other != band) {
+          any |= hit(occ, C, other);
+          if (C >= 1) any |= hit(occ, C - 1, other);
+          if (C + 1 < g.sp_cols) any |= hit(occ, C + 1, other);
+        }
+        listed = any != 0;
+      }
+      const uint32_t bal = __ballot_sync(kFull, listed);
+      if (listed) nz[n_nz + __popc(bal & lanemask_lt())] = (uint16_t)i;
+      n_nz += __popc(bal);
+    }
+    __syncwarp();
+  }
+
   // ---- insert: entry = key << 14 | (index + 1); a repeated address merges its hitmap into the first one (R1)
   const uint32_t mask = (1u << bits) - 1u;
 #pragma unroll 1
-  for (uint32_t i = lane; i < n; i += 32) {
+  for (uint32_t j = lane; j < n_nz; j += 32) {
+    const uint32_t i = nz ? nz[j] : j;
     const uint32_t w = p.sp[i];
     if (!w) continue;
     const uint32_t key = (w >> 8) & 0x3FFFFu;
@@ -240,11 +298,12 @@ __device__ __forceinline__ bool ccl_pass(const Pass& p, const ClusterStore& cs, 
 
   // ---- edges to touching forward neighbours; node = 2 * index + component
 #pragma unroll 1
-  for (uint32_t i = lane; i < n; i += 32) {
+  for (uint32_t x = lane; x < 2 * n; x += 32) p.lab[x] = (uint16_t)x;  // (dead entries too: the pointer-jumping pass reads every label)
+#pragma unroll 1
+  for (uint32_t j = lane; j < n_nz; j += 32) {
+    const uint32_t i = nz ? nz[j] : j;
     const uint32_t w = p.sp[i];
     const uint32_t nA = 2 * i, nB = 2 * i + 1;
-    p.lab[nA] = (uint16_t)nA;  // (dead entries too: the pointer-jumping pass reads every label)
-    p.lab[nB] = (uint16_t)nB;
     if (!w) continue;
     const uint32_t h = w & 0xFFu, R = (w >> 8) & 0x3Fu, C = (w >> 14) & 0x1FFu;
     const uint32_t key = (w >> 8) & 0x3FFFFu;
@@ -497,7 +556,7 @@ __device__ __noinline__ bool ccl_pass_generic(const Pass& p, const ClusterStore&
                                               const uint32_t* __restrict__ spw, uint32_t my_sensor, uint32_t my_off,
                                               uint32_t my_cnt, uint32_t k0, uint32_t k1, uint32_t& n_cl, bool& bad_sp,
                                               uint32_t* n_edges_ctr) {
-  return ccl_pass<kChecksum>(p, cs, g, spw, my_sensor, my_off, my_cnt, k0, k1, n_cl, bad_sp, n_edges_ctr);
+  return ccl_pass<kChecksum>(p, cs, g, spw, my_sensor, my_off, my_cnt, k0, k1, n_cl, bad_sp, n_edges_ctr, false);
 }
 template <bool kChecksum>
 __device__ __noinline__ void finish_layer_generic(const ClusterLaunch& a, const ClusterStore& cs, const SortStore& ss,
@@ -605,7 +664,7 @@ __device__ __forceinline__ void cluster_item(const ClusterLaunch& a, WarpSmem<kC
     return;
   }
   if (mode == 0) {
-    if (ccl_pass<kChecksum>(fast, cs, g, spw, my_sensor, my_off, cnt_k, 0, K, n_cl, bad_sp, &ws.n_edges)) {
+    if (ccl_pass<kChecksum>(fast, cs, g, spw, my_sensor, my_off, cnt_k, 0, K, n_cl, bad_sp, &ws.n_edges, true)) {
       if (__any_sync(kFull, bad_sp) && lane == 0) atomicOr(a.status + e, ALLEN_VELO_STATUS_BAD_SP);
       finish_layer<kChecksum>(a, cs, ss, item, slab0, n_sp_layer, n_cl);
       return;
