@@ -231,12 +231,15 @@ __device__ __forceinline__ bool ccl_pass(const Pass& p, const ClusterStore& cs, 
 #pragma unroll 1
     for (uint32_t s = lane; s < 2 * kOccWords; s += 32) occ[s] = 0;
     __syncwarp();
-    auto cell_of = [&](uint32_t k, uint32_t C, uint32_t band) { return ((k * g.sp_cols + C) * 2u + band) & (kOccCells - 1u); };
+    // cell of (sensor k, SP column C, band = SP row / 32) = bit 2 * (k * sp_cols + C) + band: the six cells around an SP
+    // (columns C-1 .. C+1, two bands) are six consecutive bits.  (Column -1 / sp_cols of a sensor is a column of its
+    // neighbour in the numbering, and the numbering is folded modulo kOccCells: both only ever add occupied cells.)
+    auto base_of = [&](uint32_t w) { return 2u * ((w >> 23) * g.sp_cols + ((w >> 14) & 0x1FFu)); };
 #pragma unroll 1
     for (uint32_t i = lane; i < n; i += 32) {
       const uint32_t w = p.sp[i];
       if (!w) continue;
-      const uint32_t cell = cell_of(w >> 23, (w >> 14) & 0x1FFu, ((w >> 8) & 0x3Fu) >> 5);
+      const uint32_t cell = (base_of(w) + (((w >> 8) & 0x3Fu) >> 5)) & (kOccCells - 1u);
       const uint32_t bit = 1u << (cell & 31u);
       if (atomicOr(&occ[cell >> 5], bit) & bit) atomicOr(&multi[cell >> 5], bit);
     }
@@ -248,21 +251,15 @@ __device__ __forceinline__ bool ccl_pass(const Pass& p, const ClusterStore& cs, 
       const uint32_t w = i < n ? p.sp[i] : 0u;
       bool listed = false;
       if (w) {
-        const uint32_t k = w >> 23, C = (w >> 14) & 0x1FFu, R = (w >> 8) & 0x3Fu, band = R >> 5;
-        auto hit = [&](const uint32_t* map, uint32_t c, uint32_t b) {
-          const uint32_t cell = cell_of(k, c, b);
-          return (map[cell >> 5] >> (cell & 31u)) & 1u;
-        };
-        uint32_t any = hit(multi, C, band);
-        if (C >= 1) any |= hit(occ, C - 1, band);
-        if (C + 1 < g.sp_cols) any |= hit(occ, C + 1, band);
-        const uint32_t other = R >= 1 && ((R - 1) >> 5) != band ? band - 1 : R + 1 < g.sp_rows && ((R + 1) >> 5) != band ? band + 1 : band;
-        if (other != band) {
-          any |= hit(occ, C, other);
-          if (C >= 1) any |= hit(occ, C - 1, other);
-          if (C + 1 < g.sp_cols) any |= hit(occ, C + 1, other);
-        }
-        listed = any != 0;
+        const uint32_t R = (w >> 8) & 0x3Fu, band = R >> 5;
+        const uint32_t own = (base_of(w) + band) & (kOccCells - 1u);
+        const uint32_t first = (base_of(w) - 2u) & (kOccCells - 1u);  // cell (C-1, band 0); even
+        const uint32_t wi = first >> 5, sh = first & 31u;
+        const uint32_t win = __funnelshift_r(occ[wi], occ[(wi + 1) & (kOccWords - 1u)], sh) & 0x3Fu;
+        // neighbours in the same band: columns C-1 and C+1; in the other band (only if row R-1 or R+1 lies there): all three
+        const bool crosses = (R >= 1 && ((R - 1) >> 5) != band) || (R + 1 < g.sp_rows && ((R + 1) >> 5) != band);
+        const uint32_t near = (0x11u << band) | (crosses ? (0x15u << (1u - band)) : 0u);
+        listed = (win & near) != 0 || ((multi[own >> 5] >> (own & 31u)) & 1u) != 0;
       }
       const uint32_t bal = __ballot_sync(kFull, listed);
       if (listed) nz[n_nz + __popc(bal & lanemask_lt())] = (uint16_t)i;
