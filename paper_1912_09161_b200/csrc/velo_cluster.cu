@@ -265,6 +265,7 @@ __device__ __forceinline__ bool ccl_pass(const Pass& p, const ClusterStore& cs, 
       if (listed) nz[n_nz + __popc(bal & lanemask_lt())] = (uint16_t)i;
       n_nz += __popc(bal);
     }
+    VELO_CHECK(g, n_nz <= n && 4 * (2 * kOccWords) + 2 * n <= 16 * cs.cap, 106);  // bit maps + list fit the record arrays
     __syncwarp();
   }
 

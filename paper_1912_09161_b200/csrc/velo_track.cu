@@ -1,23 +1,21 @@
-// Kernel 2 of the VELO hot path, CTA-per-event instances: the second pass for the events the two-kernel path
-// (velo_seed.cu + velo_follow.cu) hands on (seed list or track slots exhausted, event too large to stage): search by triplet
-// (A5 seeding, A6 forwarding, A7 clone/ghost killing) and the straight-line fit (A8) — SURVEY.md §8(a); the algorithm is DESIGN.md reading R5 (T1..T5) of P:181-183 ("forming
-// seeds of three hits from consecutive layers ('triplets'), and then extending these to the other layers"; "sort hits
-// on every layer by phi for fast look-up") and R6 of P:149 (straight lines).
+// Second pass of the track search, and the kernels around it: classification of the events, compaction of the tracks.
 //
-// One CTA per event ("a single event is assigned to one block, while intra-event parallelism is mapped to the threads
-// within one block").  The L-2 layer iterations are sequential.  Design for sm_100a:
+// The events the two-kernel path (velo_seed.cu + velo_follow.cu) hands on — a candidate list that outgrew its region, or
+// more active tracks than velo_follow keeps — are searched here by ONE CTA per event ("a single event is assigned to one
+// block, while intra-event parallelism is mapped to the threads within one block"): search by triplet (A5 seeding,
+// A6 forwarding, A7 clone/ghost killing) and the straight-line fit (A8) — SURVEY.md §8(a); reading R5 (T1..T5) of
+// P:181-183 and R6 of P:149.  This is the track kernel of round 1 (it applies the used flags before it looks for
+// triplets, six block barriers per layer iteration), reading the compacted cluster output velo_seed.cu has filled:
 //  * the three layers of an iteration live in shared memory as 16-byte hit records (x, y, z, phi16 | used << 16) in a
 //    ring of three slots: one LDS.128 per candidate; the next layer is brought in with cp.async into the slot of the
-//    layer that leaves, as soon as the seeding is done with it, so its DRAM latency hides behind T4;
+//    layer that leaves, as soon as the seeding is done with it;
 //  * phi look-up uses a 128-bucket start table per layer, built while the layer is staged (no binary search);
-//  * seeding is flattened: S1 lists (b, a) doublets inside the phi window, S2 gives every doublet one thread that
-//    scans b's window on layer C; the per-b argmin is a 64-bit shared-memory atomicMin on (bits(S), a, c);
+//  * S1 lists (b, a) doublets inside the phi window, S2 gives every doublet one thread that scans b's window on layer
+//    C; the per-b argmin is a 64-bit shared-memory atomicMin on (bits(S), a, c);
 //  * all conflict rules are order-independent minima on packed keys (bits(S) << 32 | index): no "first thread wins",
 //    so the result is exactly the oracle's whatever the thread schedule;
-//  * compaction of the clusters (A9) rides along: an extra warp copies the event's layers from the cluster kernel's
-//    slab to their final place while the tracking warps (own named barrier) search;
-//  * the kernel is instantiated for three staging capacities (256 / 512 / 1024 hits per layer); every event is taken
-//    by the smallest instance it fits, and an instance that runs out of track slots hands the event to the next one.
+//  * two instances by staging capacity (512 / 1024 hits per layer); one that runs out of track slots hands the event to
+//    the next, the last one flags it STAGE_OVERFLOW.
 #include <cuda_pipeline.h>
 
 #include "velo_track.cuh"
@@ -28,7 +26,7 @@ namespace {
 constexpr int kBuckets = 128;
 constexpr int kBucketShift = 9;  // 65536 / 128
 
-template <int kThreads_, int kCap_, int kCapTracks_, int kCapDoublets_, int kLevel_, bool kLast_, bool kCopier_>
+template <int kThreads_, int kCap_, int kCapTracks_, int kCapDoublets_, int kLevel_, bool kLast_>
 struct Cfg {
   static constexpr int kThreads = kThreads_;
   static constexpr int kCap = kCap_;            // hits of one layer staged
@@ -36,15 +34,14 @@ struct Cfg {
   static constexpr int kCapDoublets = kCapDoublets_;
   static constexpr int kLevel = kLevel_;
   static constexpr bool kLast = kLast_;
-  static constexpr bool kCopier = kCopier_;      // an extra warp moves the event's clusters from the slab to the output
-  static constexpr int kBlock = kThreads + (kCopier ? 32 : 0);
+  static constexpr int kBlock = kThreads;
   static constexpr int kWarps = kThreads / 32;
   static constexpr int kRoundsB = (kCap + kThreads - 1) / kThreads;
   static constexpr int kRoundsT = (kCapTracks + kThreads - 1) / kThreads;
 };
 // second pass for events the two-kernel path ran out of track or list slots on: their clusters are already in the output
-using CfgMr = Cfg<256, 512, 1024, 4096, 1, false, false>;
-using CfgLr = Cfg<512, 1024, 2048, 2048, 2, true, false>;
+using CfgMr = Cfg<256, 512, 1024, 4096, 1, false>;
+using CfgLr = Cfg<512, 1024, 2048, 2048, 2, true>;
 
 template <class C>
 struct Smem {
@@ -80,20 +77,14 @@ __device__ __forceinline__ uint32_t lower_bound_phi(const uint16_t* __restrict__
 
 __device__ __forceinline__ int wrap16(int v) { return (int)(int16_t)(uint16_t)v; }
 
-// Barrier over the tracking threads only (the copier warp, if any, runs on its own).
 template <class C>
-__device__ __forceinline__ void tsync() {
-  if (C::kCopier) asm volatile("bar.sync 1, %0;" ::"n"(C::kThreads) : "memory");
-  else __syncthreads();
-}
+__device__ __forceinline__ void tsync() { __syncthreads(); }
 
-// Where the hits are read from: the cluster kernel's slab of 16-byte records (instances with a copier warp) or the
-// compacted output an earlier kernel has filled (second-pass instances).
+// The hits are read from the compacted cluster output (velo_seed.cu has filled it).
 template <class C>
 struct Ctx {
   Smem<C>& sm;
-  const uint4* __restrict__ R;       // slab records (kCopier)
-  const float* __restrict__ X;       // output arrays (!kCopier)
+  const float* __restrict__ X;
   const float* __restrict__ Y;
   const float* __restrict__ Z;
   const int16_t* __restrict__ PHI;
@@ -104,17 +95,12 @@ struct Ctx {
 template <class C>
 __device__ __forceinline__ Hit far_hit(const Ctx<C>& c, uint32_t s) {
   Hit h;
-  if (C::kCopier) {
-    const uint4 r = __ldg(c.R + s);
-    h.x = __uint_as_float(r.x); h.y = __uint_as_float(r.y); h.z = __uint_as_float(r.z); h.w = r.w;
-  } else {
-    h.x = __ldg(c.X + s); h.y = __ldg(c.Y + s); h.z = __ldg(c.Z + s); h.w = (uint16_t)__ldg(c.PHI + s);
-  }
+  h.x = __ldg(c.X + s); h.y = __ldg(c.Y + s); h.z = __ldg(c.Z + s); h.w = (uint16_t)__ldg(c.PHI + s);
   return h;
 }
 
-// Bring layer `l` into ring slot l % 3 by cp.async (one 16-byte copy per hit from the slab, or three 4-byte copies from
-// the output arrays); the bucket table by this thread.  Completion: __pipeline_wait_prior(0) + barrier by the caller.
+// Bring layer `l` into ring slot l % 3 by cp.async (three 4-byte copies per hit from the output arrays); the bucket table
+// by this thread.  Completion: __pipeline_wait_prior(0) + barrier by the caller.
 template <class C>
 __device__ __forceinline__ void stage_layer(const Ctx<C>& c, uint32_t l) {
   Smem<C>& sm = c.sm;
@@ -128,19 +114,12 @@ __device__ __forceinline__ void stage_layer(const Ctx<C>& c, uint32_t l) {
   }
 #pragma unroll 1
   for (uint32_t k = threadIdx.x; k < n; k += C::kThreads) {
-    uint32_t ph, ph_prev = 0;
-    if (C::kCopier) {
-      __pipeline_memcpy_async(&rec[k], c.R + base + k, 16);  // the record's last word is phi16 with a clear used bit
-      ph = __ldg(reinterpret_cast<const uint32_t*>(c.R + base + k) + 3) & 0xFFFFu;
-      if (k) ph_prev = __ldg(reinterpret_cast<const uint32_t*>(c.R + base + k - 1) + 3) & 0xFFFFu;
-    } else {
-      __pipeline_memcpy_async(&rec[k].x, c.X + base + k, 4);
-      __pipeline_memcpy_async(&rec[k].y, c.Y + base + k, 4);
-      __pipeline_memcpy_async(&rec[k].z, c.Z + base + k, 4);
-      ph = (uint16_t)__ldg(c.PHI + base + k);
-      rec[k].w = ph;
-      if (k) ph_prev = (uint16_t)__ldg(c.PHI + base + k - 1);
-    }
+    __pipeline_memcpy_async(&rec[k].x, c.X + base + k, 4);
+    __pipeline_memcpy_async(&rec[k].y, c.Y + base + k, 4);
+    __pipeline_memcpy_async(&rec[k].z, c.Z + base + k, 4);
+    const uint32_t ph = (uint16_t)__ldg(c.PHI + base + k);
+    rec[k].w = ph;
+    const uint32_t ph_prev = k ? (uint16_t)__ldg(c.PHI + base + k - 1) : 0u;
     const int bk = (int)((ph ^ 0x8000u) >> kBucketShift);
     const int bp = k ? (int)((ph_prev ^ 0x8000u) >> kBucketShift) : -1;
 #pragma unroll 1
@@ -184,22 +163,7 @@ __device__ __forceinline__ void process_doublet(const Ctx<C>& c, const Hit* __re
   if (best != kNoClaim) atomicMin(&c.sm.best[kb], best);
 }
 
-// Copy n clusters from slab position src to position dst of the compacted output.
-__device__ __forceinline__ void copy_clusters(const TrackLaunch& a, uint32_t src, uint32_t dst, uint32_t n,
-                                              uint32_t first, uint32_t step) {
-#pragma unroll 1
-  for (uint32_t k = first; k < n; k += step) {
-    const uint32_t s = src + k, d = dst + k;
-    const uint4 r = __ldg(a.slab.rec + s), q = __ldg(a.slab.info + s);
-    a.clusters.key[d] = q.x; a.clusters.n_pixels[d] = q.y; a.clusters.sum_col[d] = q.z; a.clusters.sum_row[d] = q.w;
-    a.clusters.x[d] = __uint_as_float(r.x); a.clusters.y[d] = __uint_as_float(r.y); a.clusters.z[d] = __uint_as_float(r.z);
-    a.clusters.phi16[d] = (int16_t)(uint16_t)r.w;
-    if (a.clusters.checksum) a.clusters.checksum[d] = __ldg(a.slab.checksum + s);
-  }
-}
-
-// Offsets of the event's layers: lo[] relative to the event's first cluster, src[] absolute in the arrays the hits
-// are read from (the slab for instances with a copier warp, else the output a previous kernel has filled).
+// Offsets of the event's layers: lo[] relative to the event's first cluster, src[] absolute in the output arrays.
 template <class C>
 __device__ __forceinline__ void load_offsets(const TrackLaunch& a, uint32_t e, Smem<C>& sm, uint32_t co) {
   const uint32_t L = a.geo.n_layers;
@@ -207,10 +171,10 @@ __device__ __forceinline__ void load_offsets(const TrackLaunch& a, uint32_t e, S
   for (uint32_t l = threadIdx.x; l <= L; l += C::kBlock) sm.lo[l] = a.clusters.layer_offsets[e * L + l] - co;
 #pragma unroll 1
   for (uint32_t l = threadIdx.x; l < L; l += C::kBlock)
-    sm.src[l] = C::kCopier ? a.slab_base[e * L + l] : a.clusters.layer_offsets[e * L + l];
+    sm.src[l] = a.clusters.layer_offsets[e * L + l];
 }
 
-// Search by triplet, fit and (with a copier warp) cluster compaction for event e; the whole CTA calls it.
+// Search by triplet and fit for event e; the whole CTA calls it.
 template <class C>
 __device__ __forceinline__ void track_event(const TrackLaunch& a, uint32_t e, Smem<C>& sm) {
   const DeviceGeometry& g = a.geo;
@@ -221,16 +185,7 @@ __device__ __forceinline__ void track_event(const TrackLaunch& a, uint32_t e, Sm
   if (tid == 0) { sm.flags = 0; sm.min_active[0] = 0; sm.min_active[1] = 0; sm.n_doublets = 0; }
   if (tid < (uint32_t)(C::kCap + 31) / 32) sm.ovf[tid] = 0;
   __syncthreads();
-  if (C::kCopier && tid >= (uint32_t)C::kThreads) {
-    // copier warp: layers in the order the search stages them (their slab lines are then in L2 for both readers)
-#pragma unroll 1
-    for (int l = (int)L - 1; l >= 0; --l)
-      copy_clusters(a, sm.src[l], co + sm.lo[l], sm.lo[l + 1] - sm.lo[l], lane, 32);
-    __syncthreads();  // pairs with the barrier before the fit: the output arrays are complete
-    return;
-  }
-
-  Ctx<C> c{sm, a.slab.rec, a.clusters.x, a.clusters.y, a.clusters.z, a.clusters.phi16, g.params};
+  Ctx<C> c{sm, a.clusters.x, a.clusters.y, a.clusters.z, a.clusters.phi16, g.params};
   const allen_velo_params_t& P = c.P;
   uint16_t* link = a.link + co;
 
@@ -515,8 +470,7 @@ __device__ __forceinline__ void track_event(const TrackLaunch& a, uint32_t e, Sm
   // ---- T5 finalise + A8 fit: keep >= 4 hits, or 3 hits with S_seed <= s_weak; output in order of creation
   uint32_t out_tracks = 0, out_hits = 0;
   const uint32_t trk0 = co / 3;
-  // the fit reads the compacted output (complete: the copier warp passed the barrier above, or an earlier kernel
-  // filled it); __ldcg because these lines may have been written during this kernel
+  // the fit reads the compacted output (an earlier kernel filled it)
   const float* X = a.clusters.x + co;
   const float* Y = a.clusters.y + co;
   const float* Z = a.clusters.z + co;
