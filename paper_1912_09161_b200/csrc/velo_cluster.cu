@@ -278,7 +278,7 @@ __device__ __forceinline__ bool ccl_pass(const Pass& p, const ClusterStore& cs, 
     if (!w) continue;
     const uint32_t key = (w >> 8) & 0x3FFFFu;
     uint32_t s = hash_slot(key, bits);
-    uint32_t probes = 0;
+    [[maybe_unused]] uint32_t probes = 0;
 #pragma unroll 1
     for (;;) {
       VELO_CHECK(g, ++probes <= (1u << bits), 101);  // the table has twice as many slots as entries: a free one exists

@@ -281,8 +281,68 @@ __device__ __forceinline__ void follow_event(const TrackLaunch& a, uint32_t e, F
       __syncwarp();
     }
 
+    // A new track from an accepted entry: `rank` = accepted middle hits below its b (tracks are created in ascending b).
+    auto create_track = [&](unsigned long long en, uint32_t rank) {
+      const uint32_t ia = ((uint32_t)en >> 20) & 0x3FFu, kb = ((uint32_t)en >> 10) & 0x3FFu, ic = (uint32_t)en & 0x3FFu;
+      const uint32_t slot = n_act + rank, cid = n_created + rank;
+      VELO_CHECK(g, 3 * (cid + 1) <= sm.lo[L], 304);  // a track has three hits of its own: slots [co/3, (co+n)/3)
+      if (slot < kSeg) {
+        const Hit hb = load_hit(recB + kb), hc = load_hit(recC + ic);
+        const float dz = __fsub_rn(hc.z, hb.z);
+        sm.ttx[slot] = __fdiv_rn(__fsub_rn(hc.x, hb.x), dz);
+        sm.tty[slot] = __fdiv_rn(__fsub_rn(hc.y, hb.y), dz);
+        const float S = __uint_as_float((uint32_t)(en >> 32));
+        sm.tstate[slot] = ((C0 + ic) << 16) | (S <= P.s_weak ? 0x8000u : 0u) | (3u << 8);
+        sm.tseed[slot] = (uint16_t)(B0 + kb);
+        sm.tcid[slot] = (uint16_t)cid;
+        sm.twin[slot] = pack_windows(__ldg(fwd_win + C0 + ic));
+        link[B0 + kb] = (uint16_t)(A0 + ia);
+        link[C0 + ic] = (uint16_t)(B0 + kb);
+        // layer A leaves after this iteration: its used flags are never read again
+        atomicOr(&usedB[kb >> 5], 1u << (kb & 31u));
+        atomicOr(&usedC[ic >> 5], 1u << (ic & 31u));
+        return false;
+      }
+      return true;  // out of track slots: redone by the CTA-per-event kernel
+    };
+
     // ---- T3 + T4 over the list of layer B
-    if (n_t && !overflow) {
+    if (n_t && n_t <= 32 && !overflow) {
+      // A list of one round (55 % of the layers at nu = 6) is resolved in registers: lanes with equal b, a or c find each
+      // other with match_any and compare keys by shuffle — the same minima as below, no shared-memory atomics, no resets.
+      const unsigned long long en = ent0;
+      const uint32_t ia = ((uint32_t)en >> 20) & 0x3FFu, kb = ((uint32_t)en >> 10) & 0x3FFu, ic = (uint32_t)en & 0x3FFu;
+      const bool valid = en != kNoClaim && !((usedA[ia >> 5] >> (ia & 31u)) & 1u) && !((usedB[kb >> 5] >> (kb & 31u)) & 1u) &&
+                         !((usedC[ic >> 5] >> (ic & 31u)) & 1u);
+      // is the lane's key the smallest among the lanes that take part and carry the same `what`?
+      auto holds_min = [&](bool takes_part, uint32_t what, unsigned long long key) {
+        uint32_t peers = __match_any_sync(kFull, takes_part ? what : (0x10000u | lane)) & ~(1u << lane);
+        bool least = takes_part;
+#pragma unroll 1
+        while (__any_sync(kFull, peers != 0)) {
+          const uint32_t src = peers ? (uint32_t)__ffs(peers) - 1u : lane;
+          const unsigned long long other = __shfl_sync(kFull, key, src);
+          if (peers && other < key) least = false;
+          peers &= peers - 1u;
+        }
+        return least;
+      };
+      // T3: argmin per middle hit on (bits(S), a, c); T4: the winner claims its a and its c with (bits(S), b)
+      const bool best = holds_min(valid, kb, (en & 0xFFFFFFFF00000000ull) | (ia << 16) | ic);
+      const unsigned long long tkey = (en & 0xFFFFFFFF00000000ull) | kb;
+      const bool acc = holds_min(best, ia, tkey) & holds_min(best, ic, tkey);
+      const uint32_t accm = __ballot_sync(kFull, acc);
+      if (accm) {
+        uint32_t rank = 0;  // accepted middle hits below this one
+#pragma unroll 1
+        for (uint32_t rest = accm; rest; rest &= rest - 1u) rank += __shfl_sync(kFull, kb, __ffs(rest) - 1) < kb ? 1u : 0u;
+        if (acc) overflow = create_track(en, rank);
+        overflow = __any_sync(kFull, overflow);
+        n_act = min(n_act + (uint32_t)__popc(accm), kSeg);
+        n_created += __popc(accm);
+      }
+      __syncwarp();
+    } else if (n_t && !overflow) {
       const uint32_t rounds = (n_t + 31) / 32;
       auto entry = [&](uint32_t r) -> unsigned long long {
         if (r == 0) return ent0;
@@ -353,31 +413,11 @@ __device__ __forceinline__ void follow_event(const TrackLaunch& a, uint32_t e, F
 #pragma unroll 1
         for (uint32_t r = 0; r < rounds; ++r) {
           const unsigned long long en = entry(r);
-          const uint32_t ia = ((uint32_t)en >> 20) & 0x3FFu, kb = ((uint32_t)en >> 10) & 0x3FFu, ic = (uint32_t)en & 0x3FFu;
+          const uint32_t kb = ((uint32_t)en >> 10) & 0x3FFu;
           const uint32_t below = __shfl_sync(kFull, excl, kb >> 5);
           const uint32_t word = __shfl_sync(kFull, wv, kb >> 5);
           if ((sm.acce[r] >> lane) & 1u) {
-            const uint32_t rank = below + __popc(word & ((1u << (kb & 31u)) - 1u));
-            const uint32_t slot = n_act + rank, cid = n_created + rank;
-            VELO_CHECK(g, 3 * (cid + 1) <= sm.lo[L], 304);  // a track has three hits of its own: slots [co/3, (co+n)/3)
-            if (slot < kSeg) {
-              const Hit hb = load_hit(recB + kb), hc = load_hit(recC + ic);
-              const float dz = __fsub_rn(hc.z, hb.z);
-              sm.ttx[slot] = __fdiv_rn(__fsub_rn(hc.x, hb.x), dz);
-              sm.tty[slot] = __fdiv_rn(__fsub_rn(hc.y, hb.y), dz);
-              const float S = __uint_as_float((uint32_t)(en >> 32));
-              sm.tstate[slot] = ((C0 + ic) << 16) | (S <= P.s_weak ? 0x8000u : 0u) | (3u << 8);
-              sm.tseed[slot] = (uint16_t)(B0 + kb);
-              sm.tcid[slot] = (uint16_t)cid;
-              sm.twin[slot] = pack_windows(__ldg(fwd_win + C0 + ic));
-              link[B0 + kb] = (uint16_t)(A0 + ia);
-              link[C0 + ic] = (uint16_t)(B0 + kb);
-              // layer A leaves after this iteration: its used flags are never read again
-              atomicOr(&usedB[kb >> 5], 1u << (kb & 31u));
-              atomicOr(&usedC[ic >> 5], 1u << (ic & 31u));
-            } else {
-              overflow = true;  // out of track slots: redone by the CTA-per-event kernel
-            }
+            if (create_track(en, below + __popc(word & ((1u << (kb & 31u)) - 1u)))) overflow = true;
           }
         }
         overflow = __any_sync(kFull, overflow);
