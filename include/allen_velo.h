@@ -36,7 +36,9 @@ extern "C" {
 #define ALLEN_VELO_STATUS_TOO_MANY_CLUSTERS 4u  /* > 65535 clusters: clusters written, tracking skipped */
 #define ALLEN_VELO_STATUS_CLUSTER_CAPACITY 8u   /* out_clusters.capacity exceeded: this event's clusters (and tracks) are not written */
 #define ALLEN_VELO_STATUS_TRACK_CAPACITY 16u    /* out_tracks capacities exceeded: this event's tracks not written */
-#define ALLEN_VELO_STATUS_STAGE_OVERFLOW 32u    /* an on-chip staging capacity was exceeded: event incomplete */
+#define ALLEN_VELO_STATUS_STAGE_OVERFLOW 32u    /* a staging capacity was exceeded: event incomplete.  > 8192 SP words in one
+                                                 * layer: that layer's clusters are missing; > 1024 clusters in one layer (or a
+                                                 * workspace smaller than allen_velo_workspace_bytes()): clusters written, no tracks */
 
 /* Cuts of the track search (R5).  The defaults are allen_velo_default_params(). */
 typedef struct {
