@@ -66,6 +66,10 @@ class Geometry:
 
 
 def geometry_g0() -> Geometry:
+    return _pinwheel_stations(STATION_Z, LEFT_DZ_MM)
+
+
+def _pinwheel_stations(station_z, left_dz) -> Geometry:
     # (origin, e_col, e_row) of the four pinwheel sensors of a station: R0, R1 (right module), L0, L1 (left).
     g = HALF_GAP_MM
     frames = [
@@ -74,7 +78,7 @@ def geometry_g0() -> Geometry:
         ((g, -g), (-1.0, 0.0), (0.0, -1.0)),  # L0: col -> -x, row -> -y
         ((-g, -g), (0.0, 1.0), (-1.0, 0.0)),  # L1: col -> +y, row -> -x
     ]
-    n_st = len(STATION_Z)
+    n_st = len(station_z)
     n_modules, n_sensors = 2 * n_st, 4 * n_st
     sensor_module = np.zeros(n_sensors, np.uint16)
     module_layer = np.zeros(n_modules, np.uint16)
@@ -84,7 +88,7 @@ def geometry_g0() -> Geometry:
         for side in range(2):
             m = 2 * k + side
             module_layer[m] = k
-            zm = STATION_Z[k] + (LEFT_DZ_MM if side else 0.0)
+            zm = station_z[k] + (left_dz if side else 0.0)
             for j in range(2):
                 s = 2 * m + j
                 (ox, oy), (ecx, ecy), (erx, ery) = frames[2 * side + j]
@@ -92,6 +96,27 @@ def geometry_g0() -> Geometry:
                 ltg[s] = [ecx, erx, ox, ecy, ery, oy, 0.0, 0.0, zm]
                 frame[s] = [ox, oy, ecx, ecy, erx, ery, zm]
     return Geometry(n_sensors, n_modules, n_st, N_COLS, N_ROWS, PITCH_MM, sensor_module, module_layer, ltg, frame)
+
+
+def geometry_variant(kind: str) -> Geometry:
+    """Other detector descriptions the C ABI admits (include/allen_velo.h: 3 <= n_layers <= 64, at most 8 sensors per
+    layer, other sensor sizes), built from G0's sensor frames; for tests beyond the one geometry the benchmarks use.
+
+    "g52": 52 stations (G0's and one more 12.5 mm behind each, left modules 5 mm behind the right ones): 52 layers;
+    "g13": two stations per layer (13 layers of 8 sensors at four different z);
+    "coarse": G0 with sensors of 384 x 128 pixels of 0.11 mm (same area, a quarter of the pixels).
+    """
+    g = geometry_g0()
+    if kind == "g52":
+        g = _pinwheel_stations(np.sort(np.concatenate([STATION_Z, STATION_Z + 12.5])), 5.0)
+    elif kind == "g13":
+        g.module_layer = (np.arange(g.n_modules, dtype=np.uint16) // 4).astype(np.uint16)
+        g.n_layers = g.n_modules // 4
+    elif kind == "coarse":
+        g.n_cols, g.n_rows, g.pitch_mm = N_COLS // 2, N_ROWS // 2, 2.0 * PITCH_MM
+    else:
+        raise ValueError(kind)
+    return g
 
 
 # ----------------------------------------------------------------------------------------------

@@ -116,3 +116,22 @@ def test_pack_events_matches_generator_packer(geometry):
         events[e].append((int(s), int(c), int(r)))
     raw, off = workload.pack_events(geometry, events)
     assert np.array_equal(off, b.event_offsets) and np.array_equal(raw, b.raw)
+
+
+def test_geometry_variants():
+    """The other detector descriptions of tests/test_gpu_geometries.py: inside what include/allen_velo.h admits, layers
+    numbered by increasing z, and the oracle finds the generated tracks on each of them."""
+    import oracle
+
+    for kind, layers, per_layer in (("g52", 52, 4), ("g13", 13, 8), ("coarse", 26, 4)):
+        g = workload.geometry_variant(kind)
+        assert g.n_layers == layers and 3 <= g.n_layers <= 64
+        lay = g.sensor_layer()
+        assert np.array_equal(np.bincount(lay, minlength=layers), np.full(layers, per_layer))
+        z = g.sensor_ltg[:, 8]
+        zmin = np.array([z[lay == l].min() for l in range(layers)])
+        assert np.all(np.diff(zmin) > 0)
+        assert g.n_cols % 2 == 0 and g.n_rows % 4 == 0 and g.n_cols * g.n_rows <= 1 << 18
+        b = workload.generate(2, n_events=8, geometry=g)
+        r = oracle.reconstruct(g, b.raw, b.event_offsets)
+        assert len(r.tracks.x0) > 8 * 80 and not r.clusters.status.any()
