@@ -325,15 +325,16 @@ def measure_ours(args, headline=True):
     chunk_raw = int(1.25 * raw_bytes * chunk / n_events) + (1 << 20)
     sv = binding.StreamedVelo(geo, chunk, chunk_raw, n_streams=args.e2e_streams, device=device)
     off64 = batch.event_offsets.astype(np.int64)
+    first_chunk = [min(args.e2e_first_chunk, chunk)] if args.e2e_first_chunk > 0 and n_events > chunk else None
     for _ in range(2):
-        infos = sv.reconstruct(h_raw, off64)
+        infos = sv.reconstruct(h_raw, off64, chunk_sizes=first_chunk)
     if sum(i["n_tracks"] for i in infos) != n_tracks:
         raise RuntimeError("streamed reconstruction found a different number of tracks")
     barrier()
     torch.cuda.synchronize()
     e2 = time.time()
     for _ in range(args.steps):
-        sv.reconstruct(h_raw, off64)
+        sv.reconstruct(h_raw, off64, chunk_sizes=first_chunk)
     torch.cuda.synchronize()
     e3 = time.time()
     barrier()
@@ -428,7 +429,8 @@ def measure_ours(args, headline=True):
                     tracks_per_event=n_tracks / n_events, hits_per_track=n_track_hits / max(1, n_tracks),
                     raw_bytes_per_event=raw_bytes / n_events, generator_s=round(t_gen, 2)),
         e2e=dict(value=e2e_value, unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h_holder[0],
-                 ms_per_step=e2e_ms, how=f"binding.StreamedVelo: chunks of {chunk} events on {args.e2e_streams} streams, "
+                 ms_per_step=e2e_ms, how=f"binding.StreamedVelo: chunks of {chunk} events "
+                                         f"{'(the first one ' + str(first_chunk[0]) + ') ' if first_chunk else ''}on {args.e2e_streams} streams, "
                                          "pinned host buffers, H2D raw + offsets and D2H tracks inside the timed region; "
                                          "the clusters stay on the device (P:132: only tracks and vertices are copied back)",
                  single_call=dict(value=single_value, ms_per_step=single_ms) if single_ms else None,
@@ -516,7 +518,9 @@ def main():
                     help="also produce the simple Kalman fit (SURVEY 8(f1), beyond the headline path; +48 B per track)")
     ap.add_argument("--with-vertices", action="store_true",
                     help="also find primary vertices (SURVEY 8(f2), beyond the headline path; implies --with-kalman)")
-    ap.add_argument("--e2e-chunk", type=int, default=2500, help="events per chunk of the streamed end-to-end run")
+    ap.add_argument("--e2e-chunk", type=int, default=3000, help="events per chunk of the streamed end-to-end run")
+    ap.add_argument("--e2e-first-chunk", type=int, default=1000,
+                    help="events of the first chunk when the batch needs several (gets the GPU started early); 0 = e2e-chunk")
     ap.add_argument("--e2e-streams", type=int, default=4)
     ap.add_argument("--sweep", action="store_true",
                     help="also measure BASELINE.json configs[4] (500 / 2k / 50k events) and configs[3] (nu = 12): one line each, "

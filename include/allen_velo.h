@@ -155,6 +155,9 @@ int allen_velo_set_vertex_output(allen_velo_t* handle, const allen_velo_vertices
  *   event_offsets  DEVICE [n_events+1]: byte offset of every event in raw_banks, multiples of 16
  *   cuda_stream    a cudaStream_t (NULL = legacy default stream)
  *   out_clusters / out_tracks  HOST structs of DEVICE pointers; outputs are valid once the stream reaches this point.
+ * The call only enqueues kernels, memsets and event waits (the larger search instances run on streams owned by the
+ * handle that fork from and join `cuda_stream`); it allocates nothing and never waits for the device, so it may be
+ * captured in a CUDA graph (stream capture on `cuda_stream`) and replayed on new contents of the same buffers.
  * Returns ALLEN_VELO_OK, ALLEN_VELO_ERR_INVALID, ALLEN_VELO_ERR_WORKSPACE or ALLEN_VELO_ERR_CUDA (launch failure). */
 int allen_velo_reconstruct(allen_velo_t* handle, const void* raw_banks, const uint32_t* event_offsets,
                            uint32_t n_events, void* cuda_stream,

@@ -377,7 +377,7 @@ class StreamedVelo:
     """
 
     def __init__(self, geometry, chunk_events: int, max_chunk_raw_bytes: int, n_streams: int = 2, device="cuda:0",
-                 params: dict | None = None):
+                 params: dict | None = None, prioritise: bool = False):
         import torch
 
         self.device, self.chunk_events, self.n_layers = torch.device(device), int(chunk_events), geometry.n_layers
@@ -422,24 +422,35 @@ class StreamedVelo:
         s["pending"] = None
         return dict(first_event=p["first"], n_events=n, n_tracks=nt, n_hits=nh)
 
-    def reconstruct(self, h_raw, h_event_offsets, on_chunk=None):
+    def reconstruct(self, h_raw, h_event_offsets, on_chunk=None, chunk_sizes=None):
         """h_raw: pinned uint8 tensor (raw format v1, events back to back); h_event_offsets: int64/int32 numpy array
         [n_events+1].  Calls on_chunk(info, slot) when a chunk's tracks are on their way to the slot's pinned buffers
-        (valid after slot['stream'].synchronize()).  Returns the list of chunk infos."""
+        (valid after slot['stream'].synchronize()).  `chunk_sizes`: events of the first chunks (each <= chunk_events; the
+        rest of the batch goes in chunks of chunk_events) — a short first chunk gets the GPU started while the next
+        ones are still being copied.  Returns the list of chunk infos."""
         import torch
 
         off = np.asarray(h_event_offsets).astype(np.int64)
         n_events = len(off) - 1
         self.h2d_bytes = self.d2h_bytes = 0
         infos = []
-        for k, first in enumerate(range(0, n_events, self.chunk_events)):
+        firsts, at = [], 0
+        for size in list(chunk_sizes or []):
+            if not 0 < int(size) <= self.chunk_events:
+                raise ValueError("chunk_sizes entries must be in [1, chunk_events]")
+            if at < n_events:
+                firsts.append((at, min(at + int(size), n_events)))
+                at = firsts[-1][1]
+        while at < n_events:
+            firsts.append((at, min(at + self.chunk_events, n_events)))
+            at = firsts[-1][1]
+        for k, (first, last) in enumerate(firsts):
             s = self.slots[k % len(self.slots)]
             done = self._finish(s)  # the slot's previous chunk (the other slots keep running meanwhile)
             if done is not None:
                 infos.append(done)
                 if on_chunk:
                     on_chunk(done, s)
-            last = min(first + self.chunk_events, n_events)
             n = last - first
             b0, b1 = int(off[first]), int(off[last])
             if b1 - b0 > self.max_raw:

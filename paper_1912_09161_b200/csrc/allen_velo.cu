@@ -378,6 +378,7 @@ int allen_velo_reconstruct(allen_velo_t* h, const void* raw_banks, const uint32_
 
   CompactTracksLaunch ct{};
   ct.n_events = n_events;
+  ct.n_layers = h->dev.n_layers;
   ct.pitch = h->dev.pitch;
   ct.clusters = *oc;
   ct.hits_slab = hits_slab;

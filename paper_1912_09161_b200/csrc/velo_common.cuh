@@ -199,6 +199,7 @@ cudaError_t cluster_prepare();  // likewise for the cluster kernels
 
 struct CompactTracksLaunch {
   uint32_t n_events;
+  uint32_t n_layers;
   float pitch;  // pixel pitch, mm (measurement error of the Kalman fit)
   allen_velo_clusters_t clusters;
   const uint16_t* hits_slab;

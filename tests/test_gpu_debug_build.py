@@ -76,3 +76,22 @@ def test_stress_inputs_under_bounds_checks(geometry):
         assert np.array_equal(tracks["hits"], ref.tracks.hits)
     finally:
         v.destroy()
+
+
+@pytest.mark.parametrize("kind", ["g52", "g13", "coarse"])
+def test_other_geometries_under_bounds_checks(kind):
+    """52 layers (two layer offsets per lane), 8 sensors per layer, a coarser pixel matrix: no check fails."""
+    import oracle
+    from paper_1912_09161_b200 import binding, build, workload
+
+    build.build(debug=True)
+    geo = workload.geometry_variant(kind)
+    batch = workload.generate(2, n_events=64, geometry=geo)
+    ref = oracle.reconstruct(geo, batch.raw, batch.event_offsets, n_threads=8)
+    v = binding.AllenVelo(geo, debug=True)
+    try:
+        clusters, tracks = binding.reconstruct_batch(v, batch.raw, batch.event_offsets)
+        assert v.debug_fault() == 0
+        assert np.array_equal(clusters["key"], ref.clusters.key) and np.array_equal(tracks["hits"], ref.tracks.hits)
+    finally:
+        v.destroy()

@@ -238,10 +238,20 @@ def test_streamed_host_to_host_reconstruction(geometry, oracle_of):
     sv = binding.StreamedVelo(geometry, 64, int(batch.raw.size), n_streams=3)
     try:
         infos = sv.reconstruct(h_raw, batch.event_offsets.astype(np.int64), on_chunk=on_chunk)
+        assert [i["first_event"] for i in infos] == [0, 64, 128, 192]
+        check_chunks(got, ref.tracks, infos)
+        got.clear()
+        # a short first chunk (bench.py's e2e does this), then a 40-event one, the rest in chunks of 64
+        infos = sv.reconstruct(h_raw, batch.event_offsets.astype(np.int64), on_chunk=on_chunk, chunk_sizes=[8, 40])
+        assert [(i["first_event"], i["n_events"]) for i in infos] == [(0, 8), (8, 40), (48, 64), (112, 64), (176, 24)]
+        check_chunks(got, ref.tracks, infos)
+        with pytest.raises(ValueError):
+            sv.reconstruct(h_raw, batch.event_offsets.astype(np.int64), chunk_sizes=[65])
     finally:
         sv.destroy()
-    assert [i["first_event"] for i in infos] == [0, 64, 128, 192]
-    rt = ref.tracks
+
+
+def check_chunks(got, rt, infos):
     for first, g in got.items():
         n = len(g["te"]) - 1
         t0, t1 = int(rt.event_offsets[first]), int(rt.event_offsets[first + n])
