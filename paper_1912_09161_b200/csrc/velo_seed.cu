@@ -320,7 +320,7 @@ __device__ __forceinline__ void seed_unit(const TrackLaunch& a, SeedWarp& ws, ui
 }
 
 // One warp per (event, layer); the warps of a CTA take consecutive layers of one event (their windows overlap in the L1).
-__global__ void __launch_bounds__(kSeedWarps * 32, 12) velo_seed_kernel(const __grid_constant__ TrackLaunch a) {
+__global__ void __launch_bounds__(kSeedWarps * 32, 10) velo_seed_kernel(const __grid_constant__ TrackLaunch a) {
   __shared__ SeedWarp ws[kSeedWarps];
   const uint32_t unit = blockIdx.x * kSeedWarps + (threadIdx.x >> 5);
   const uint32_t L = a.geo.n_layers;
