@@ -38,7 +38,10 @@
 namespace velo {
 namespace {
 
-constexpr int kWarps = 4;  // warps per CTA (independent work items)
+constexpr int kWarps = 4;  // warps per CTA (independent work items) of the 128-entry instance
+// (the 256-entry instance over ALL items, which busy batches start with, is 2 % faster with two warps per CTA: 4.11 against
+// 4.19 ms at nu = 12; the list instances and the 128-entry instance are faster with four)
+template <uint32_t kCap> struct WarpsOf { static constexpr int v = kCap <= 128 ? kWarps : 2; };
 constexpr uint32_t kDescWords = 18;  // per (event, layer) descriptor written by velo_prepare_kernel
 // per-warp shared memory
 // kCap SP words / clusters / edges per layer, 2 * kCap hash slots; two instances: 256 (nu ~ 6) and 512 (busier batches)
@@ -778,14 +781,15 @@ __device__ __forceinline__ void cluster_item(const ClusterLaunch& a, WarpSmem<kC
 // taking items from a counter, was measured: no gain at 10 000 events, a loss at 1 000).
 constexpr uint32_t kItemsPerWarp = 1;
 template <bool kChecksum, uint32_t kCap, bool kDefer>
-__global__ void __launch_bounds__(kWarps * 32) velo_cluster_kernel(const __grid_constant__ ClusterLaunch a) {
+__global__ void __launch_bounds__(WarpsOf<kCap>::v * 32, kCap <= 128 ? 11 : 1) velo_cluster_kernel(const __grid_constant__ ClusterLaunch a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   using WS = WarpSmem<kChecksum, kCap>;
   WS& ws = reinterpret_cast<WS*>(smem_raw)[threadIdx.x >> 5];
   const uint32_t n = a.n_events * a.geo.n_layers;
 #pragma unroll 1
   for (uint32_t r = 0; r < kItemsPerWarp; ++r) {
-    const uint32_t item = (blockIdx.x * kItemsPerWarp + r) * kWarps + (threadIdx.x >> 5);
+    constexpr uint32_t w = WarpsOf<kCap>::v;
+    const uint32_t item = (blockIdx.x * kItemsPerWarp + r) * w + (threadIdx.x >> 5);
     if (item >= n) return;
     cluster_item<kChecksum, kCap, kDefer>(a, ws, item);
     __syncwarp();
@@ -885,8 +889,10 @@ size_t cluster_big_slot_bytes() { return BigSlot::kBytes; }
 
 template <bool kChecksum, uint32_t kCap, bool kDefer>
 cudaError_t launch_cluster_instance(const ClusterLaunch& a, uint32_t grid, cudaStream_t stream) {
-  const size_t smem = sizeof(WarpSmem<kChecksum, kCap>) * kWarps;
-  velo_cluster_kernel<kChecksum, kCap, kDefer><<<grid, kWarps * 32, smem, stream>>>(a);
+  constexpr uint32_t w = WarpsOf<kCap>::v;
+  const size_t smem = sizeof(WarpSmem<kChecksum, kCap>) * w;
+  grid = (grid * kWarps + w - 1) / w;  // (the caller counts CTAs of kWarps warps)
+  velo_cluster_kernel<kChecksum, kCap, kDefer><<<grid, w * 32, smem, stream>>>(a);
   return cudaGetLastError();
 }
 
@@ -900,8 +906,8 @@ cudaError_t launch_cluster_list(const ClusterLaunch& a, uint32_t grid, cudaStrea
 template <bool kChecksum>
 cudaError_t prepare_cluster_kernels() {
   const auto attr = cudaFuncAttributeMaxDynamicSharedMemorySize;
-  cudaError_t err = cudaFuncSetAttribute(velo_cluster_kernel<kChecksum, 128, true>, attr, (int)sizeof(WarpSmem<kChecksum, 128>) * kWarps);
-  if (err == cudaSuccess) err = cudaFuncSetAttribute(velo_cluster_kernel<kChecksum, 256, true>, attr, (int)sizeof(WarpSmem<kChecksum, 256>) * kWarps);
+  cudaError_t err = cudaFuncSetAttribute(velo_cluster_kernel<kChecksum, 128, true>, attr, (int)sizeof(WarpSmem<kChecksum, 128>) * WarpsOf<128>::v);
+  if (err == cudaSuccess) err = cudaFuncSetAttribute(velo_cluster_kernel<kChecksum, 256, true>, attr, (int)sizeof(WarpSmem<kChecksum, 256>) * WarpsOf<256>::v);
   if (err == cudaSuccess) err = cudaFuncSetAttribute(velo_cluster_list_kernel<kChecksum, 256, true, 0>, attr, (int)sizeof(WarpSmem<kChecksum, 256>) * kWarps);
   if (err == cudaSuccess) err = cudaFuncSetAttribute(velo_cluster_list_kernel<kChecksum, 512, false, 1>, attr, (int)sizeof(WarpSmem<kChecksum, 512>) * kWarps);
   return err;
