@@ -101,11 +101,30 @@ def load_library(debug: bool = False):
         L.allen_velo_debug_fault.restype = ctypes.c_int
         L.allen_velo_debug_checks_compiled.argtypes = []
         L.allen_velo_debug_checks_compiled.restype = ctypes.c_int
+        L.allen_velo_offsets_noalloc.argtypes = [ctypes.c_void_p, ctypes.c_uint32, ctypes.c_void_p, ctypes.c_void_p,
+                                                 ctypes.c_char_p, ctypes.c_size_t]
+        L.allen_velo_offsets_noalloc.restype = ctypes.c_int
         if debug:
             _debug_lib = L
         else:
             _lib = L
     return _debug_lib if debug else _lib
+
+
+NOALLOC_MAX_COUNTS = 4194304  # ALLEN_VELO_NOALLOC_MAX_COUNTS
+ERR_TOO_LARGE = -4
+
+
+def offsets_noalloc(counts, n: int, offsets, stream=None) -> tuple[int, str]:
+    """include/allen_velo_noalloc.h: offsets[0..n] = exclusive prefix sum of counts[0..n) with the scan's scratch in the
+    library's static device array (no handle, no workspace, no allocation).  `counts` / `offsets`: uint32-sized device
+    tensors (int32 views); only pointers are passed.  Returns (return code, error text).  One call at a time per device."""
+    lib = load_library()
+    text = ctypes.create_string_buffer(256)
+    s = ctypes.c_void_p(stream.cuda_stream) if stream is not None else None
+    rc = lib.allen_velo_offsets_noalloc(ctypes.c_void_p(counts.data_ptr()) if counts is not None else None, n,
+                                        ctypes.c_void_p(offsets.data_ptr()) if offsets is not None else None, s, text, 256)
+    return int(rc), text.value.decode()
 
 
 def allen_velo_default_params() -> allen_velo_params_t:

@@ -14,8 +14,11 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "_allen_velo.so")
 LIB_DEBUG = os.path.join(HERE, "_allen_velo_debug.so")  # the same sources with -DVELO_DEBUG (bounds checks)
 SOURCES = ["allen_velo.cu", "velo_cluster.cu", "velo_scan.cu", "velo_track.cu", "velo_seed.cu", "velo_follow.cu", "velo_pv.cu"]
+# include/allen_velo_noalloc.h: its own translation unit (static device scratch array), outside csrc/
+SOURCES.append(os.path.join("..", "csrc_noalloc", "offsets_static.cu"))
 HEADERS = ["velo_common.cuh", "velo_track.cuh", os.path.join("..", "..", "include", "allen_velo.h"),
-           os.path.join("..", "..", "include", "allen_velo_debug.h")]
+           os.path.join("..", "..", "include", "allen_velo_debug.h"),
+           os.path.join("..", "..", "include", "allen_velo_noalloc.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

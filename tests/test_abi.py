@@ -6,7 +6,7 @@ import re
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def declared_functions(headers=("allen_velo.h", "allen_velo_debug.h")):
+def declared_functions(headers=("allen_velo.h", "allen_velo_debug.h", "allen_velo_noalloc.h")):
     names = []
     for h in headers:
         text = open(os.path.join(ROOT, "include", h)).read()
@@ -47,6 +47,12 @@ def test_calls_that_need_no_device():
     assert lib.allen_velo_set_workspace(None, None, 0) == binding.ERR_INVALID
     assert lib.allen_velo_reconstruct(None, None, None, 0, None, None, None) == binding.ERR_INVALID
     lib.allen_velo_destroy(None)
+    # the no-allocation entry point checks its arguments before it touches the device
+    rc, text = binding.offsets_noalloc(None, 5, None)
+    assert rc == binding.ERR_INVALID and "null pointer" in text
+    buf = ctypes.create_string_buffer(256)  # (the pointers are never dereferenced: the size is rejected first)
+    rc = lib.allen_velo_offsets_noalloc(ctypes.c_void_p(256), binding.NOALLOC_MAX_COUNTS + 1, ctypes.c_void_p(512), None, buf, 256)
+    assert rc == binding.ERR_TOO_LARGE and b"exceeds ALLEN_VELO_NOALLOC_MAX_COUNTS = 4194304" in buf.value
 
 
 def test_binding_structs_match_the_header_layout():
@@ -73,3 +79,14 @@ def test_product_path_refuses_to_run_without_cuda(geometry):
         pytest.skip("a CUDA device is present")
     with pytest.raises(RuntimeError, match="no CPU fallback"):
         binding.AllenVelo(geometry)
+
+
+def test_the_no_allocation_entry_point_has_no_allocating_call():
+    """include/allen_velo_noalloc.h promises it: the translation unit holds a static device array, looks its address up
+    with cudaGetSymbolAddress, and calls nothing that allocates."""
+    src = open(os.path.join(ROOT, "paper_1912_09161_b200", "csrc_noalloc", "offsets_static.cu")).read()
+    code = re.sub(r"//[^\n]*", "", re.sub(r"/\*.*?\*/", "", src, flags=re.S))
+    assert re.search(r"static\s+__device__\s+__align__\(256\)\s+unsigned long long\s+g_offsets_state\[", code)
+    assert "cudaGetSymbolAddress" in code
+    for banned in ("cudaMalloc", "cudaFree", "cudaHostAlloc", "cudaMallocAsync", "malloc(", "new ", "std::vector", "std::string"):
+        assert banned not in code, banned
