@@ -104,7 +104,9 @@ def geometry_variant(kind: str) -> Geometry:
 
     "g52": 52 stations (G0's and one more 12.5 mm behind each, left modules 5 mm behind the right ones): 52 layers;
     "g13": two stations per layer (13 layers of 8 sensors at four different z);
-    "coarse": G0 with sensors of 384 x 128 pixels of 0.11 mm (same area, a quarter of the pixels).
+    "coarse": G0 with sensors of 384 x 128 pixels of 0.11 mm (same area, a quarter of the pixels);
+    "shuffled": G0 with the sensors (= raw banks) numbered in a fixed random order, so that the banks of a layer's
+                sensors are scattered over the raw event instead of following one another.
     """
     g = geometry_g0()
     if kind == "g52":
@@ -114,6 +116,11 @@ def geometry_variant(kind: str) -> Geometry:
         g.n_layers = g.n_modules // 4
     elif kind == "coarse":
         g.n_cols, g.n_rows, g.pitch_mm = N_COLS // 2, N_ROWS // 2, 2.0 * PITCH_MM
+    elif kind == "shuffled":
+        perm = np.random.default_rng(20191209).permutation(g.n_sensors)  # new sensor i is G0's sensor perm[i]
+        g.sensor_module = np.ascontiguousarray(g.sensor_module[perm])
+        g.sensor_ltg = np.ascontiguousarray(g.sensor_ltg[perm])
+        g.sensor_frame = np.ascontiguousarray(g.sensor_frame[perm])
     else:
         raise ValueError(kind)
     return g

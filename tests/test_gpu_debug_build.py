@@ -78,7 +78,7 @@ def test_stress_inputs_under_bounds_checks(geometry):
         v.destroy()
 
 
-@pytest.mark.parametrize("kind", ["g52", "g13", "coarse"])
+@pytest.mark.parametrize("kind", ["g52", "g13", "coarse", "shuffled"])
 def test_other_geometries_under_bounds_checks(kind):
     """52 layers (two layer offsets per lane), 8 sensors per layer, a coarser pixel matrix: no check fails."""
     import oracle

@@ -1,7 +1,8 @@
 """Parity on detector descriptions other than G0 (include/allen_velo.h, allen_velo_geometry_t: "3 <= n_layers <= 64; at
 most 8 sensors per layer", other sensor sizes).  The benchmarks use G0 only; the boundary promises more, so the kernels'
 per-layer tables (sensors of a layer, occupancy cells, phi tables, layer offsets held by lane) are exercised here with
-52 layers (two offsets per lane), 8 sensors per layer at four z, and a coarser pixel matrix.  Same bar as
+52 layers (two offsets per lane), 8 sensors per layer at four z, a coarser pixel matrix, and sensors numbered in random
+order (the banks of a layer are then not contiguous in the raw event).  Same bar as
 test_gpu_parity.py: clusters bit-exact, tracks and hit lists identical and in the same order, fit within 1e-5."""
 import numpy as np
 import pytest
@@ -15,6 +16,9 @@ pytestmark = pytest.mark.gpu
     ("g13", None),
     ("coarse", None),
     ("coarse", dict(w_seed_phi16=1500, w_fwd_phi16=1500, max_skipped=2)),
+    # the banks of a layer's sensors are scattered over the raw event: the cluster kernel stages word by word instead
+    # of one contiguous range with 128-bit loads
+    ("shuffled", None),
 ])
 def test_parity_on_other_geometries(kind, params):
     import oracle

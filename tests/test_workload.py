@@ -123,7 +123,7 @@ def test_geometry_variants():
     numbered by increasing z, and the oracle finds the generated tracks on each of them."""
     import oracle
 
-    for kind, layers, per_layer in (("g52", 52, 4), ("g13", 13, 8), ("coarse", 26, 4)):
+    for kind, layers, per_layer in (("g52", 52, 4), ("g13", 13, 8), ("coarse", 26, 4), ("shuffled", 26, 4)):
         g = workload.geometry_variant(kind)
         assert g.n_layers == layers and 3 <= g.n_layers <= 64
         lay = g.sensor_layer()
@@ -135,3 +135,5 @@ def test_geometry_variants():
         b = workload.generate(2, n_events=8, geometry=g)
         r = oracle.reconstruct(g, b.raw, b.event_offsets)
         assert len(r.tracks.x0) > 8 * 80 and not r.clusters.status.any()
+        if kind == "shuffled":  # the sensors of a layer are no longer neighbours in the bank order
+            assert max(np.ptp(np.nonzero(lay == l)[0]) for l in range(layers)) > 50
