@@ -95,3 +95,22 @@ def test_other_geometries_under_bounds_checks(kind):
         assert np.array_equal(clusters["key"], ref.clusters.key) and np.array_equal(tracks["hits"], ref.tracks.hits)
     finally:
         v.destroy()
+
+
+@pytest.mark.parametrize("params", [dict(w_fwd_phi16=16383), dict(w_seed_phi16=16383, w_fwd_phi16=16383),
+                                    dict(max_skipped=4, w_fwd_phi16=1500, s_fwd=0.5)])
+def test_extreme_windows_under_bounds_checks(geometry, params):
+    """Windows of half the circle (velo_follow searches the layer itself), tracks that skip four layers: no check fails."""
+    import oracle
+    from paper_1912_09161_b200 import binding, build, workload
+
+    build.build(debug=True)
+    batch = workload.generate(2, n_events=64, batch_index=2)
+    ref = oracle.reconstruct(geometry, batch.raw, batch.event_offsets, params=params, n_threads=8)
+    v = binding.AllenVelo(geometry, params=params, debug=True)
+    try:
+        _, tracks = binding.reconstruct_batch(v, batch.raw, batch.event_offsets)
+        assert v.debug_fault() == 0
+        assert np.array_equal(tracks["hits"], ref.tracks.hits)
+    finally:
+        v.destroy()

@@ -172,6 +172,12 @@ def test_deterministic_across_runs(velo, oracle_of):
     dict(max_skipped=4, w_fwd_phi16=1500, s_fwd=0.5),
     # tight windows, no weak tracks
     dict(w_seed_phi16=100, w_fwd_phi16=60, s_weak=0.0),
+    # the widest forwarding window the ABI admits (half the circle: more than 63 hits, so velo_follow searches the layer
+    # itself instead of using the packed window), with the default and with the widest seeding window
+    dict(w_fwd_phi16=16383),
+    dict(w_seed_phi16=16383, w_fwd_phi16=16383),
+    # no window at all: only hits at exactly the same phi16
+    dict(w_seed_phi16=0, w_fwd_phi16=0),
 ])
 def test_parity_with_other_cuts(geometry, batch_of, params):
     import oracle
